@@ -1,0 +1,188 @@
+"""ctypes binding of the CPU oracle (oracle/prepos_oracle.c).
+
+TEST INFRASTRUCTURE ONLY.  Importable from tests/, __graft_entry__.smoke() and bench.py's
+cpu_baseline / --impl reference legs; the product package never imports this module and
+this module never imports the product package.
+
+All arithmetic lives in prepos_oracle.c; this file only builds the shared object with gcc,
+marshals arrays, and loops the single-session / single-layer C calls over sessions and layers.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import subprocess
+from dataclasses import dataclass
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "prepos_oracle.c")
+_SO = os.path.join(_HERE, "libprepos_oracle.so")
+
+SERVED, GAP_BELOW_TAU, NOT_IN_FAST_SET, STALE_OR_INVALID, INELIGIBLE = 0, 1, 2, 3, 4
+
+
+def build(force: bool = False) -> str:
+    """Compile the oracle with gcc (-O2, OpenMP over independent outputs)."""
+    if force or not os.path.exists(_SO) or os.path.getmtime(_SO) < os.path.getmtime(_SRC):
+        tmp = _SO + f".{os.getpid()}.tmp"
+        subprocess.check_call(
+            ["gcc", "-O2", "-std=c11", "-fopenmp", "-fPIC", "-shared", "-Wall", "-Wextra",
+             _SRC, "-o", tmp, "-lm"])
+        os.replace(tmp, _SO)
+    return _SO
+
+
+class _Rec(C.Structure):
+    _fields_ = [("max_logit", C.c_double), ("lse", C.c_double), ("gap", C.c_double),
+                ("top1", C.c_int32), ("top2", C.c_int32), ("nonfinite", C.c_int32), ("pad_", C.c_int32)]
+
+
+_lib = None
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        L = C.CDLL(build())
+        p = C.c_void_p
+        L.oracle_entry_attn.restype = C.c_int
+        L.oracle_entry_attn.argtypes = [p, p, p, p, p, p, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int,
+                                        C.c_int, C.c_int, C.c_double, p, p, p]
+        L.oracle_logits.restype = None
+        L.oracle_logits.argtypes = [p, p, C.c_int, C.c_int, p]
+        L.oracle_record.restype = None
+        L.oracle_record.argtypes = [p, C.c_int, C.POINTER(_Rec)]
+        L.oracle_gate.restype = C.c_int
+        L.oracle_gate.argtypes = [C.c_double, C.c_int32, C.c_int, C.c_int, C.c_uint64, C.c_uint64,
+                                  C.c_uint64, C.c_uint64, p, C.c_int, C.c_double, C.c_int, p]
+        L.oracle_invalidate.restype = None
+        L.oracle_invalidate.argtypes = [p, C.c_int, p, p]
+        L.oracle_stamp.restype = None
+        L.oracle_stamp.argtypes = [C.c_int32, p, p, p]
+        L.oracle_fastset_bitmap.restype = None
+        L.oracle_fastset_bitmap.argtypes = [p, C.c_int, C.c_int, p]
+        L.oracle_num_threads.restype = C.c_int
+        _lib = L
+    return _lib
+
+
+def num_threads() -> int:
+    return int(lib().oracle_num_threads())
+
+
+def bf16_bits(t) -> np.ndarray:
+    """torch bf16 tensor (any device) or uint16 ndarray -> contiguous uint16 ndarray of the same bits."""
+    if isinstance(t, np.ndarray):
+        assert t.dtype == np.uint16
+        return np.ascontiguousarray(t)
+    import torch
+    assert t.dtype == torch.bfloat16, t.dtype
+    return t.detach().cpu().contiguous().view(torch.int16).numpy().view(np.uint16)
+
+
+def _ptr(a: np.ndarray):
+    return a.ctypes.data_as(C.c_void_p)
+
+
+def entry_attn(q, k_new, v_new, k_pool, v_pool, page_table, n_s, capacity_tokens, scale=None,
+               want_rowsum=False):
+    """O1 for one session, one layer.  q [L,Hq,d], k_new/v_new [L,Hkv,d], pools [n_pages,Hkv,page,d]
+    (uint16 ndarrays; pools are modified in place by the append).  Returns dict(status, out, rowsum, position)."""
+    L, Hq, d = q.shape
+    Hkv = k_new.shape[1]
+    page = k_pool.shape[2]
+    assert k_pool.dtype == np.uint16 and k_pool.flags.c_contiguous and v_pool.flags.c_contiguous
+    q = np.ascontiguousarray(q)
+    k_new = np.ascontiguousarray(k_new)
+    v_new = np.ascontiguousarray(v_new)
+    pt = np.ascontiguousarray(page_table, dtype=np.int32)
+    out = np.full((L, Hq, d), np.nan, dtype=np.float64)
+    rowsum = np.zeros((L, Hq), dtype=np.float64) if want_rowsum else None
+    pos = np.zeros(1, dtype=np.int64)
+    if scale is None:
+        scale = 1.0 / float(np.sqrt(d))
+    st = lib().oracle_entry_attn(_ptr(q), _ptr(k_new), _ptr(v_new), _ptr(k_pool), _ptr(v_pool), _ptr(pt),
+                                 int(n_s), int(L), int(capacity_tokens), int(Hq), int(Hkv), int(d), int(page),
+                                 float(scale), _ptr(out), _ptr(rowsum) if want_rowsum else None, _ptr(pos))
+    if st < 0:
+        raise ValueError("oracle_entry_attn: bad argument")
+    return {"status": st, "out": out, "rowsum": rowsum, "position": int(pos[0]) if st == 0 else None}
+
+
+def logits(w, x) -> np.ndarray:
+    """O2.  w [V,H] uint16 bits, x [H] uint16 bits -> fp64 [V]."""
+    V, H = w.shape
+    w = np.ascontiguousarray(w)
+    x = np.ascontiguousarray(x)
+    assert x.shape == (H,)
+    out = np.empty(V, dtype=np.float64)
+    lib().oracle_logits(_ptr(w), _ptr(x), V, H, _ptr(out))
+    return out
+
+
+@dataclass
+class Record:
+    max_logit: float
+    lse: float
+    gap: float
+    top1: int
+    top2: int
+    nonfinite: int
+
+
+def record(lg: np.ndarray) -> Record:
+    """O3 from an fp64 logit vector."""
+    lg = np.ascontiguousarray(lg, dtype=np.float64)
+    r = _Rec()
+    lib().oracle_record(_ptr(lg), int(lg.shape[0]), C.byref(r))
+    return Record(r.max_logit, r.lse, r.gap, r.top1, r.top2, r.nonfinite)
+
+
+def fastset_bitmap(ids, V) -> np.ndarray:
+    ids = np.ascontiguousarray(ids, dtype=np.int32)
+    bm = np.zeros((V + 31) // 32, dtype=np.uint32)
+    lib().oracle_fastset_bitmap(_ptr(ids), int(ids.shape[0]), int(V), _ptr(bm))
+    return bm
+
+
+def gate(gap, top1, valid, nonfinite, record_version, session_version, record_hash, request_hash,
+         bitmap, V, tau, strict_gt=False):
+    """O4 for one request -> (decision, token)."""
+    tok = np.zeros(1, dtype=np.int32)
+    bm = np.ascontiguousarray(bitmap, dtype=np.uint32)
+    dec = lib().oracle_gate(float(gap), int(top1), int(bool(valid)), int(bool(nonfinite)),
+                            int(record_version), int(session_version), int(record_hash), int(request_hash),
+                            _ptr(bm), int(V), float(tau), int(bool(strict_gt)), _ptr(tok))
+    return int(dec), int(tok[0])
+
+
+class SessionTable:
+    """O5: the session state machine of Fig. 3 for n sessions -- plain arrays."""
+
+    def __init__(self, n_sessions: int):
+        self.version = np.zeros(n_sessions, dtype=np.uint64)
+        self.rec_version = np.zeros(n_sessions, dtype=np.uint64)
+        self.rec_valid = np.zeros(n_sessions, dtype=np.int32)
+        self.rec_hash = np.zeros(n_sessions, dtype=np.uint64)
+        self.rec_position = np.zeros(n_sessions, dtype=np.int64)
+        self.rec: list = [None] * n_sessions
+
+    def invalidate(self, ids):
+        ids = np.ascontiguousarray(ids, dtype=np.int32)
+        lib().oracle_invalidate(_ptr(ids), int(ids.shape[0]), _ptr(self.version), _ptr(self.rec_valid))
+
+    def preposition(self, sid: int, rec: Record, position: int = 0, entry_hash: int = 0):
+        """Alg. 1 l.10-12: store the record, stamp it with the live version, mark valid."""
+        self.rec[sid] = rec
+        self.rec_hash[sid] = entry_hash
+        self.rec_position[sid] = position
+        lib().oracle_stamp(int(sid), _ptr(self.version), _ptr(self.rec_version), _ptr(self.rec_valid))
+
+    def serve(self, sid: int, bitmap, V, tau, request_hash: int = 0, strict_gt=False):
+        r = self.rec[sid]
+        if r is None:
+            return gate(0.0, -1, False, 0, 0, int(self.version[sid]), 0, request_hash, bitmap, V, tau, strict_gt)
+        return gate(r.gap, r.top1, bool(self.rec_valid[sid]), r.nonfinite, int(self.rec_version[sid]),
+                    int(self.version[sid]), int(self.rec_hash[sid]), request_hash, bitmap, V, tau, strict_gt)

@@ -1,0 +1,217 @@
+"""Seeded synthetic inputs shaped like the paper's streaming and agentic sessions.
+
+This module serves BOTH the CUDA path and the CPU oracle and therefore holds none of the
+method's arithmetic (no attention, no softmax, no top-2 / logsumexp, no gate).  It only draws
+random tensors, lays them out as a paged KV pool with shuffled page tables, and -- for the
+"planted margin" recipe of BASELINE.json configs 1/2/4 -- nudges a hidden state towards one
+row of W_vocab.  The only linear algebra used is a library mat-vec to choose that nudge's scale
+(reading Q14); the realised gap is whatever each side then computes.
+
+These inputs stand in for the paper's binary market-trend streaming task and its agentic
+tool-calling workload, whose data is not available.
+"""
+from __future__ import annotations
+
+import math
+from dataclasses import dataclass, field, replace
+from typing import Optional
+
+import torch
+
+SEED_BASE = 20260629  # seed = SEED_BASE + config index
+
+
+@dataclass(frozen=True)
+class Shape:
+    """Model-side shape of a workload (BASELINE.json `configs`)."""
+    name: str
+    layers: int
+    Hq: int
+    Hkv: int
+    d: int
+    H: int
+    V: int
+    page: int = 16
+    fast_set: int = 16
+    tau: float = 3.0
+    planted_frac: float = 0.5
+
+    @property
+    def G(self) -> int:
+        return self.Hq // self.Hkv
+
+
+# BASELINE.json configs[0..4]
+C1 = Shape("c1_tiny", layers=1, Hq=4, Hkv=2, d=64, H=256, V=1024, fast_set=16, tau=3.0, planted_frac=0.5)
+C2 = Shape("c2_8b_stream", layers=32, Hq=32, Hkv=8, d=128, H=4096, V=128256, fast_set=64, tau=3.0, planted_frac=0.6)
+C3 = replace(C2, name="c3_8b_long")
+C4 = replace(C2, name="c4_agentic")
+C5 = Shape("c5_70b", layers=80, Hq=64, Hkv=8, d=128, H=8192, V=128256, fast_set=256, tau=4.0, planted_frac=0.6)
+
+
+def gen(seed: int, device="cpu") -> torch.Generator:
+    g = torch.Generator(device=device)
+    g.manual_seed(int(seed))
+    return g
+
+
+def randn_bf16(shape, g: torch.Generator, std: float = 1.0, chunk_elems: int = 1 << 28) -> torch.Tensor:
+    """N(0, std^2) rounded to bf16, drawn in fp32 chunks so multi-GB pools do not need an fp32 copy."""
+    device = g.device
+    out = torch.empty(shape, dtype=torch.bfloat16, device=device)
+    flat = out.view(-1)
+    n = flat.numel()
+    for lo in range(0, n, chunk_elems):
+        hi = min(n, lo + chunk_elems)
+        t = torch.randn(hi - lo, generator=g, device=device, dtype=torch.float32)
+        if std != 1.0:
+            t.mul_(std)
+        flat[lo:hi] = t.to(torch.bfloat16)
+    return out
+
+
+@dataclass
+class SessionBatch:
+    """A batch of sessions sharing one paged pool per layer (device tensors)."""
+    shape: Shape
+    n_s: list               # cached tokens per session (host ints)
+    l_entry: list           # entry tokens per session (host ints)
+    capacity: list          # tokens the session's page table can hold (host ints)
+    page_table: torch.Tensor  # [n_sessions, stride] int32, physical page ids (shuffled)
+    k_pool: torch.Tensor    # [layers, n_pages, Hkv, page, d] bf16
+    v_pool: torch.Tensor
+    q: torch.Tensor         # [layers, sum_L, Hq, d] bf16
+    k_new: torch.Tensor     # [layers, sum_L, Hkv, d] bf16
+    v_new: torch.Tensor
+    row_offset: list = field(default_factory=list)  # start row of each session in the packed sum_L axis
+
+    @property
+    def n_sessions(self) -> int:
+        return len(self.n_s)
+
+    @property
+    def sum_l(self) -> int:
+        return int(sum(self.l_entry))
+
+
+def make_sessions(shape: Shape, n_s, l_entry, seed: int, device="cpu", layers: Optional[int] = None,
+                  extra_pages: int = 0, shuffle_pages: bool = True, tight_capacity=None) -> SessionBatch:
+    """Paged bf16 KV pool, N(0,1) K/V/Q, one shuffled page table over all sessions.
+
+    Every session gets ceil((n_s+L)/page) pages (+ extra_pages); `tight_capacity[s]` (tokens), when
+    given, overrides its capacity so the Alg. 1 l.2 budget skip can be exercised.
+    """
+    layers = shape.layers if layers is None else layers
+    g = gen(seed, device)
+    n_s = [int(v) for v in n_s]
+    l_entry = [int(v) for v in l_entry]
+    page = shape.page
+    pages_per = [max(1, -(-(a + b) // page)) + extra_pages for a, b in zip(n_s, l_entry)]
+    n_pages = sum(pages_per)
+    stride = max(pages_per)
+    gc = gen(seed + 7919, "cpu")
+    perm = torch.randperm(n_pages, generator=gc) if shuffle_pages else torch.arange(n_pages)
+    table = torch.zeros((len(n_s), stride), dtype=torch.int32)
+    off = 0
+    for s, pp in enumerate(pages_per):
+        table[s, :pp] = perm[off:off + pp].to(torch.int32)
+        off += pp
+    capacity = [pp * page for pp in pages_per]
+    if tight_capacity is not None:
+        capacity = [int(c) if c is not None else cap for c, cap in zip(tight_capacity, capacity)]
+    k_pool = randn_bf16((layers, n_pages, shape.Hkv, page, shape.d), g)
+    v_pool = randn_bf16((layers, n_pages, shape.Hkv, page, shape.d), g)
+    sum_l = sum(l_entry)
+    q = randn_bf16((layers, sum_l, shape.Hq, shape.d), g)
+    k_new = randn_bf16((layers, sum_l, shape.Hkv, shape.d), g)
+    v_new = randn_bf16((layers, sum_l, shape.Hkv, shape.d), g)
+    row_offset, acc = [], 0
+    for le in l_entry:
+        row_offset.append(acc)
+        acc += le
+    return SessionBatch(shape, n_s, l_entry, capacity, table.to(device), k_pool, v_pool, q, k_new, v_new, row_offset)
+
+
+def make_w_vocab(shape: Shape, seed: int, device="cpu") -> torch.Tensor:
+    """W_vocab ~ N(0, 1/H) i.e. std = 1/sqrt(H) (reading Q13), bf16 [V, H]."""
+    return randn_bf16((shape.V, shape.H), gen(seed + 101, device), std=1.0 / math.sqrt(shape.H))
+
+
+def make_fast_set(shape: Shape, seed: int) -> torch.Tensor:
+    """|A| distinct seeded token ids (host int32, sorted)."""
+    g = gen(seed + 202, "cpu")
+    return torch.randperm(shape.V, generator=g)[: shape.fast_set].sort().values.to(torch.int32)
+
+
+def make_hidden(shape: Shape, n: int, w_vocab: torch.Tensor, fast_ids: torch.Tensor, seed: int,
+                planted_frac: Optional[float] = None):
+    """n hidden states ~ N(0,1) bf16; a `planted_frac` share is nudged towards a fast-set row of W.
+
+    Planting (reading Q14): pick a in A and a target g* ~ U(1,6); set x' = bf16(x + alpha * W[a]) with
+    alpha from three fixed-point steps of alpha <- (g* + max_{v!=a}(W x')_v - (W x)_a) / |W[a]|^2, all in
+    fp64 through a library mat-vec.  g* is only the generator's aim.  Returns (hidden [n,H] bf16,
+    planted mask [n] bool, target gaps [n] float64 (nan where unplanted)).
+    """
+    device = w_vocab.device
+    g = gen(seed + 303, device)
+    gc = gen(seed + 404, "cpu")
+    frac = shape.planted_frac if planted_frac is None else planted_frac
+    hidden = randn_bf16((n, shape.H), g)
+    planted = torch.rand(n, generator=gc) < frac
+    target = torch.full((n,), float("nan"), dtype=torch.float64)
+    w64 = None
+    for r in range(n):
+        if not bool(planted[r]):
+            continue
+        a = int(fast_ids[int(torch.randint(0, fast_ids.numel(), (1,), generator=gc))])
+        gstar = 1.0 + 5.0 * float(torch.rand(1, generator=gc))
+        target[r] = gstar
+        if w64 is None:
+            w64 = w_vocab.to(torch.float64) if w_vocab.numel() <= (1 << 26) else None
+        wa = w_vocab[a].to(torch.float64)
+        x0 = hidden[r].to(torch.float64)
+        wa2 = float(wa.dot(wa))
+        alpha = 0.0
+        xp = hidden[r]
+        for _ in range(3):
+            xq = xp.to(torch.float64)
+            lg = (w64 @ xq) if w64 is not None else _chunked_mv(w_vocab, xq)
+            la0 = float(w_vocab[a].to(torch.float64).dot(x0))
+            lg[a] = -float("inf")
+            alpha = (gstar + float(lg.max()) - la0) / wa2
+            xp = (x0 + alpha * wa).to(torch.bfloat16)
+        hidden[r] = xp
+    return hidden, planted, target
+
+
+def _chunked_mv(w: torch.Tensor, x64: torch.Tensor, rows: int = 16384) -> torch.Tensor:
+    out = torch.empty(w.shape[0], dtype=torch.float64, device=w.device)
+    for lo in range(0, w.shape[0], rows):
+        out[lo:lo + rows] = w[lo:lo + rows].to(torch.float64) @ x64
+    return out
+
+
+def lognormal_ns(n: int, seed: int, lo: int = 1024, hi: int = 16384, median: float = 4096.0, sigma: float = 0.75):
+    """Config 4 cached lengths: clip(round(exp(N(ln median, sigma^2))), lo, hi) (reading Q15)."""
+    g = gen(seed + 505, "cpu")
+    z = torch.randn(n, generator=g, dtype=torch.float64)
+    v = torch.exp(math.log(median) + sigma * z).round().clamp(lo, hi)
+    return [int(t) for t in v]
+
+
+def uniform_l(n: int, seed: int, lo: int = 32, hi: int = 96):
+    """Config 4 post-tool-call entry lengths L ~ U{lo..hi}."""
+    g = gen(seed + 606, "cpu")
+    return [int(t) for t in torch.randint(lo, hi + 1, (n,), generator=g)]
+
+
+def bump_trace(n_steps: int, seed: int, p_bump: float = 0.3):
+    """Config 3 update trace: per step, True = the update bumps the state version (reading Q16)."""
+    g = gen(seed + 707, "cpu")
+    return [bool(t) for t in (torch.rand(n_steps, generator=g) < p_bump)]
+
+
+def serve_requests(n_requests: int, n_sessions: int, seed: int) -> torch.Tensor:
+    """Config 4 gate-serve batch: session ids ~ U{0..n_sessions-1} (host int32)."""
+    g = gen(seed + 808, "cpu")
+    return torch.randint(0, n_sessions, (n_requests,), generator=g).to(torch.int32)
