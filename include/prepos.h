@@ -1,0 +1,206 @@
+/*
+ * prepos.h -- C ABI of libprepos: the data-parallel hot path of speculative pre-positioning
+ * (arxiv/paper_2606_29565; citations are PAPER.md:<line> of the paper text) on one B200 (sm_100a).
+ *
+ * The calls follow the paper's problem statement (Alg. 1 PAPER.md:140-164,
+ * Alg. 2, Sec. 3.6):
+ *
+ *   prepos_entry_attn   Alg. 1 l.2-6: budget check, Append(E), attention part of Forward(E)
+ *   prepos_ready_dist   Alg. 1 l.6 (LM head at the last entry position) + l.10-12 (record)
+ *                       + Alg. 2 l.3-4 (Top2, gamma, argmax) moved to pre-position time
+ *   prepos_scan_logits  Alg. 2 l.3-4 on a stored logit vector: the serve-time T_scan(V), Eq. 3
+ *   prepos_gate_serve   Alg. 2, batched: validity/eligibility, Eq. 12 gate, serve or fall through
+ *   prepos_invalidate   Sec. 3.6: version bump + valid clear in the step that mutates the state
+ *
+ * Conventions
+ *   - Every call returns an int status: 0 = PREPOS_OK, > 0 informational, < 0 error.  No exceptions,
+ *     no exit(), no memory handed to the caller.  prepos_strerror() names a status.
+ *   - Pointers marked DEVICE are device pointers owned by the caller (16-byte aligned); pointers marked
+ *     HOST are ordinary host memory, read (or written) before the call returns.  The library never
+ *     allocates, frees, evicts or resizes caller memory ("skips the pre-position rather
+ *     than evicting live state").  It owns only the opaque prepos_ctx, whose device scratch is the
+ *     caller-supplied workspace.
+ *   - Launches are asynchronous on `stream` (a cudaStream_t passed as void*; NULL = the legacy default
+ *     stream) and stream-ordered with each other.  An asynchronous CUDA fault surfaces as PREPOS_E_CUDA
+ *     on a later call or on prepos_ctx_sync().
+ *   - bf16 tensors are raw 16-bit patterns (void*).  All accumulation and every record field is fp32.
+ *   - A ctx is not thread-safe; use one ctx per host thread / stream.
+ */
+#ifndef PREPOS_H_
+#define PREPOS_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define PREPOS_VERSION 100 /* 0.1.0 */
+
+/* status codes */
+enum {
+    PREPOS_OK = 0,
+    PREPOS_SKIPPED_BUDGET = 1, /* Alg. 1 l.2-3: L_entry > headroom; nothing was touched */
+    PREPOS_E_INVALID_ARG = -1,
+    PREPOS_E_SHAPE = -2,     /* shape outside what the kernels support (see prepos_ctx_create) */
+    PREPOS_E_ALIGN = -3,     /* a device pointer or stride is not 16-byte aligned */
+    PREPOS_E_CUDA = -4,      /* a CUDA runtime/driver call or an earlier kernel failed */
+    PREPOS_E_WORKSPACE = -5, /* the workspace given to prepos_ctx_create is too small for this call */
+    PREPOS_E_NO_DEVICE = -6  /* no sm_100 device / driver: there is no CPU fallback */
+};
+
+/* serve decisions written by prepos_gate_serve (Alg. 2) */
+enum {
+    PREPOS_SERVED = 0,           /* l.6: one cached token returned, scheduler bypassed */
+    PREPOS_GAP_BELOW_TAU = 1,    /* l.9: gamma < tau (or <= tau when strict) */
+    PREPOS_NOT_IN_FAST_SET = 2,  /* l.9: argmax not in A */
+    PREPOS_STALE_OR_INVALID = 3, /* l.1-2: no valid record for the live state version */
+    PREPOS_INELIGIBLE = 4        /* l.1-2: realised entry != pre-positioned entry */
+};
+
+/* record flag bits */
+#define PREPOS_FLAG_VALID 1u     /* Alg. 1 l.12 decoded/valid */
+#define PREPOS_FLAG_NONFINITE 2u /* a logit was NaN/Inf: never served */
+
+typedef struct prepos_ctx prepos_ctx;
+
+typedef struct {
+    int32_t layers;     /* KV layers */
+    int32_t n_q_heads;  /* Hq */
+    int32_t n_kv_heads; /* Hkv, divides Hq; query head h reads kv head h / (Hq/Hkv) */
+    int32_t head_dim;   /* d: multiple of 8, <= 256.  d in {64,128} with page_size 16 takes the tcgen05 path */
+    int32_t hidden;     /* H: multiple of 256 */
+    int32_t vocab;      /* V >= 2 */
+    int32_t page_size;  /* tokens per KV page (power of two, <= 128) */
+} prepos_model_shape;
+
+/*
+ * The ready-distribution record kept on the session ("or only
+ * (argmax, gamma) under the gate").  48 bytes, 16-byte aligned, one per session id.
+ */
+typedef struct {
+    float max_logit;     /* l^(1) */
+    float lse;           /* log sum_v exp(l_v), natural log */
+    int32_t top1;        /* argmax(l_ready): ties -> lowest id */
+    int32_t top2;        /* id of l^(2) under the order (logit desc, id asc) */
+    float gap;           /* gamma = l^(1) - l^(2), Eq. 11 */
+    uint32_t flags;      /* PREPOS_FLAG_* */
+    uint64_t version;    /* session state version the record was computed at */
+    uint64_t entry_hash; /* caller's hash of the pre-positioned entry tokens; 0 = relaxed match */
+    int64_t position;    /* decision point p = n_s + L_entry, Eq. 1 */
+} prepos_record;
+
+const char *prepos_strerror(int status);
+int prepos_version(void);
+
+/* Bytes of device workspace a ctx needs to serve calls of up to max_sessions sessions per call. */
+size_t prepos_workspace_bytes(const prepos_model_shape *shape, int max_sessions);
+
+/*
+ * Creates a context bound to the current CUDA device.  `workspace` (DEVICE, 256-byte aligned,
+ * workspace_bytes >= prepos_workspace_bytes()) stays owned by the caller and must outlive the ctx.
+ * Errors: PREPOS_E_NO_DEVICE, PREPOS_E_SHAPE, PREPOS_E_WORKSPACE, PREPOS_E_ALIGN, PREPOS_E_CUDA.
+ */
+int prepos_ctx_create(prepos_ctx **out, const prepos_model_shape *shape, int max_sessions,
+                      void *workspace, size_t workspace_bytes);
+int prepos_ctx_destroy(prepos_ctx *ctx);
+/* cudaStreamSynchronize(stream) + report any pending asynchronous error. */
+int prepos_ctx_sync(prepos_ctx *ctx, void *stream);
+/* Number of libprepos kernels launched through this ctx since creation (for accounting). */
+int64_t prepos_ctx_launch_count(const prepos_ctx *ctx);
+/* Tuning knob: 0 = automatic; 1 = force the generic CUDA-core attention kernel; 2 = force tcgen05. */
+int prepos_ctx_set_attn_path(prepos_ctx *ctx, int path);
+
+/*
+ * Alg. 1 l.2-6 for layers [layer_begin, layer_end) over a batch of sessions.
+ *
+ * For every session s, layer l, query head h and entry row i in [0, L_s): softmax over the cached
+ * tokens j < n_s[s] (read through the page table) and the entry tokens j' <= i ("causal among
+ * themselves") of (q_i . k_j) * scale, times V -- and the entry K/V are written into the session's
+ * pages at positions n_s .. n_s+L_s-1 (Append(E), l.5).  The decision point is p = n_s + L_s (Eq. 1);
+ * the caller advances its own n_s after the call.
+ *
+ * q, out     DEVICE bf16 [layer][sum_L][Hq][d]; rows of session s start at sum_{t<s} L_t; layer l at
+ *            base + l * q_layer_stride elements (out: out_layer_stride)
+ * k_new,v_new DEVICE bf16 [layer][sum_L][Hkv][d], layer stride kv_new_layer_stride elements
+ * k_pool,v_pool DEVICE bf16 [layer][n_pages][Hkv][page_size][d], layer stride pool_layer_stride elements
+ * page_table DEVICE int32 [n_sessions][page_table_stride]: physical page of logical page t of session s
+ * n_s, l_entry, capacity_tokens  HOST int32 [n_sessions]: cached tokens, entry tokens, tokens the
+ *            session's pages can hold (cell budget: headroom B = capacity - n_s)
+ * status_per_session HOST int32 [n_sessions] (nullable): PREPOS_OK or PREPOS_SKIPPED_BUDGET.  A skipped
+ *            session has no side effect at all: its pages and its rows of `out` are untouched.
+ * softmax_scale  <= 0 means 1/sqrt(d)
+ *
+ * Returns PREPOS_OK (also when some sessions were skipped) or an error; on error nothing was launched.
+ */
+int prepos_entry_attn(prepos_ctx *ctx, int layer_begin, int layer_end, int n_sessions,
+                      const void *q, int64_t q_layer_stride,
+                      const void *k_new, const void *v_new, int64_t kv_new_layer_stride,
+                      void *k_pool, void *v_pool, int64_t pool_layer_stride, int64_t n_pages,
+                      const int32_t *page_table, int page_table_stride,
+                      const int32_t *n_s, const int32_t *l_entry, const int32_t *capacity_tokens,
+                      void *out, int64_t out_layer_stride,
+                      int32_t *status_per_session, float softmax_scale, void *stream);
+
+/*
+ * Alg. 1 l.6 (LM head) + l.10-12 and Alg. 2 l.3-4 (Eq. 11):
+ * logits l_v = sum_k W[v][k] x_r[k] for each of n hidden rows, reduced in the same pass to the
+ * record {max, lse, top1, top2, gap} under the order (logit desc, id asc).  records[session_ids[r]]
+ * is overwritten: version = session_version[session_ids[r]] (the live version at pre-position
+ * time), flags = VALID (| NONFINITE), position = position_p[r] (0 if NULL), entry_hash likewise.
+ * skip_mask (DEVICE int32 [n], nullable): rows with a non-zero entry are left untouched (sessions
+ * whose pre-position was skipped on budget; their record is NOT made valid).
+ *
+ * hidden DEVICE bf16 [n][H]; w_vocab DEVICE bf16 [V][H] row-major; session_ids DEVICE int32 [n];
+ * position_p DEVICE int64 [n] nullable; entry_hash DEVICE uint64 [n] nullable;
+ * records DEVICE (indexed by session id); session_version DEVICE uint64 (indexed by session id);
+ * logits_out DEVICE fp32 [n][V] nullable (the full ready distribution).
+ */
+int prepos_ready_dist(prepos_ctx *ctx, int n, const int32_t *session_ids,
+                      const void *hidden, const void *w_vocab,
+                      const int64_t *position_p, const uint64_t *entry_hash, const int32_t *skip_mask,
+                      prepos_record *records, const uint64_t *session_version,
+                      float *logits_out, void *stream);
+
+/*
+ * Alg. 2 l.3-4 on stored logits (the paper's serve-time vocabulary scan, Eq. 3):
+ * out[r] gets max_logit, lse, top1, top2, gap and the NONFINITE flag from logits[r][0..V); the other
+ * fields of out[r] (version, entry_hash, position, VALID bit) are left as they are.
+ * logits DEVICE fp32 [n][V]; out DEVICE [n].
+ */
+int prepos_scan_logits(prepos_ctx *ctx, int n, const float *logits, prepos_record *out, void *stream);
+
+/*
+ * Alg. 2, batched.  For request r on session sid = session_ids[r]:
+ *   records[sid] not VALID, NONFINITE, or records[sid].version != session_version[sid] -> STALE_OR_INVALID
+ *   both hashes non-zero and different                                               -> INELIGIBLE
+ *   top1 not in A                                                                    -> NOT_IN_FAST_SET
+ *   gap < tau (strict_gt: gap <= tau, the paper's Eq. 12 form)                        -> GAP_BELOW_TAU
+ *   otherwise SERVED with token_out[r] = top1.  token_out[r] = -1 unless SERVED.
+ * All arrays DEVICE.  request_entry_hash nullable (= all relaxed).  fast_set_bitmap: ceil(V/32) words,
+ * bit (id & 31) of word (id >> 5).  The version compare is the authority (Sec. 3.6): a record whose
+ * session was invalidated earlier in stream order is never served.
+ */
+int prepos_gate_serve(prepos_ctx *ctx, int n_requests, const int32_t *session_ids,
+                      const uint64_t *request_entry_hash,
+                      const prepos_record *records, const uint64_t *session_version,
+                      const uint32_t *fast_set_bitmap, float tau, int strict_gt,
+                      int32_t *decision_out, int32_t *token_out, void *stream);
+
+/*
+ * Sec. 3.6: for every listed session (ids may repeat; each occurrence is one
+ * mutation) session_version[sid] += 1 and records[sid].flags &= ~VALID.  Call it on the stream, and
+ * in the step, that performs the mutation; later serves on that stream see the bump.
+ * session_ids DEVICE int32 [n]; session_version, records DEVICE.
+ */
+int prepos_invalidate(prepos_ctx *ctx, int n, const int32_t *session_ids,
+                      uint64_t *session_version, prepos_record *records, void *stream);
+
+/* HOST helper: A as a bitmap.  ids HOST int32 [n]; bitmap_host HOST uint32 [ceil(V/32)] (overwritten). */
+int prepos_fastset_build(const int32_t *ids, int n, int V, uint32_t *bitmap_host);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PREPOS_H_ */

@@ -1,0 +1,115 @@
+// common.cuh -- shared declarations of libprepos' translation units (CUDA side only; the CPU oracle
+// under oracle/ shares nothing with this tree).
+#pragma once
+
+#include <cuda.h>
+#include <cuda_bf16.h>
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include <vector>
+
+#include "../../include/prepos.h"
+
+static_assert(sizeof(prepos_record) == 48, "prepos_record must be 48 bytes");
+
+#define PREPOS_CUDA_TRY(expr)                                  \
+    do {                                                       \
+        cudaError_t e_ = (expr);                               \
+        if (e_ != cudaSuccess) {                               \
+            prepos_note_cuda_error(e_, #expr, __FILE__, __LINE__); \
+            return PREPOS_E_CUDA;                              \
+        }                                                      \
+    } while (0)
+
+void prepos_note_cuda_error(cudaError_t e, const char *what, const char *file, int line);
+
+constexpr int kMaxRdPartials = 1024;  // CTAs of a ready-dist launch (upper bound on its grid)
+constexpr int kRdMaxRows = 128;       // hidden rows reduced by one ready-dist launch
+constexpr int kAttnTileTokens = 128;  // KV tokens per tile of the tcgen05 attention kernel
+constexpr int kAttnMaxRows = 256;     // query rows (G * entry tokens) per attention unit
+constexpr int kAttnMaxCtas = 1024;    // upper bound on the persistent attention grid
+
+// per-CTA partial of the vocabulary reduction (a4): merged under the order (logit desc, id asc)
+struct RdPartial {
+    float m;   // running max
+    float s;   // sum exp(l - m)
+    float v1;  // best logit
+    float v2;  // second best
+    int32_t i1;
+    int32_t i2;
+    int32_t nonfinite;
+    int32_t pad;
+};
+static_assert(sizeof(RdPartial) == 32, "RdPartial");
+
+// one (session, row-chunk) of an attention call; (layer, kv head) are grid dimensions on top of it
+struct AttnUnit {
+    int32_t session;      // index in the call's batch
+    int32_t n_s;          // cached tokens
+    int32_t l_entry;      // entry tokens of the session
+    int32_t tok0;         // first entry token of this row chunk
+    int32_t ntok;         // entry tokens in this chunk (rows = ntok * G)
+    int32_t row0;         // session's first row in the packed sum_L axis
+    int32_t n_cached_tiles;  // ceil(n_s / tile)
+    int32_t n_tiles;      // cached tiles + new-token tiles visible to this chunk
+    int32_t tile_prefix;  // sum of n_tiles of the units before this one (within one (layer, head))
+    int32_t pad[3];
+};
+static_assert(sizeof(AttnUnit) == 48, "AttnUnit");
+
+struct prepos_ctx {
+    prepos_model_shape shape;
+    int max_sessions;
+    int device;
+    int num_sms;
+    int cc_major, cc_minor;
+    char *ws;
+    size_t ws_bytes;
+    int64_t launches;
+    int attn_path;
+    // workspace carve-up (device pointers into ws)
+    RdPartial *rd_partials;    // [kRdMaxRows][kMaxRdPartials]
+    unsigned int *rd_counter;  // arrival counter of the cross-CTA pass (self-resetting)
+    AttnUnit *attn_units;      // device copy of the plan
+    int max_units;
+    float *attn_partials;      // [2 * kAttnMaxCtas] slots of kAttnMaxRows * (d + 2) floats
+    unsigned int *attn_counters;  // [layers * Hkv * max_units] arrival counters (self-resetting)
+    size_t attn_counters_n;
+    // host-side plan cache
+    std::vector<AttnUnit> plan_units;
+    std::vector<int32_t> plan_key;
+    AttnUnit *plan_staging;  // pinned host staging for the H2D plan copy
+    cudaEvent_t plan_copied;
+    bool plan_inflight;
+    // TMA descriptor cache for the KV pools
+    void *tm_k_ptr, *tm_v_ptr;
+    int64_t tm_layer_stride, tm_n_pages;
+    CUtensorMap tm_k, tm_v;
+};
+
+// ---- per-file launchers (all return a PREPOS_* status) -------------------------------------------
+int prepos_launch_ready_dist(prepos_ctx *ctx, int n, const int32_t *session_ids, const __nv_bfloat16 *hidden,
+                             const __nv_bfloat16 *w, const int64_t *position_p, const uint64_t *entry_hash,
+                             const int32_t *skip_mask, prepos_record *records, const uint64_t *session_version,
+                             float *logits_out, cudaStream_t stream);
+int prepos_launch_scan_logits(prepos_ctx *ctx, int n, const float *logits, prepos_record *out, cudaStream_t stream);
+int prepos_launch_gate_serve(prepos_ctx *ctx, int n, const int32_t *session_ids, const uint64_t *req_hash,
+                             const prepos_record *records, const uint64_t *session_version,
+                             const uint32_t *bitmap, float tau, int strict_gt, int32_t *decision, int32_t *token,
+                             cudaStream_t stream);
+int prepos_launch_invalidate(prepos_ctx *ctx, int n, const int32_t *session_ids, uint64_t *session_version,
+                             prepos_record *records, cudaStream_t stream);
+
+struct AttnArgs {
+    int layer_begin, layer_end, n_units;
+    const __nv_bfloat16 *q, *k_new, *v_new;
+    __nv_bfloat16 *k_pool, *v_pool, *out;
+    int64_t q_layer_stride, kv_new_layer_stride, pool_layer_stride, out_layer_stride, n_pages;
+    const int32_t *page_table;
+    int page_table_stride;
+    float scale;
+};
+int prepos_launch_attn_generic(prepos_ctx *ctx, const AttnArgs &a, cudaStream_t stream);
+int prepos_launch_attn_umma(prepos_ctx *ctx, const AttnArgs &a, int total_tiles_per_lh, cudaStream_t stream);
+bool prepos_attn_umma_supported(const prepos_ctx *ctx);

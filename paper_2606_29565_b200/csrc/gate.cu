@@ -1,0 +1,88 @@
+// gate.cu -- the serve-side kernels: batched confidence gate (Alg. 2; Eq. 12,
+// PAPER.md:111) and invalidation (Sec. 3.6).  Both are a handful of bytes per
+// request: launch-latency bound, one thread per request.
+#include "common.cuh"
+
+namespace {
+
+// Alg. 2 for one request.  The record is read as three 16-byte words; the version compare is the
+// authority for staleness (reading Q11), the VALID bit is redundant with it.
+__global__ void __launch_bounds__(128) gate_serve_kernel(int n, const int32_t *__restrict__ session_ids,
+                                                         const uint64_t *__restrict__ req_hash,
+                                                         const prepos_record *__restrict__ records,
+                                                         const uint64_t *__restrict__ session_version,
+                                                         const uint32_t *__restrict__ bitmap, int vocab, float tau,
+                                                         int strict_gt, int32_t *__restrict__ decision,
+                                                         int32_t *__restrict__ token)
+{
+    const int r = blockIdx.x * blockDim.x + threadIdx.x;
+    if (r >= n) return;
+    const int sid = session_ids[r];
+    const uint4 *p = reinterpret_cast<const uint4 *>(records + sid);
+    const uint4 w0 = p[0];  // max_logit, lse, top1, top2
+    const uint4 w1 = p[1];  // gap, flags, version
+    const uint4 w2 = p[2];  // entry_hash, position
+    const int32_t top1 = static_cast<int32_t>(w0.z);
+    const float gap = __uint_as_float(w1.x);
+    const uint32_t flags = w1.y;
+    const uint64_t rec_version = (static_cast<uint64_t>(w1.w) << 32) | w1.z;
+    const uint64_t rec_hash = (static_cast<uint64_t>(w2.y) << 32) | w2.x;
+    const uint64_t live = session_version[sid];
+    const uint64_t rh = req_hash ? req_hash[r] : 0ull;
+
+    int dec;
+    if (!(flags & PREPOS_FLAG_VALID) || (flags & PREPOS_FLAG_NONFINITE) || rec_version != live) {
+        dec = PREPOS_STALE_OR_INVALID;  // Alg. 2 l.1-2
+    } else if (rec_hash != 0ull && rh != 0ull && rec_hash != rh) {
+        dec = PREPOS_INELIGIBLE;  // Alg. 2 l.1-2, realised entry != pre-positioned entry
+    } else if (top1 < 0 || top1 >= vocab || !((bitmap[top1 >> 5] >> (top1 & 31)) & 1u)) {
+        dec = PREPOS_NOT_IN_FAST_SET;  // Eq. 12, argmax not in A
+    } else if (strict_gt ? !(gap > tau) : !(gap >= tau)) {
+        dec = PREPOS_GAP_BELOW_TAU;  // Eq. 12, gamma vs tau
+    } else {
+        dec = PREPOS_SERVED;  // Alg. 2 l.6
+    }
+    decision[r] = dec;
+    token[r] = (dec == PREPOS_SERVED) ? top1 : -1;
+}
+
+// Sec. 3.6: version bump + valid clear.  Atomics so that repeated ids each count as one mutation.
+__global__ void __launch_bounds__(128) invalidate_kernel(int n, const int32_t *__restrict__ session_ids,
+                                                         unsigned long long *__restrict__ session_version,
+                                                         prepos_record *__restrict__ records)
+{
+    const int r = blockIdx.x * blockDim.x + threadIdx.x;
+    if (r >= n) return;
+    const int sid = session_ids[r];
+    atomicAnd(&records[sid].flags, ~PREPOS_FLAG_VALID);
+    __threadfence();
+    atomicAdd(&session_version[sid], 1ull);
+}
+
+}  // namespace
+
+int prepos_launch_gate_serve(prepos_ctx *ctx, int n, const int32_t *session_ids, const uint64_t *req_hash,
+                             const prepos_record *records, const uint64_t *session_version,
+                             const uint32_t *bitmap, float tau, int strict_gt, int32_t *decision, int32_t *token,
+                             cudaStream_t stream)
+{
+    if (n == 0) return PREPOS_OK;
+    const int threads = 128;
+    gate_serve_kernel<<<(n + threads - 1) / threads, threads, 0, stream>>>(
+        n, session_ids, req_hash, records, session_version, bitmap, ctx->shape.vocab, tau, strict_gt, decision, token);
+    PREPOS_CUDA_TRY(cudaGetLastError());
+    ctx->launches += 1;
+    return PREPOS_OK;
+}
+
+int prepos_launch_invalidate(prepos_ctx *ctx, int n, const int32_t *session_ids, uint64_t *session_version,
+                             prepos_record *records, cudaStream_t stream)
+{
+    if (n == 0) return PREPOS_OK;
+    const int threads = 128;
+    invalidate_kernel<<<(n + threads - 1) / threads, threads, 0, stream>>>(
+        n, session_ids, reinterpret_cast<unsigned long long *>(session_version), records);
+    PREPOS_CUDA_TRY(cudaGetLastError());
+    ctx->launches += 1;
+    return PREPOS_OK;
+}

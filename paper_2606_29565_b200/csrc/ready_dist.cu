@@ -1,0 +1,486 @@
+// ready_dist.cu -- a3 + a4: the last-position LM head fused with the vocabulary reduction into the
+// ready-distribution record (Alg. 1 l.6, l.10-12; Top2/gamma/argmax of Alg. 2
+// l.3-4, Eq. 11), plus a4' the standalone scan of stored logits
+// (Eq. 3).
+//
+// The pass is a pure HBM stream of W_vocab [V][H] bf16 (1.05 GB at V=128256, H=4096).  Design:
+//   * persistent CTAs, one per SM; CTA c owns the 128-row vocabulary tiles c, c+grid, ...
+//   * one producer warp streams [128 rows x 128 cols] stages of W through a ring of shared-memory
+//     buffers with TMA (cp.async.bulk.tensor, 128B swizzle) completing on mbarriers;
+//   * eight consumer warps (16 rows each) read the swizzled tiles with ldmatrix and multiply them
+//     with up to 8 hidden rows held in shared memory using warp-level bf16 MMA with fp32
+//     accumulation.  The work is HBM-bound (2 flop/byte per hidden row): the tensor instruction is
+//     used only to keep the instruction count per byte far below the issue limit, so that the
+//     stream is never stalled by ALU work; it is not a tcgen05-class contraction.
+//   * every lane keeps a running (top1, top2, max, sum-exp) state for the logits it produces, warp
+//     shuffles reduce it, and a single cross-CTA pass by the last-arriving CTA merges the per-CTA
+//     partials in CTA order under the total order (logit desc, id asc), so ids are independent of
+//     the reduction tree.
+#include <math_constants.h>
+
+#include "common.cuh"
+#include "ptx.cuh"
+
+namespace {
+
+constexpr int kTileRows = 128;
+constexpr int kBoxCols = 64;                                  // 128 B of bf16: one swizzle span
+constexpr int kStageCols = 128;                               // two TMA boxes per stage
+constexpr int kBoxBytes = kTileRows * kBoxCols * 2;           // 16 KB
+constexpr int kStageBytes = kTileRows * kStageCols * 2;       // 32 KB
+constexpr int kConsumerWarps = 8;
+constexpr int kThreads = (kConsumerWarps + 1) * 32;
+constexpr int kNB = 8;       // hidden rows per pass (the n8 of m16n8k16)
+constexpr int kXPad = 8;     // bf16 elements of row padding of the hidden rows in smem (bank spread)
+constexpr int kMaxStages = 6;
+
+struct Top2Lse {
+    float v1, v2, m, s;
+    int i1, i2;
+    int nonfinite;
+};
+
+__device__ __forceinline__ Top2Lse t2_init()
+{
+    Top2Lse t;
+    t.v1 = t.v2 = -CUDART_INF_F;
+    t.i1 = t.i2 = 0x7fffffff;
+    t.m = -CUDART_INF_F;
+    t.s = 0.f;
+    t.nonfinite = 0;
+    return t;
+}
+// (logit desc, id asc): the one order used everywhere (reading Q8)
+__device__ __forceinline__ bool t2_better(float va, int ia, float vb, int ib)
+{
+    return va > vb || (va == vb && ia < ib);
+}
+__device__ __forceinline__ void t2_insert(Top2Lse &t, float v, int i)
+{
+    if (t2_better(v, i, t.v1, t.i1)) {
+        t.v2 = t.v1;
+        t.i2 = t.i1;
+        t.v1 = v;
+        t.i1 = i;
+    } else if (t2_better(v, i, t.v2, t.i2)) {
+        t.v2 = v;
+        t.i2 = i;
+    }
+}
+__device__ __forceinline__ void t2_push(Top2Lse &t, float v, int i)
+{
+    if (!(fabsf(v) <= 3.0e38f)) t.nonfinite = 1;  // NaN or Inf
+    t2_insert(t, v, i);
+    if (v > t.m) {
+        t.s = t.s * __expf(t.m - v) + 1.f;
+        t.m = v;
+    } else {
+        t.s += __expf(v - t.m);
+    }
+}
+__device__ __forceinline__ void t2_merge(Top2Lse &a, const Top2Lse &b)
+{
+    t2_insert(a, b.v1, b.i1);
+    t2_insert(a, b.v2, b.i2);
+    const float m = fmaxf(a.m, b.m);
+    if (m > -CUDART_INF_F) {
+        a.s = a.s * __expf(a.m - m) + b.s * __expf(b.m - m);
+        a.m = m;
+    }
+    a.nonfinite |= b.nonfinite;
+}
+__device__ __forceinline__ Top2Lse t2_shfl_xor(const Top2Lse &t, int mask)
+{
+    Top2Lse o;
+    o.v1 = __shfl_xor_sync(0xffffffffu, t.v1, mask);
+    o.v2 = __shfl_xor_sync(0xffffffffu, t.v2, mask);
+    o.m = __shfl_xor_sync(0xffffffffu, t.m, mask);
+    o.s = __shfl_xor_sync(0xffffffffu, t.s, mask);
+    o.i1 = __shfl_xor_sync(0xffffffffu, t.i1, mask);
+    o.i2 = __shfl_xor_sync(0xffffffffu, t.i2, mask);
+    o.nonfinite = __shfl_xor_sync(0xffffffffu, t.nonfinite, mask);
+    return o;
+}
+__device__ __forceinline__ void t2_store(RdPartial *p, const Top2Lse &t)
+{
+    RdPartial r;
+    r.m = t.m;
+    r.s = t.s;
+    r.v1 = t.v1;
+    r.v2 = t.v2;
+    r.i1 = t.i1;
+    r.i2 = t.i2;
+    r.nonfinite = t.nonfinite;
+    r.pad = 0;
+    *reinterpret_cast<uint4 *>(p) = *reinterpret_cast<uint4 *>(&r);
+    *(reinterpret_cast<uint4 *>(p) + 1) = *(reinterpret_cast<uint4 *>(&r) + 1);
+}
+__device__ __forceinline__ Top2Lse t2_load(const RdPartial *p)
+{
+    // written by another CTA in this launch: read through L2
+    const uint4 a = __ldcg(reinterpret_cast<const uint4 *>(p));
+    const uint4 b = __ldcg(reinterpret_cast<const uint4 *>(p) + 1);
+    Top2Lse t;
+    t.m = __uint_as_float(a.x);
+    t.s = __uint_as_float(a.y);
+    t.v1 = __uint_as_float(a.z);
+    t.v2 = __uint_as_float(a.w);
+    t.i1 = static_cast<int>(b.x);
+    t.i2 = static_cast<int>(b.y);
+    t.nonfinite = static_cast<int>(b.z);
+    return t;
+}
+
+// the record's reduction fields; version/hash/position/VALID are the caller's business
+__device__ __forceinline__ void write_record_fields(prepos_record *rec, const Top2Lse &t)
+{
+    rec->max_logit = t.v1;
+    rec->lse = t.m + __logf(t.s);
+    rec->top1 = t.i1;
+    rec->top2 = (t.i2 == 0x7fffffff) ? -1 : t.i2;
+    rec->gap = (t.i2 == 0x7fffffff) ? CUDART_INF_F : t.v1 - t.v2;
+}
+
+// Merge `n_parts` per-CTA partials of row `row` (partials[row * kMaxRdPartials + c]) in CTA order with one
+// warp; result valid in lane 0.
+__device__ __forceinline__ Top2Lse merge_partials_warp(const RdPartial *partials, int row, int n_parts, int lane)
+{
+    Top2Lse acc = t2_init();
+    for (int c = lane; c < n_parts; c += 32) {
+        const Top2Lse p = t2_load(partials + static_cast<size_t>(row) * kMaxRdPartials + c);
+        t2_merge(acc, p);
+    }
+#pragma unroll
+    for (int mask = 1; mask < 32; mask <<= 1) {
+        const Top2Lse o = t2_shfl_xor(acc, mask);
+        t2_merge(acc, o);
+    }
+    return acc;
+}
+
+struct RdParams {
+    int n;  // hidden rows in this pass (<= kNB)
+    int H, V;
+    int n_stages;
+    int x_rows;  // rows of the smem hidden block (n+1 with a trailing zero row, or 8)
+    const __nv_bfloat16 *hidden;  // [n][H]
+    const int32_t *session_ids;   // [n]
+    const int64_t *position_p;
+    const uint64_t *entry_hash;
+    const int32_t *skip_mask;
+    prepos_record *records;
+    const uint64_t *session_version;
+    float *logits_out;  // [n][V] or null
+    RdPartial *partials;
+    unsigned int *counter;
+};
+
+__global__ void __launch_bounds__(kThreads, 1)
+ready_dist_kernel(const __grid_constant__ CUtensorMap tm_w, const RdParams p)
+{
+    extern __shared__ __align__(1024) uint8_t smem_raw[];
+    // carve: [stages][32 KB] | x block | barriers | per-warp partials
+    uint8_t *smem = reinterpret_cast<uint8_t *>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
+    uint8_t *stage_base = smem;
+    const int x_stride = p.H + kXPad;  // elements
+    __nv_bfloat16 *xs = reinterpret_cast<__nv_bfloat16 *>(smem + static_cast<size_t>(p.n_stages) * kStageBytes);
+    uint64_t *bars = reinterpret_cast<uint64_t *>(reinterpret_cast<uint8_t *>(xs) +
+                                                  ((static_cast<size_t>(p.x_rows) * x_stride * 2 + 15) & ~size_t(15)));
+    uint64_t *full_bar = bars;
+    uint64_t *empty_bar = bars + kMaxStages;
+    RdPartial *warp_part = reinterpret_cast<RdPartial *>(bars + 2 * kMaxStages);  // [kConsumerWarps][kNB]
+    __shared__ int s_is_last;
+
+    const int warp = threadIdx.x >> 5;
+    const int lane = threadIdx.x & 31;
+    const int n_tiles = (p.V + kTileRows - 1) / kTileRows;
+    const int n_kc = p.H / kStageCols;
+
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < p.n_stages; ++s) {
+            ptx::mbar_init(ptx::smem_u32(&full_bar[s]), 1);
+            ptx::mbar_init(ptx::smem_u32(&empty_bar[s]), kConsumerWarps);
+        }
+        ptx::fence_mbar_init();
+    }
+    // hidden rows -> smem (row x_rows-1 is zero when n < 8; lanes of absent rows read it)
+    {
+        const int chunks_per_row = p.H / 8;
+        for (int idx = threadIdx.x; idx < p.x_rows * chunks_per_row; idx += kThreads) {
+            const int r = idx / chunks_per_row, c = idx - r * chunks_per_row;
+            uint4 v = make_uint4(0, 0, 0, 0);
+            if (r < p.n) v = *reinterpret_cast<const uint4 *>(p.hidden + static_cast<size_t>(r) * p.H + c * 8);
+            *reinterpret_cast<uint4 *>(xs + static_cast<size_t>(r) * x_stride + c * 8) = v;
+        }
+    }
+    __syncthreads();
+
+    if (warp == kConsumerWarps) {
+        // ===== TMA producer =====
+        if (lane == 0) {
+            ptx::prefetch_tmap(&tm_w);
+            const uint64_t pol = ptx::policy_evict_first();  // W is read once per pass
+            int stage = 0;
+            uint32_t phase = 0;
+            for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+                for (int kc = 0; kc < n_kc; ++kc) {
+                    ptx::mbar_wait(ptx::smem_u32(&empty_bar[stage]), phase ^ 1);
+                    const uint32_t fb = ptx::smem_u32(&full_bar[stage]);
+                    ptx::mbar_arrive_expect_tx(fb, kStageBytes);
+                    const uint32_t dst = ptx::smem_u32(stage_base + static_cast<size_t>(stage) * kStageBytes);
+                    ptx::tma_load_2d(dst, &tm_w, fb, kc * kStageCols, tile * kTileRows, pol);
+                    ptx::tma_load_2d(dst + kBoxBytes, &tm_w, fb, kc * kStageCols + kBoxCols, tile * kTileRows, pol);
+                    if (++stage == p.n_stages) {
+                        stage = 0;
+                        phase ^= 1;
+                    }
+                }
+            }
+        }
+    } else {
+        // ===== consumers: 16 vocabulary rows per warp =====
+        Top2Lse st[2];
+        st[0] = t2_init();
+        st[1] = t2_init();
+        const int n0 = 2 * (lane & 3);  // this lane's two hidden rows (accumulator columns)
+        // ldmatrix lane addressing.  A: matrices (r0-7,k0-7) (r8-15,k0-7) (r0-7,k8-15) (r8-15,k8-15)
+        const int a_row = warp * 16 + (lane & 7) + ((lane >> 3) & 1) * 8;
+        const int a_kc = lane >> 4;  // 16-byte chunk within the 32-byte k-step
+        // B: matrices (k0-7) (k8-15) (k16-23) (k24-31), each 8 hidden rows x 16 B
+        const int b_row = min(lane & 7, p.x_rows - 1);
+        const uint32_t xs_lane = ptx::smem_u32(xs + static_cast<size_t>(b_row) * x_stride + (lane >> 3) * 8);
+
+        int stage = 0;
+        uint32_t phase = 0;
+        for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+            float acc[4] = {0.f, 0.f, 0.f, 0.f};
+            for (int kc = 0; kc < n_kc; ++kc) {
+                ptx::mbar_wait(ptx::smem_u32(&full_bar[stage]), phase);
+                const uint32_t sbase = ptx::smem_u32(stage_base + static_cast<size_t>(stage) * kStageBytes);
+#pragma unroll
+                for (int box = 0; box < 2; ++box) {
+                    const uint32_t abase = sbase + box * kBoxBytes + a_row * 128;
+                    const uint32_t xk = xs_lane + (kc * kStageCols + box * kBoxCols) * 2;
+#pragma unroll
+                    for (int kk = 0; kk < 2; ++kk) {  // 32 columns = two k16 steps per B ldmatrix
+                        uint32_t b0, b1, b2, b3;
+                        ptx::ldmatrix_x4(xk + kk * 64, b0, b1, b2, b3);
+#pragma unroll
+                        for (int ks = 0; ks < 2; ++ks) {
+                            const int chunk = (kk * 2 + ks) * 2 + a_kc;  // 16-byte chunk index in the 128-byte row
+                            uint32_t a0, a1, a2, a3;
+                            ptx::ldmatrix_x4(abase + ((chunk ^ (a_row & 7)) << 4), a0, a1, a2, a3);
+                            ptx::mma_bf16_16816(acc, a0, a1, a2, a3, ks ? b2 : b0, ks ? b3 : b1);
+                        }
+                    }
+                }
+                __syncwarp();
+                if (lane == 0) ptx::mbar_arrive(ptx::smem_u32(&empty_bar[stage]));
+                if (++stage == p.n_stages) {
+                    stage = 0;
+                    phase ^= 1;
+                }
+            }
+            // logits of rows v, v+8 for hidden rows n0, n0+1
+            const int v = tile * kTileRows + warp * 16 + (lane >> 2);
+#pragma unroll
+            for (int j = 0; j < 2; ++j) {
+                if (n0 + j < p.n) {
+                    if (v < p.V) t2_push(st[j], acc[j], v);
+                    if (v + 8 < p.V) t2_push(st[j], acc[2 + j], v + 8);
+                    if (p.logits_out) {
+                        float *lo = p.logits_out + static_cast<size_t>(n0 + j) * p.V;
+                        if (v < p.V) lo[v] = acc[j];
+                        if (v + 8 < p.V) lo[v + 8] = acc[2 + j];
+                    }
+                }
+            }
+        }
+        // lanes sharing lane&3 hold the same hidden rows: reduce over lane bits 2..4
+#pragma unroll
+        for (int j = 0; j < 2; ++j) {
+#pragma unroll
+            for (int mask = 4; mask < 32; mask <<= 1) {
+                const Top2Lse o = t2_shfl_xor(st[j], mask);
+                t2_merge(st[j], o);
+            }
+        }
+        if (lane < 4) {
+            t2_store(&warp_part[warp * kNB + n0], st[0]);
+            t2_store(&warp_part[warp * kNB + n0 + 1], st[1]);
+        }
+    }
+    __syncthreads();
+    // CTA partial per hidden row (fixed warp order), then the single cross-CTA pass
+    if (threadIdx.x < p.n) {
+        Top2Lse acc = t2_init();
+        for (int w = 0; w < kConsumerWarps; ++w) {
+            const RdPartial *q = &warp_part[w * kNB + threadIdx.x];
+            Top2Lse t;
+            t.m = q->m, t.s = q->s, t.v1 = q->v1, t.v2 = q->v2, t.i1 = q->i1, t.i2 = q->i2, t.nonfinite = q->nonfinite;
+            t2_merge(acc, t);
+        }
+        t2_store(p.partials + static_cast<size_t>(threadIdx.x) * kMaxRdPartials + blockIdx.x, acc);
+        __threadfence();
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        const unsigned int prev = atomicAdd(p.counter, 1u);
+        s_is_last = (prev == gridDim.x - 1);
+    }
+    __syncthreads();
+    if (!s_is_last) return;
+    __threadfence();
+    if (warp < p.n) {
+        const Top2Lse t = merge_partials_warp(p.partials, warp, gridDim.x, lane);
+        if (lane == 0 && !(p.skip_mask && p.skip_mask[warp])) {
+            const int sid = p.session_ids[warp];
+            prepos_record *rec = p.records + sid;
+            // Alg. 1 l.10-12: position, dist (here: argmax, gamma, max, lse), decoded/valid.
+            write_record_fields(rec, t);
+            rec->entry_hash = p.entry_hash ? p.entry_hash[warp] : 0ull;
+            rec->position = p.position_p ? p.position_p[warp] : 0ll;
+            rec->version = p.session_version[sid];
+            __threadfence();  // payload before the valid bit
+            rec->flags = PREPOS_FLAG_VALID | (t.nonfinite ? PREPOS_FLAG_NONFINITE : 0u);
+        }
+    }
+    if (threadIdx.x == 0) *p.counter = 0u;  // self-reset for the next launch on this stream
+}
+
+// ---- a4': scan of stored fp32 logits ---------------------------------------------------------------
+constexpr int kScanThreads = 256;
+
+__global__ void __launch_bounds__(kScanThreads)
+scan_logits_kernel(int V, const float *__restrict__ logits, prepos_record *__restrict__ out, RdPartial *partials,
+                   unsigned int *counters)
+{
+    const int row = blockIdx.y;
+    const float *lg = logits + static_cast<size_t>(row) * V;
+    Top2Lse st = t2_init();
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    // 128-bit loads where the row base allows it
+    const bool vec_ok = ((reinterpret_cast<uintptr_t>(lg) & 15) == 0);
+    const int v4 = vec_ok ? V / 4 : 0;
+    for (int i = blockIdx.x * kScanThreads + threadIdx.x; i < v4; i += gridDim.x * kScanThreads) {
+        const float4 x = __ldg(reinterpret_cast<const float4 *>(lg) + i);
+        t2_push(st, x.x, 4 * i);
+        t2_push(st, x.y, 4 * i + 1);
+        t2_push(st, x.z, 4 * i + 2);
+        t2_push(st, x.w, 4 * i + 3);
+    }
+    for (int i = v4 * 4 + blockIdx.x * kScanThreads + threadIdx.x; i < V; i += gridDim.x * kScanThreads)
+        t2_push(st, __ldg(lg + i), i);
+#pragma unroll
+    for (int mask = 1; mask < 32; mask <<= 1) {
+        const Top2Lse o = t2_shfl_xor(st, mask);
+        t2_merge(st, o);
+    }
+    __shared__ RdPartial s_part[kScanThreads / 32];
+    __shared__ int s_is_last;
+    if (lane == 0) t2_store(&s_part[warp], st);
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        Top2Lse acc = t2_init();
+        for (int w = 0; w < kScanThreads / 32; ++w) {
+            const RdPartial *q = &s_part[w];
+            Top2Lse t;
+            t.m = q->m, t.s = q->s, t.v1 = q->v1, t.v2 = q->v2, t.i1 = q->i1, t.i2 = q->i2, t.nonfinite = q->nonfinite;
+            t2_merge(acc, t);
+        }
+        t2_store(partials + static_cast<size_t>(row) * kMaxRdPartials + blockIdx.x, acc);
+        __threadfence();
+        const unsigned int prev = atomicAdd(&counters[row], 1u);
+        s_is_last = (prev == gridDim.x - 1);
+    }
+    __syncthreads();
+    if (!s_is_last) return;
+    __threadfence();
+    if (warp == 0) {
+        const Top2Lse t = merge_partials_warp(partials, row, gridDim.x, lane);
+        if (lane == 0) {
+            prepos_record *rec = out + row;
+            write_record_fields(rec, t);
+            const uint32_t f = rec->flags & ~PREPOS_FLAG_NONFINITE;
+            rec->flags = f | (t.nonfinite ? PREPOS_FLAG_NONFINITE : 0u);
+            counters[row] = 0u;
+        }
+    }
+}
+
+typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
+                                  const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+}  // namespace
+
+void *prepos_get_encode_tiled();  // api.cu
+
+int prepos_launch_ready_dist(prepos_ctx *ctx, int n, const int32_t *session_ids, const __nv_bfloat16 *hidden,
+                             const __nv_bfloat16 *w, const int64_t *position_p, const uint64_t *entry_hash,
+                             const int32_t *skip_mask, prepos_record *records, const uint64_t *session_version,
+                             float *logits_out, cudaStream_t stream)
+{
+    const int H = ctx->shape.hidden, V = ctx->shape.vocab;
+    EncodeTiledFn encode = reinterpret_cast<EncodeTiledFn>(prepos_get_encode_tiled());
+    if (!encode) return PREPOS_E_CUDA;
+    CUtensorMap tm;
+    const cuuint64_t dims[2] = {static_cast<cuuint64_t>(H), static_cast<cuuint64_t>(V)};
+    const cuuint64_t strides[1] = {static_cast<cuuint64_t>(H) * 2};
+    const cuuint32_t box[2] = {kBoxCols, kTileRows};
+    const cuuint32_t estr[2] = {1, 1};
+    if (encode(&tm, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<__nv_bfloat16 *>(w), dims, strides, box, estr,
+               CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+               CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+        return PREPOS_E_CUDA;
+
+    const int n_tiles = (V + kTileRows - 1) / kTileRows;
+    const int grid = n_tiles < ctx->num_sms ? n_tiles : ctx->num_sms;
+    for (int r0 = 0; r0 < n; r0 += kNB) {
+        RdParams p;
+        p.n = (n - r0 < kNB) ? n - r0 : kNB;
+        p.H = H;
+        p.V = V;
+        p.x_rows = (p.n < kNB) ? p.n + 1 : kNB;
+        const size_t x_bytes = (static_cast<size_t>(p.x_rows) * (H + kXPad) * 2 + 15) & ~size_t(15);
+        const size_t fixed = 1024 + x_bytes + 2 * kMaxStages * 8 + kConsumerWarps * kNB * sizeof(RdPartial);
+        int stages = static_cast<int>((232448 - fixed) / kStageBytes);
+        if (stages > kMaxStages) stages = kMaxStages;
+        if (stages < 2) return PREPOS_E_SHAPE;
+        p.n_stages = stages;
+        p.hidden = hidden + static_cast<size_t>(r0) * H;
+        p.session_ids = session_ids + r0;
+        p.position_p = position_p ? position_p + r0 : nullptr;
+        p.entry_hash = entry_hash ? entry_hash + r0 : nullptr;
+        p.skip_mask = skip_mask ? skip_mask + r0 : nullptr;
+        p.records = records;
+        p.session_version = session_version;
+        p.logits_out = logits_out ? logits_out + static_cast<size_t>(r0) * V : nullptr;
+        p.partials = ctx->rd_partials;
+        p.counter = ctx->rd_counter;
+        const size_t smem = fixed + static_cast<size_t>(stages) * kStageBytes;
+        PREPOS_CUDA_TRY(cudaFuncSetAttribute(ready_dist_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                             static_cast<int>(smem)));
+        ready_dist_kernel<<<grid, kThreads, smem, stream>>>(tm, p);
+        PREPOS_CUDA_TRY(cudaGetLastError());
+        ctx->launches += 1;
+    }
+    return PREPOS_OK;
+}
+
+int prepos_launch_scan_logits(prepos_ctx *ctx, int n, const float *logits, prepos_record *out, cudaStream_t stream)
+{
+    const int V = ctx->shape.vocab;
+    for (int r0 = 0; r0 < n; r0 += kRdMaxRows) {
+        const int rows = (n - r0 < kRdMaxRows) ? n - r0 : kRdMaxRows;
+        int gx = (V + kScanThreads * 16 - 1) / (kScanThreads * 16);  // >= 16 logits per thread
+        if (gx > 64) gx = 64;
+        if (gx < 1) gx = 1;
+        scan_logits_kernel<<<dim3(gx, rows), kScanThreads, 0, stream>>>(V, logits + static_cast<size_t>(r0) * V,
+                                                                        out + r0, ctx->rd_partials,
+                                                                        ctx->rd_counter + 1);
+        PREPOS_CUDA_TRY(cudaGetLastError());
+        ctx->launches += 1;
+    }
+    return PREPOS_OK;
+}

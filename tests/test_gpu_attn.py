@@ -1,0 +1,209 @@
+"""GPU parity of a0/a1/a2 (prepos_entry_attn) against oracle O1, through the C ABI."""
+import numpy as np
+import pytest
+import torch
+
+from paper_2606_29565_b200 import synth
+from helpers import bits, oracle_attn_batch, oracle_attn_rows, check_attn, ATTN_ATOL
+
+pytestmark = pytest.mark.gpu
+
+PATHS = [1, 2]   # 1 = generic CUDA-core kernel, 2 = tcgen05 kernel
+
+
+@pytest.fixture(scope="module")
+def prepos():
+    from paper_2606_29565_b200 import prepos as p
+    p.lib()
+    return p
+
+
+def _ctx(prepos, shape, n_sessions, path):
+    ctx = prepos.Context(shape.layers, shape.Hq, shape.Hkv, shape.d, shape.H, shape.V, shape.page,
+                         max_sessions=max(n_sessions, 1))
+    try:
+        ctx.set_attn_path(path)
+    except prepos.PreposError as e:
+        if e.status == prepos.E_SHAPE:
+            pytest.skip("shape not taken by the tcgen05 path")
+        raise
+    return ctx
+
+
+def _gpu_run(prepos, sb, path, layers=None, poison=True):
+    """Copies the batch to the GPU (optionally NaN-poisoning every pool slot beyond n_s), runs entry_attn."""
+    shape = sb.shape
+    dev = "cuda"
+    kp, vp = sb.k_pool.to(dev).clone(), sb.v_pool.to(dev).clone()
+    if poison:
+        page = shape.page
+        used = torch.zeros(kp.shape[1] * page, dtype=torch.bool)
+        pt = sb.page_table.cpu()
+        for s in range(sb.n_sessions):
+            j = torch.arange(sb.n_s[s])
+            used[pt[s, j // page].long() * page + j % page] = True
+        mask = (~used).view(kp.shape[1], 1, page, 1).to(dev)
+        kp.masked_fill_(mask, float("nan"))
+        vp.masked_fill_(mask, float("nan"))
+    before = (kp.clone(), vp.clone())
+    out = torch.full(sb.q.shape, float("nan"), dtype=torch.bfloat16, device=dev)
+    ctx = _ctx(prepos, shape, sb.n_sessions, path)
+    nl = sb.k_pool.shape[0]
+    lb, le = (0, nl) if layers is None else layers
+    status = ctx.entry_attn(sb.q.to(dev), sb.k_new.to(dev), sb.v_new.to(dev), kp, vp, sb.page_table.to(dev),
+                            sb.n_s, sb.l_entry, sb.capacity, out, layer_begin=lb, layer_end=le)
+    ctx.sync()
+    return out, kp, vp, before, status, ctx
+
+
+def _check_append(sb, kp, vp, before, status, layers):
+    """a1 post-condition: appended slots == K_new/V_new bit for bit; every other pool element bit-identical."""
+    page = sb.shape.page
+    pt = sb.page_table.cpu()
+    for l in layers:
+        touched = torch.zeros(kp.shape[1], page, dtype=torch.bool)
+        for s in range(sb.n_sessions):
+            if status[s] != 0:
+                continue
+            r0 = sb.row_offset[s]
+            for jp in range(sb.l_entry[s]):
+                j = sb.n_s[s] + jp
+                pg, sl = int(pt[s, j // page]), j % page
+                assert torch.equal(kp[l, pg, :, sl].cpu().view(torch.int16), sb.k_new[l, r0 + jp].view(torch.int16))
+                assert torch.equal(vp[l, pg, :, sl].cpu().view(torch.int16), sb.v_new[l, r0 + jp].view(torch.int16))
+                touched[pg, sl] = True
+        m = (~touched).view(kp.shape[1], 1, page, 1).expand_as(kp[l]).cpu()
+        assert torch.equal(kp[l].cpu().view(torch.int16)[m], before[0][l].cpu().view(torch.int16)[m])
+        assert torch.equal(vp[l].cpu().view(torch.int16)[m], before[1][l].cpu().view(torch.int16)[m])
+
+
+@pytest.mark.parametrize("path", PATHS)
+def test_config1_many_seeds(prepos, oracle, path):
+    """BASELINE config 1 attention: 1 session, n_s=256, L=8, 4/2 heads, d=64 -- 24 seeds, full outputs."""
+    worst = 0.0
+    for k in range(24):
+        sb = synth.make_sessions(synth.C1, [256], [8], seed=synth.SEED_BASE + 1000 * k)
+        out, kp, vp, before, status, _ = _gpu_run(prepos, sb, path)
+        outs, st, _, _ = oracle_attn_batch(oracle, sb)
+        assert status == [0] and st[0] == 0
+        worst = max(worst, check_attn(out, outs, sb))
+        if k < 3:
+            _check_append(sb, kp, vp, before, status, [0])
+    assert worst <= ATTN_ATOL
+
+
+SHAPES = {
+    "d128_g4": synth.Shape("a", layers=2, Hq=8, Hkv=2, d=128, H=128, V=64, page=16),
+    "d128_g8": synth.Shape("b", layers=1, Hq=16, Hkv=2, d=128, H=128, V=64, page=16),
+    "d64_g2": synth.Shape("c", layers=2, Hq=4, Hkv=2, d=64, H=128, V=64, page=16),
+    "d128_g1": synth.Shape("d", layers=1, Hq=2, Hkv=2, d=128, H=128, V=64, page=16),
+}
+
+
+@pytest.mark.parametrize("path", PATHS)
+@pytest.mark.parametrize("shape_key,n_s,l_entry", [
+    ("d128_g4", [0], [24]),                       # n_s = 0: ordinary causal attention
+    ("d128_g4", [1], [1]),                        # smallest non-trivial
+    ("d128_g4", [127, 128, 129], [5, 16, 33]),    # around one 128-token tile; ragged pages
+    ("d128_g4", [700, 15, 300], [24, 96, 64]),    # several tiles + ragged tail; rows 96 / 384 / 256
+    ("d128_g8", [517], [32]),                     # G=8: 256 rows (config 5 row geometry)
+    ("d128_g8", [40], [70]),                      # 560 rows: three row chunks
+    ("d64_g2", [333, 64], [8, 40]),
+    ("d128_g1", [260], [3]),
+    ("d128_g4", [2500], [24]),                    # long enough to be split over many CTAs
+    ("d128_g4", [300, 100], [0, 7]),              # an empty entry next to a real one
+])
+def test_shapes_vs_oracle(prepos, oracle, path, shape_key, n_s, l_entry):
+    shape = SHAPES[shape_key]
+    sb = synth.make_sessions(shape, n_s, l_entry, seed=1000 + 7 * sum(n_s) + sum(l_entry) + len(shape_key))
+    out, kp, vp, before, status, _ = _gpu_run(prepos, sb, path)
+    outs, st, _, _ = oracle_attn_batch(oracle, sb)
+    assert status == [0] * len(n_s)
+    check_attn(out, outs, sb)
+    _check_append(sb, kp, vp, before, status, range(shape.layers))
+
+
+@pytest.mark.parametrize("path", PATHS)
+def test_budget_skip_no_side_effects(prepos, oracle, path):
+    """Alg. 1 l.2-3: a session whose entry exceeds its headroom is skipped: status, no pool write, out untouched."""
+    shape = SHAPES["d128_g4"]
+    sb = synth.make_sessions(shape, [100, 50, 200], [12, 20, 8], seed=77, tight_capacity=[None, 69, 208])
+    out, kp, vp, before, status, _ = _gpu_run(prepos, sb, path)
+    assert status == [0, prepos.SKIPPED_BUDGET, 0]          # 50+20 > 69 skipped; 200+8 == 208 admitted
+    outs, st, _, _ = oracle_attn_batch(oracle, sb)
+    assert st == {0: 0, 1: 1, 2: 0}
+    check_attn(out, outs, sb)
+    r0 = sb.row_offset[1]
+    assert torch.isnan(out[:, r0:r0 + 20].float()).all()    # rows of the skipped session untouched
+    _check_append(sb, kp, vp, before, status, range(shape.layers))
+
+
+@pytest.mark.parametrize("path", PATHS)
+def test_layer_range_and_page_shuffle_bit_identical(prepos, oracle, path):
+    """(a) layer_begin/layer_end touch only those layers; (b) permuting physical pages leaves the result
+    bit-identical (SURVEY pin 9 on the GPU, fixed split plan)."""
+    shape = SHAPES["d128_g4"]
+    sb = synth.make_sessions(shape, [900, 130], [24, 9], seed=5)
+    out_a, kp, vp, before, status, _ = _gpu_run(prepos, sb, path, layers=(1, 2), poison=False)
+    assert torch.isnan(out_a[0].float()).all() and not torch.isnan(out_a[1].float()).any()
+    assert torch.equal(kp[0].view(torch.int16), before[0][0].view(torch.int16))
+    outs, _, _, _ = oracle_attn_batch(oracle, sb, layers=[1])
+    check_attn(out_a, outs, sb)
+    n_pages = sb.k_pool.shape[1]
+    perm = torch.randperm(n_pages, generator=torch.Generator().manual_seed(1))
+    inv = torch.empty_like(perm)
+    inv[perm] = torch.arange(n_pages)
+    sb2 = synth.make_sessions(shape, [900, 130], [24, 9], seed=5)
+    sb2.k_pool.copy_(sb.k_pool[:, inv])
+    sb2.v_pool.copy_(sb.v_pool[:, inv])
+    sb2.page_table.copy_(perm[sb.page_table.long()].to(torch.int32))
+    out_b, *_ = _gpu_run(prepos, sb2, path, layers=(1, 2), poison=False)
+    assert torch.equal(out_a[1].view(torch.int16), out_b[1].view(torch.int16))
+
+
+@pytest.mark.parametrize("path", PATHS)
+def test_two_step_consistency(prepos, oracle, path):
+    """Pre-position L1 then L2 tokens (second call sees n_s + L1 through the appended pages) ~ one call."""
+    shape = SHAPES["d128_g4"]
+    L1, L2, n = 10, 14, 200
+    sb = synth.make_sessions(shape, [n], [L1 + L2], seed=9)
+    out_one, kp1, vp1, _, _, _ = _gpu_run(prepos, sb, path, poison=False)
+    dev = "cuda"
+    kp, vp = sb.k_pool.to(dev).clone(), sb.v_pool.to(dev).clone()
+    ctx = _ctx(prepos, shape, 1, path)
+    q, kn, vn = sb.q.to(dev), sb.k_new.to(dev), sb.v_new.to(dev)
+    o1 = torch.zeros((shape.layers, L1, shape.Hq, shape.d), dtype=torch.bfloat16, device=dev)
+    o2 = torch.zeros((shape.layers, L2, shape.Hq, shape.d), dtype=torch.bfloat16, device=dev)
+    ctx.entry_attn(q[:, :L1].contiguous(), kn[:, :L1].contiguous(), vn[:, :L1].contiguous(), kp, vp,
+                   sb.page_table.to(dev), [n], [L1], sb.capacity, o1)
+    ctx.entry_attn(q[:, L1:].contiguous(), kn[:, L1:].contiguous(), vn[:, L1:].contiguous(), kp, vp,
+                   sb.page_table.to(dev), [n + L1], [L2], sb.capacity, o2)
+    ctx.sync()
+    two = torch.cat([o1, o2], dim=1).float()
+    assert (two - out_one.float()).abs().max() <= 2e-2       # both within 1e-2 of the oracle
+    assert torch.equal(kp.view(torch.int16), kp1.view(torch.int16)) and torch.equal(vp.view(torch.int16), vp1.view(torch.int16))
+    outs, _, _, _ = oracle_attn_batch(oracle, sb)
+    check_attn(torch.cat([o1, o2], dim=1), outs, sb)
+
+
+@pytest.mark.parametrize("path", PATHS)
+def test_config4_like_batch_sampled(prepos, oracle, path):
+    """A scaled-down agentic batch (BASELINE config 4 structure): 6 sessions, lognormal n_s, L ~ U{32..96},
+    one shuffled pool, 2 layers of 8B head geometry (32/8, d=128); oracle on sampled (layer, session, head, row)."""
+    shape = synth.Shape("c4s", layers=2, Hq=32, Hkv=8, d=128, H=128, V=64, page=16)
+    n_s = synth.lognormal_ns(6, 42, lo=256, hi=3000, median=900.0)
+    l_e = synth.uniform_l(6, 42)
+    sb = synth.make_sessions(shape, n_s, l_e, seed=43)
+    out, kp, vp, before, status, _ = _gpu_run(prepos, sb, path)
+    assert status == [0] * 6
+    rng = np.random.default_rng(0)
+    worst = 0.0
+    for s in range(6):
+        for l in range(2):
+            picks = [(int(rng.integers(0, 32)), int(rng.integers(0, l_e[s]))) for _ in range(3)] + [(31, l_e[s] - 1), (0, 0)]
+            ref = oracle_attn_rows(oracle, sb, l, s, picks)
+            for (h, i), o in ref.items():
+                got = out[l, sb.row_offset[s] + i, h].cpu().to(torch.float64).numpy()
+                worst = max(worst, float(np.abs(got - o).max()))
+    assert worst <= ATTN_ATOL, worst
+    _check_append(sb, kp, vp, before, status, range(2))

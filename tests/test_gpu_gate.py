@@ -1,0 +1,147 @@
+"""GPU parity of a5/a6 (prepos_gate_serve, prepos_invalidate): integer work, bit-exact against the oracle."""
+import numpy as np
+import pytest
+import torch
+
+from paper_2606_29565_b200 import synth
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def prepos():
+    from paper_2606_29565_b200 import prepos as p
+    p.lib()
+    return p
+
+
+def _pack_records(n, gap, top1, flags, version, ehash):
+    """Host-side packing of a record table from given fields (layout of include/prepos.h)."""
+    raw = np.zeros((n, 48), dtype=np.uint8)
+    f = raw.view(np.float32).reshape(n, 12)
+    i = raw.view(np.int32).reshape(n, 12)
+    q = raw.view(np.int64).reshape(n, 6)
+    f[:, 0] = 1.0
+    f[:, 1] = 2.0
+    i[:, 2] = top1
+    i[:, 3] = 0
+    f[:, 4] = gap
+    i[:, 5] = flags
+    q[:, 3] = version
+    q[:, 4] = ehash
+    return torch.from_numpy(raw)
+
+
+def test_truth_table_random_batch(prepos, oracle):
+    """4096 requests over 64 records (BASELINE config 4's serve batch) with every reason code present."""
+    V, n_sess, n_req = 128256, 64, 4096
+    rng = np.random.default_rng(3)
+    fast = synth.make_fast_set(synth.C4, synth.SEED_BASE + 3)
+    gap = rng.uniform(0, 6, n_sess).astype(np.float32)
+    gap[:4] = [3.0, np.nextafter(np.float32(3.0), np.float32(0)), np.nextafter(np.float32(3.0), np.float32(9)), 0.0]
+    top1 = np.where(rng.random(n_sess) < 0.7, rng.choice(fast.numpy(), n_sess), rng.integers(0, V, n_sess)).astype(np.int32)
+    flags = np.where(rng.random(n_sess) < 0.85, 1, 0).astype(np.int32)
+    flags[5] = 3                                   # valid but non-finite
+    rec_ver = rng.integers(0, 3, n_sess)
+    live = np.where(rng.random(n_sess) < 0.8, rec_ver, rec_ver + 1).astype(np.int64)
+    ehash = np.where(rng.random(n_sess) < 0.5, 0, rng.integers(1, 1 << 40, n_sess)).astype(np.int64)
+    recs = _pack_records(n_sess, gap, top1, flags, rec_ver, ehash).cuda()
+    sids = synth.serve_requests(n_req, n_sess, synth.SEED_BASE + 3)
+    rh = np.where(rng.random(n_req) < 0.5, 0, np.where(rng.random(n_req) < 0.5, ehash[sids.numpy()], 12345)).astype(np.int64)
+    ctx = prepos.Context(32, 32, 8, 128, 4096, V, 16, max_sessions=64)
+    bm = prepos.fastset_build(fast, V)
+    obm = oracle.fastset_bitmap(fast.numpy(), V)
+    for strict in (False, True):
+        dec = torch.full((n_req,), -9, dtype=torch.int32, device="cuda")
+        tok = torch.full((n_req,), -9, dtype=torch.int32, device="cuda")
+        ctx.gate_serve(sids.cuda(), recs, torch.from_numpy(live).cuda(), bm.cuda(), 3.0, dec, tok,
+                       request_entry_hash=torch.from_numpy(rh).cuda(), strict_gt=strict)
+        ctx.sync()
+        dec, tok = dec.cpu().numpy(), tok.cpu().numpy()
+        seen = set()
+        for r in range(n_req):
+            s = int(sids[r])
+            d, t = oracle.gate(float(gap[s]), int(top1[s]), flags[s] & 1, (flags[s] >> 1) & 1, int(rec_ver[s]),
+                               int(live[s]), int(ehash[s]), int(rh[r]), obm, V, 3.0, strict)
+            assert (int(dec[r]), int(tok[r])) == (d, t), (r, s)
+            seen.add(d)
+        assert seen == {0, 1, 2, 3, 4}
+    # no hashes at all = relaxed
+    dec = torch.zeros(n_req, dtype=torch.int32, device="cuda")
+    tok = torch.zeros(n_req, dtype=torch.int32, device="cuda")
+    ctx.gate_serve(sids.cuda(), recs, torch.from_numpy(live).cuda(), bm.cuda(), 3.0, dec, tok)
+    ctx.sync()
+    assert prepos.INELIGIBLE not in set(dec.cpu().tolist())
+
+
+def test_tau_monotone_coverage(prepos):
+    """the served set is non-increasing in tau."""
+    V, n = 1024, 512
+    rng = np.random.default_rng(5)
+    recs = _pack_records(n, rng.uniform(0, 8, n).astype(np.float32), rng.integers(0, V, n).astype(np.int32),
+                         np.ones(n, np.int32), np.zeros(n, np.int64), np.zeros(n, np.int64)).cuda()
+    ctx = prepos.Context(1, 4, 2, 64, 256, V, 16, max_sessions=8)
+    bm = prepos.fastset_build(rng.choice(V, 300, replace=False).tolist(), V).cuda()
+    sid = torch.arange(n, dtype=torch.int32, device="cuda")
+    ver = torch.zeros(n, dtype=torch.int64, device="cuda")
+    prev = None
+    for tau in np.linspace(0, 9, 19):
+        dec = torch.zeros(n, dtype=torch.int32, device="cuda")
+        tok = torch.zeros(n, dtype=torch.int32, device="cuda")
+        ctx.gate_serve(sid, recs, ver, bm, float(tau), dec, tok)
+        ctx.sync()
+        fired = set(torch.nonzero(dec == 0).flatten().cpu().tolist())
+        if prev is not None:
+            assert fired <= prev
+        prev = fired
+    assert not prev
+
+
+def test_config3_trace_invalidate_never_serves_stale(prepos, oracle):
+    """BASELINE config 3 trace (reading Q16): 1000 updates, each bumping the version with p=0.3, a serve after each;
+    stale records are refused; re-pre-position (ready_dist on the next hidden row of a pool of 16) after a bump.
+    GPU state machine vs the oracle's SessionTable, step by step."""
+    shape = synth.Shape("c3v", layers=1, Hq=4, Hkv=2, d=64, H=256, V=2048, fast_set=32, tau=3.0, planted_frac=0.75)
+    seed = synth.SEED_BASE + 2
+    w = synth.make_w_vocab(shape, seed)
+    fast = synth.make_fast_set(shape, seed)
+    pool, _, _ = synth.make_hidden(shape, 16, w, fast, seed)
+    from helpers import bits
+    refs = [oracle.record(oracle.logits(bits(w), bits(pool[r]))) for r in range(16)]
+    bumps = synth.bump_trace(1000, seed)
+    ctx = prepos.Context(1, 4, 2, 64, 256, 2048, 16, max_sessions=4)
+    wd, pd = w.cuda(), pool.cuda()
+    recs = prepos.new_records(2)
+    ver = torch.zeros(2, dtype=torch.int64, device="cuda")
+    sid = torch.tensor([1], dtype=torch.int32, device="cuda")
+    bm = prepos.fastset_build(fast, shape.V).cuda()
+    obm = oracle.fastset_bitmap(fast.numpy(), shape.V)
+    st = oracle.SessionTable(2)
+    decs = torch.full((1000,), -9, dtype=torch.int32, device="cuda")
+    toks = torch.full((1000,), -9, dtype=torch.int32, device="cuda")
+    exp, cur = [], 0
+    ctx.ready_dist(sid, pd[0:1], wd, recs, ver)
+    st.preposition(1, refs[0])
+    for t, b in enumerate(bumps):
+        if b:
+            ctx.invalidate(sid, ver, recs)
+            st.invalidate([1])
+        ctx.gate_serve(sid, recs, ver, bm, shape.tau, decs[t:t + 1], toks[t:t + 1])
+        exp.append(st.serve(1, obm, shape.V, shape.tau))
+        if b:
+            assert exp[-1] == (oracle.STALE_OR_INVALID, -1)
+            cur = (cur + 1) % 16
+            ctx.ready_dist(sid, pd[cur:cur + 1], wd, recs, ver)
+            st.preposition(1, refs[cur])
+    ctx.sync()
+    got = list(zip(decs.cpu().tolist(), toks.cpu().tolist()))
+    amb = [abs(r.gap - shape.tau) < 4e-2 or r.gap < 4e-2 for r in refs]
+    assert not any(amb), "regenerate the pool: an ambiguous record would make the trace comparison inexact"
+    assert got == exp
+    assert sum(1 for d, _ in got if d == 0) > 0 and sum(1 for d, _ in got if d == 3) == sum(bumps)
+    assert int(ver[1]) == sum(bumps) and int(ver[0]) == 0
+    # repeated ids: each occurrence is one mutation
+    ctx.invalidate(torch.tensor([1, 1, 0], dtype=torch.int32, device="cuda"), ver, recs)
+    ctx.sync()
+    assert ver.cpu().tolist() == [1, sum(bumps) + 2]
+    assert prepos.unpack_records(recs)["flags"].tolist() == [0, 0]

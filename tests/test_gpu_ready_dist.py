@@ -1,0 +1,190 @@
+"""GPU parity of a3/a4/a4' (prepos_ready_dist, prepos_scan_logits) against the oracle, through the C ABI."""
+import numpy as np
+import pytest
+import torch
+
+from paper_2606_29565_b200 import synth
+from helpers import bits, check_record, check_decision, LOGIT_ATOL
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def prepos():
+    from paper_2606_29565_b200 import prepos as p
+    p.lib()
+    return p
+
+
+def _run_ready(prepos, shape, hidden, w, n_sessions=None, with_logits=True, session_ids=None, skip=None,
+               versions=None, position=None, ehash=None):
+    n = hidden.shape[0]
+    n_sessions = n if n_sessions is None else n_sessions
+    ctx = prepos.Context(shape.layers, shape.Hq, shape.Hkv, shape.d, shape.H, shape.V, shape.page, max_sessions=max(n, 1))
+    dev = "cuda"
+    sid = torch.arange(n, dtype=torch.int32, device=dev) if session_ids is None else session_ids.to(dev)
+    recs = prepos.new_records(n_sessions)
+    ver = torch.zeros(n_sessions, dtype=torch.int64, device=dev) if versions is None else versions.to(dev)
+    logits = torch.full((n, shape.V), float("nan"), dtype=torch.float32, device=dev) if with_logits else None
+    ctx.ready_dist(sid, hidden.to(dev), w.to(dev), recs, ver, position_p=None if position is None else position.to(dev),
+                   entry_hash=None if ehash is None else ehash.to(dev), skip_mask=None if skip is None else skip.to(dev),
+                   logits_out=logits)
+    ctx.sync()
+    return ctx, recs, ver, logits
+
+
+def test_config1_many_seeds_records_and_gate(prepos, oracle):
+    """BASELINE config 1 vocabulary side: 208 hidden rows (50% planted), records + gate decisions vs oracle."""
+    shape, seed = synth.C1, synth.SEED_BASE
+    w = synth.make_w_vocab(shape, seed)
+    fast = synth.make_fast_set(shape, seed)
+    hidden, planted, _ = synth.make_hidden(shape, 208, w, fast, seed)
+    ctx, recs, ver, logits = _run_ready(prepos, shape, hidden, w)
+    rec = prepos.unpack_records(recs)
+    lg_gpu = logits.cpu().numpy()
+    bm_host = prepos.fastset_build(fast, shape.V)
+    assert np.array_equal(bm_host.numpy().view(np.uint32), oracle.fastset_bitmap(fast.numpy(), shape.V))
+    n = hidden.shape[0]
+    dec = torch.full((n,), -7, dtype=torch.int32, device="cuda")
+    tok = torch.full((n,), -7, dtype=torch.int32, device="cuda")
+    ctx.gate_serve(torch.arange(n, dtype=torch.int32, device="cuda"), recs, ver, bm_host.cuda(), shape.tau, dec, tok)
+    ctx.sync()
+    dec, tok = dec.cpu().tolist(), tok.cpu().tolist()
+    served = 0
+    wb, obm = bits(w), oracle.fastset_bitmap(fast.numpy(), shape.V)
+    for r in range(n):
+        lg64 = oracle.logits(wb, bits(hidden[r]))
+        ref = check_record(oracle, rec, r, lg64, lg_gpu[r])
+        assert int(rec["flags"][r]) == prepos.FLAG_VALID
+        d, _ = check_decision(oracle, dec[r], tok[r], ref, True, 0, 0, obm, shape.V, shape.tau)
+        served += d == oracle.SERVED
+    assert 20 <= served <= 100      # planted rows with realised gap >= 3 fire; unplanted never
+
+
+@pytest.mark.parametrize("V,H,n", [(1000, 128, 3), (130, 384, 1), (257, 256, 9), (4096, 1024, 8), (2, 128, 1)])
+def test_ragged_vocab_and_batches(prepos, oracle, V, H, n):
+    """V not a multiple of the 128-row tile, H with a single stage, n crossing the 8-row pass."""
+    shape = synth.Shape("r", layers=1, Hq=4, Hkv=2, d=64, H=H, V=V, fast_set=2)
+    w = synth.make_w_vocab(shape, 5)
+    hidden = synth.randn_bf16((n, H), synth.gen(6))
+    ctx, recs, ver, logits = _run_ready(prepos, shape, hidden, w)
+    rec = prepos.unpack_records(recs)
+    for r in range(n):
+        check_record(oracle, rec, r, oracle.logits(bits(w), bits(hidden[r])), logits[r].cpu().numpy())
+
+
+def test_ties_lowest_id_wins(prepos, oracle):
+    """Reading Q8: duplicated W rows give bit-equal logits on the GPU; the lower id must be top1, gap 0."""
+    shape = synth.Shape("t", layers=1, Hq=4, Hkv=2, d=64, H=256, V=700, fast_set=2)
+    w = synth.make_w_vocab(shape, 8)
+    hidden = synth.randn_bf16((2, 256), synth.gen(9))
+    lg = oracle.logits(bits(w), bits(hidden[0]))
+    best = int(np.argmax(lg))
+    dup = [3, 650] if best not in (3, 650) else [5, 651]
+    w[dup[0]] = w[best]
+    w[dup[1]] = w[best]
+    ctx, recs, ver, _ = _run_ready(prepos, shape, hidden[:1], w, with_logits=False)
+    rec = prepos.unpack_records(recs)
+    ids = sorted([best] + dup)
+    assert int(rec["top1"][0]) == ids[0] and int(rec["top2"][0]) == ids[1]
+    assert float(rec["gap"][0]) == 0.0
+    ref = oracle.record(oracle.logits(bits(w), bits(hidden[0])))
+    assert (ref.top1, ref.top2, ref.gap) == (ids[0], ids[1], 0.0)
+
+
+def test_record_stamping_skip_and_ids(prepos, oracle):
+    """Alg. 1 l.10-12: position, hash, live version stamped; skip_mask rows untouched; records indexed by id."""
+    shape = synth.Shape("s", layers=1, Hq=4, Hkv=2, d=64, H=128, V=300, fast_set=2)
+    w = synth.make_w_vocab(shape, 11)
+    hidden = synth.randn_bf16((3, 128), synth.gen(12))
+    sid = torch.tensor([4, 0, 2], dtype=torch.int32)
+    ver = torch.tensor([7, 0, 9, 0, 11], dtype=torch.int64)
+    pos = torch.tensor([100, 200, 300], dtype=torch.int64)
+    eh = torch.tensor([0x1234, 0, 0x7fffffffffffffff], dtype=torch.int64)
+    skip = torch.tensor([0, 1, 0], dtype=torch.int32)
+    ctx, recs, _, _ = _run_ready(prepos, shape, hidden, w, n_sessions=5, session_ids=sid, skip=skip, versions=ver,
+                                 position=pos, ehash=eh, with_logits=False)
+    rec = prepos.unpack_records(recs)
+    assert rec["flags"].tolist() == [0, 0, 1, 0, 1]
+    assert rec["version"].tolist() == [0, 0, 9, 0, 11]
+    assert rec["position"].tolist() == [0, 0, 300, 0, 100]
+    assert rec["entry_hash"].tolist() == [0, 0, 0x7fffffffffffffff, 0, 0x1234]
+    for row, s in ((0, 4), (2, 2)):
+        check_record(oracle, rec, s, oracle.logits(bits(w), bits(hidden[row])))
+
+
+def test_nonfinite_logit_is_flagged_and_never_served(prepos, oracle):
+    shape = synth.Shape("n", layers=1, Hq=4, Hkv=2, d=64, H=128, V=256, fast_set=2)
+    w = synth.make_w_vocab(shape, 13)
+    hidden = synth.randn_bf16((1, 128), synth.gen(14))
+    w[17, 5] = float("inf")
+    ctx, recs, ver, _ = _run_ready(prepos, shape, hidden, w, with_logits=False)
+    rec = prepos.unpack_records(recs)
+    assert int(rec["flags"][0]) & prepos.FLAG_NONFINITE
+    bm = prepos.fastset_build(list(range(256)), 256).cuda()
+    dec = torch.zeros(1, dtype=torch.int32, device="cuda")
+    tok = torch.zeros(1, dtype=torch.int32, device="cuda")
+    ctx.gate_serve(torch.zeros(1, dtype=torch.int32, device="cuda"), recs, ver, bm, -1e30, dec, tok)
+    ctx.sync()
+    assert (int(dec[0]), int(tok[0])) == (prepos.STALE_OR_INVALID, -1)
+
+
+def test_scan_logits_matches_oracle_and_shift_invariance(prepos, oracle):
+    """a4' on stored fp32 logits: ids exact (same fp32 values on both sides); shift by c moves max/lse by c."""
+    V = 128256
+    shape = synth.Shape("v", layers=1, Hq=4, Hkv=2, d=64, H=128, V=V, fast_set=2)
+    ctx = prepos.Context(1, 4, 2, 64, 128, V, 16, max_sessions=4)
+    g = synth.gen(21, "cuda")
+    lg = torch.randn((3, V), generator=g, device="cuda", dtype=torch.float32) * 2
+    lg[1] = (lg[1] * 4).round() / 4          # many exact ties
+    lg[2] = lg[0] + 16.0
+    recs = prepos.new_records(3)
+    ctx.scan_logits(lg, recs)
+    ctx.sync()
+    rec = prepos.unpack_records(recs)
+    host = lg.cpu().numpy().astype(np.float64)
+    for r in range(3):
+        ref = oracle.record(host[r])
+        assert (int(rec["top1"][r]), int(rec["top2"][r])) == (ref.top1, ref.top2)
+        assert abs(float(rec["gap"][r]) - ref.gap) < 1e-5 and abs(float(rec["max_logit"][r]) - ref.max_logit) < 1e-6
+        assert abs(float(rec["lse"][r]) - ref.lse) <= 1e-4 * abs(ref.lse)
+    assert int(rec["top1"][2]) == int(rec["top1"][0]) and int(rec["top2"][2]) == int(rec["top2"][0])
+    assert abs(float(rec["lse"][2]) - float(rec["lse"][0]) - 16.0) < 1e-3
+    # unaligned row base (V odd) and tiny V
+    for V2 in (5, 1023):
+        ctx2 = prepos.Context(1, 4, 2, 64, 128, V2, 16, max_sessions=4)
+        lg2 = torch.randn((2, V2), generator=g, device="cuda", dtype=torch.float32)
+        r2 = prepos.new_records(2)
+        ctx2.scan_logits(lg2, r2)
+        ctx2.sync()
+        rr = prepos.unpack_records(r2)
+        for r in range(2):
+            ref = oracle.record(lg2[r].cpu().numpy().astype(np.float64))
+            assert (int(rr["top1"][r]), int(rr["top2"][r])) == (ref.top1, ref.top2)
+
+
+def test_config2_vocabulary_full_size(prepos, oracle):
+    """BASELINE config 2 vocabulary side at full size (V=128256, H=4096): 12 hidden rows, planted fraction 0.6,
+    full logits + records + decisions against the oracle, in the launch configuration bench.py times."""
+    shape, seed = synth.C2, synth.SEED_BASE + 1
+    w = synth.make_w_vocab(shape, seed, "cuda")
+    fast = synth.make_fast_set(shape, seed)
+    hidden, planted, target = synth.make_hidden(shape, 12, w, fast.cuda(), seed)
+    ctx, recs, ver, logits = _run_ready(prepos, shape, hidden, w)
+    rec = prepos.unpack_records(recs)
+    wb = bits(w)
+    obm = oracle.fastset_bitmap(fast.numpy(), shape.V)
+    bm = prepos.fastset_build(fast, shape.V).cuda()
+    n = hidden.shape[0]
+    dec = torch.zeros(n, dtype=torch.int32, device="cuda")
+    tok = torch.zeros(n, dtype=torch.int32, device="cuda")
+    ctx.gate_serve(torch.arange(n, dtype=torch.int32, device="cuda"), recs, ver, bm, shape.tau, dec, tok)
+    ctx.sync()
+    fired = 0
+    for r in range(n):
+        ref = check_record(oracle, rec, r, oracle.logits(wb, bits(hidden[r])), logits[r].cpu().numpy())
+        d, _ = check_decision(oracle, int(dec[r]), int(tok[r]), ref, True, 0, 0, obm, shape.V, shape.tau)
+        fired += d == oracle.SERVED
+        if planted[r]:
+            assert abs(ref.gap - float(target[r])) < 0.3
+    assert fired >= 1
