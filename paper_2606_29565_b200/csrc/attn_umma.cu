@@ -1,6 +1,747 @@
-// attn_umma.cu -- tcgen05/TMEM kernel for a1 + a2 (placeholder until the UMMA path lands).
+// attn_umma.cu -- a1 + a2 on the 5th-generation tensor cores: the entry tokens' G*L query rows attend the
+// session's paged bf16 KV cache (Alg. 1 l.5-6; Eq. 1) as a dense contraction
+// [G*L x d] . [d x n_s] -> softmax -> [G*L x n_s] . [n_s x d] per KV head.  Arithmetic intensity is G*L
+// flop per KV byte (96..384 at the BASELINE configs), so the pass is HBM-bound up to the ridge and needs
+// ~0.6-1 PFLOP/s to stay there: tcgen05.mma with TMEM accumulators, KV pages staged by TMA.
+//
+// Work decomposition (stream-K over KV tiles): the launch's work is the linear space
+//   (layer, kv head) x units x 128-token tiles
+// cut into one contiguous range per persistent CTA (1 CTA / SM).  A CTA walks its range as segments
+// (= its part of one unit).  A unit covered by one segment is written directly; otherwise every
+// covering CTA writes a normalised fp32 partial + log-sum-exp and a small merge kernel combines them in
+// CTA order (deterministic for a fixed plan).
+//
+// Inside a CTA (384 threads):
+//   warp 0  K producer: TMA (5-D map over the pool: one 4 KB box per page) into a ring of K tiles
+//   warp 3  V producer: same for V
+//   warp 2  TMEM allocator; loader of the entry-token tile (K_new/V_new -> swizzled smem) and the
+//           Append(E) writer (Alg. 1 l.5)
+//   warp 1  MMA issuer: S = Q K^T (SS, K-major SW128) into TMEM, O += P V (A = P from TMEM, B = V MN-major)
+//   warps 4-7 / 8-11  two softmax warpgroups, one TMEM lane (= query row) per thread: online softmax
+//           with lazy rescaling, P written back to TMEM as bf16 over S.
+// The CTA always runs two independent streams (S_w, O_w, own running max/sum): with >128 rows stream w
+// owns M-tile w; with <=128 rows the streams take alternate KV tiles and are merged in the epilogue.
+#include <math_constants.h>
+#include <stdio.h>
+
 #include "common.cuh"
+#include "ptx.cuh"
 
-bool prepos_attn_umma_supported(const prepos_ctx *) { return false; }
+namespace {
 
-int prepos_launch_attn_umma(prepos_ctx *, const AttnArgs &, int, cudaStream_t) { return PREPOS_E_SHAPE; }
+constexpr int kThreads = 384;
+constexpr int kTile = kAttnTileTokens;  // 128 tokens
+constexpr int kNK = 3;                  // K ring slots
+constexpr int kMaxNV = 3;               // V ring slots (3 when only one Q tile is resident, else 2)
+constexpr float kRescaleThreshold = 8.f;  // log2 units: lazy rescale (P <= 2^8)
+
+struct UmmaParams {
+    AttnArgs a;
+    const AttnUnit *units;
+    int Hq, Hkv, page, page_shift;
+    int n_lh;           // (layer, kv head) pairs in this launch
+    int tiles_per_lh;   // sum of n_tiles over units
+    long long total_tiles;
+    int q_tiles;        // resident Q M-tiles (1 or 2)
+    int nv;             // V ring slots
+    float scale_log2;
+    float *partials;    // [2 * grid] slots of kAttnMaxRows * (D + 2) floats: O [256][D], lse2 [256], pad [256]
+};
+
+struct Seg {
+    AttnUnit u;
+    int unit_idx, layer, kvh;
+    int tb, te;      // tile range within the unit
+    int first;       // 1 = first segment of this CTA
+    int direct;      // segment covers the whole unit
+};
+
+// Walks the CTA's contiguous range [t0, t1) of the global tile space as segments.
+struct SegIter {
+    long long t, t1;
+    int first, prev_unit;
+    __device__ SegIter(long long t0_, long long t1_) : t(t0_), t1(t1_), first(1), prev_unit(-1) {}
+    __device__ bool next(const UmmaParams &p, Seg &s)
+    {
+        if (t >= t1) return false;
+        const int lh = static_cast<int>(t / p.tiles_per_lh);
+        const int off = static_cast<int>(t - static_cast<long long>(lh) * p.tiles_per_lh);
+        int lo;
+        if (prev_unit < 0) {
+            // first segment: binary search for the last unit with tile_prefix <= off
+            lo = 0;
+            int hi = p.a.n_units - 1;
+            while (lo < hi) {
+                const int mid = (lo + hi + 1) >> 1;
+                if (p.units[mid].tile_prefix <= off) lo = mid;
+                else hi = mid - 1;
+            }
+        } else {
+            lo = (prev_unit + 1 == p.a.n_units) ? 0 : prev_unit + 1;  // segments end on unit boundaries
+        }
+        prev_unit = lo;
+        s.unit_idx = lo;
+        s.u = p.units[lo];
+        s.layer = p.a.layer_begin + lh / p.Hkv;
+        s.kvh = lh % p.Hkv;
+        s.tb = off - s.u.tile_prefix;
+        const long long unit_end = static_cast<long long>(lh) * p.tiles_per_lh + s.u.tile_prefix + s.u.n_tiles;
+        const long long end = unit_end < t1 ? unit_end : t1;
+        s.te = s.tb + static_cast<int>(end - t);
+        s.first = first;
+        s.direct = (s.tb == 0 && s.te == s.u.n_tiles);
+        first = 0;
+        t = end;
+        return true;
+    }
+};
+
+__device__ __forceinline__ long long cta_begin(long long total, int grid, int c)
+{
+    return total * c / grid;
+}
+
+// 64-bit UMMA shared-memory descriptor, SWIZZLE_128B, version 1 (sm_100)
+__device__ __forceinline__ uint64_t make_desc(uint32_t saddr, uint32_t lbo_bytes, uint32_t sbo_bytes)
+{
+    uint64_t d = 0;
+    d |= static_cast<uint64_t>((saddr >> 4) & 0x3fff);
+    d |= static_cast<uint64_t>((lbo_bytes >> 4) & 0x3fff) << 16;
+    d |= static_cast<uint64_t>((sbo_bytes >> 4) & 0x3fff) << 32;
+    d |= 1ull << 46;  // descriptor version
+    d |= 2ull << 61;  // SWIZZLE_128B
+    return d;
+}
+
+// byte offset of (row r, 16-byte chunk c of a D-wide bf16 row) in a tile laid out
+// [row group of 8][64-column half][8 rows][128 B] with the 128-byte swizzle (chunk ^= row % 8)
+template <int D>
+__device__ __forceinline__ uint32_t tile_offset(int r, int c)
+{
+    constexpr int kHalves = D / 64;
+    const int hf = c >> 3, cc = c & 7;
+    return static_cast<uint32_t>((r >> 3) * (kHalves * 1024) + hf * 1024 + (r & 7) * 128 + ((cc ^ (r & 7)) << 4));
+}
+
+__device__ __forceinline__ uint32_t pack_bf16(float lo, float hi)
+{
+    uint32_t r;
+    asm("cvt.rn.bf16x2.f32 %0, %1, %2;" : "=r"(r) : "f"(hi), "f"(lo));
+    return r;
+}
+
+template <int D>
+__global__ void __launch_bounds__(kThreads, 1)
+attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__ CUtensorMap tm_v,
+                 const UmmaParams p)
+{
+    constexpr int kHalves = D / 64;
+    constexpr int kTileBytes = kTile * D * 2;         // one K or V tile / one Q M-tile
+    constexpr int kGroupStride = kHalves * 1024;      // bytes between 8-row groups
+    constexpr uint32_t kIdescQK = (1u << 4) | (1u << 7) | (1u << 10) | ((kTile >> 3) << 17) | ((128u >> 4) << 24);
+    constexpr uint32_t kIdescPV = (1u << 4) | (1u << 7) | (1u << 10) | (1u << 16) | ((D >> 3) << 17) | ((128u >> 4) << 24);
+    constexpr int kColS = 0;        // S_w at columns w * 128 (P_w aliases its first 64 columns)
+    constexpr int kColO = 256;      // O_w at columns 256 + w * D
+
+    extern __shared__ __align__(1024) uint8_t smem_raw[];
+    if (ptx::smem_u32(smem_raw) & 1023u) __trap();  // the swizzled tiles rely on the 1024-byte base alignment
+    uint8_t *q_s = smem_raw;
+    uint8_t *k_s = q_s + p.q_tiles * kTileBytes;
+    uint8_t *v_s = k_s + kNK * kTileBytes;
+    uint8_t *tail = v_s + p.nv * kTileBytes;
+    uint64_t *bars = reinterpret_cast<uint64_t *>(tail);
+    uint64_t *k_full = bars, *k_empty = bars + 3, *v_full = bars + 6, *v_empty = bars + 9;
+    uint64_t *s_full = bars + 12, *p_ready = bars + 14, *o_done = bars + 16, *q_full = bars + 18;
+    float2 *ml_x = reinterpret_cast<float2 *>(bars + 20);  // [2][128] (m_used, l) exchange
+    uint32_t *tmem_slot = reinterpret_cast<uint32_t *>(ml_x + 256);
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+
+    if (threadIdx.x == 32) {
+        for (int i = 0; i < 3; ++i) {
+            ptx::mbar_init(ptx::smem_u32(&k_full[i]), 1);
+            ptx::mbar_init(ptx::smem_u32(&k_empty[i]), 1);
+            ptx::mbar_init(ptx::smem_u32(&v_full[i]), 1);
+            ptx::mbar_init(ptx::smem_u32(&v_empty[i]), 1);
+        }
+        for (int i = 0; i < 2; ++i) {
+            ptx::mbar_init(ptx::smem_u32(&s_full[i]), 1);
+            ptx::mbar_init(ptx::smem_u32(&p_ready[i]), 128);
+            ptx::mbar_init(ptx::smem_u32(&o_done[i]), 1);
+        }
+        ptx::mbar_init(ptx::smem_u32(q_full), 256);
+        ptx::fence_mbar_init();
+    }
+    if (warp == 2) {
+        ptx::tmem_alloc<512>(ptx::smem_u32(tmem_slot));
+        ptx::tmem_relinquish();
+    }
+    ptx::tc_fence_before();
+    __syncthreads();
+    ptx::tc_fence_after();
+    const uint32_t tmem = *tmem_slot;
+
+    const long long t0 = cta_begin(p.total_tiles, gridDim.x, blockIdx.x);
+    const long long t1 = cta_begin(p.total_tiles, gridDim.x, blockIdx.x + 1);
+    const int G = p.Hq / p.Hkv;
+    const int pages_per_tile = kTile >> p.page_shift;
+    const int page_bytes = p.page * D * 2;
+    const int page_groups = p.page >> 3;
+
+    // register budget: the four service warps need few registers, the softmax threads hold a 128-wide score row
+    // (setmaxnreg tuning comes after correctness)
+
+    if (warp == 0 || warp == 3) {
+        // ===================== K (warp 0) / V (warp 3) TMA producers =====================
+        const bool is_v = (warp == 3);
+        const CUtensorMap *tm = is_v ? &tm_v : &tm_k;
+        uint64_t *full = is_v ? v_full : k_full, *empty = is_v ? v_empty : k_empty;
+        uint8_t *ring = is_v ? v_s : k_s;
+        const int n_slots = is_v ? p.nv : kNK;
+        if (lane == 0) ptx::prefetch_tmap(tm);
+        const uint64_t pol = ptx::policy_evict_first();
+        int slot = 0;
+        uint32_t ph = 0;
+        SegIter it(t0, t1);
+        Seg s;
+        while (it.next(p, s)) {
+            const int n_pages_valid = (s.u.n_s + p.page - 1) >> p.page_shift;
+            const int32_t *pt = p.a.page_table + static_cast<size_t>(s.u.session) * p.a.page_table_stride;
+            for (int t = s.tb; t < s.te; ++t) {
+                if (t < s.u.n_cached_tiles) {
+                    const int first_page = t * pages_per_tile;
+                    int nvp = n_pages_valid - first_page;
+                    nvp = nvp < pages_per_tile ? nvp : pages_per_tile;
+                    int pg = 0;
+                    if (lane < nvp) pg = __ldg(pt + first_page + lane);
+                    if (lane == 0) {
+                        ptx::mbar_wait(ptx::smem_u32(&empty[slot]), ph ^ 1);
+                        ptx::mbar_arrive_expect_tx(ptx::smem_u32(&full[slot]), nvp * page_bytes);
+                    }
+                    __syncwarp();
+                    if (lane < nvp)
+                        ptx::tma_load_5d(ptx::smem_u32(ring + slot * kTileBytes + lane * page_bytes), tm,
+                                         ptx::smem_u32(&full[slot]), 0, 0, 0, (pg * p.Hkv + s.kvh) * page_groups,
+                                         s.layer, pol);
+                } else {
+                    // entry-token tiles are filled by warp 2; wait all the same so that the phase parity this
+                    // warp tracks never falls two rounds behind the barrier
+                    if (lane == 0) ptx::mbar_wait(ptx::smem_u32(&empty[slot]), ph ^ 1);
+                    __syncwarp();
+                }
+                if (++slot == n_slots) {
+                    slot = 0;
+                    ph ^= 1;
+                }
+            }
+        }
+    } else if (warp == 2) {
+        // ===================== entry-token tile loader + Append(E) =====================
+        int kslot = 0, vslot = 0;
+        uint32_t kph = 0, vph = 0;
+        SegIter it(t0, t1);
+        Seg s;
+        constexpr int kChunks = D / 8;  // 16-byte chunks per row
+        while (it.next(p, s)) {
+            for (int t = s.tb; t < s.te; ++t) {
+                if (t >= s.u.n_cached_tiles) {
+                    const int nb = (t - s.u.n_cached_tiles) * kTile;      // first entry token of this tile
+                    int nvis = s.u.tok0 + s.u.ntok - nb;                   // entry tokens this unit can see here
+                    nvis = nvis < kTile ? nvis : kTile;
+                    const bool append = (s.u.tok0 + s.u.ntok == s.u.l_entry);  // last row chunk owns Append(E)
+                    const size_t lo = static_cast<size_t>(s.layer);
+                    const int32_t *pt = p.a.page_table + static_cast<size_t>(s.u.session) * p.a.page_table_stride;
+#pragma unroll 1
+                    for (int which = 0; which < 2; ++which) {
+                        const __nv_bfloat16 *src = (which ? p.a.v_new : p.a.k_new) + lo * p.a.kv_new_layer_stride;
+                        __nv_bfloat16 *pool = (which ? p.a.v_pool : p.a.k_pool) + lo * p.a.pool_layer_stride;
+                        uint8_t *dst = which ? v_s + vslot * kTileBytes : k_s + kslot * kTileBytes;
+                        ptx::mbar_wait(ptx::smem_u32(which ? &v_empty[vslot] : &k_empty[kslot]), (which ? vph : kph) ^ 1);
+                        for (int idx = lane; idx < kTile * kChunks; idx += 32) {
+                            const int r = idx / kChunks, c = idx - r * kChunks;
+                            uint4 val = make_uint4(0, 0, 0, 0);
+                            if (r < nvis) {
+                                const int tok = nb + r;
+                                val = *reinterpret_cast<const uint4 *>(
+                                    src + (static_cast<size_t>(s.u.row0 + tok) * p.Hkv + s.kvh) * D + c * 8);
+                                if (append) {
+                                    const int j = s.u.n_s + tok;
+                                    const int pg = __ldg(pt + (j >> p.page_shift));
+                                    *reinterpret_cast<uint4 *>(
+                                        pool + ((static_cast<size_t>(pg) * p.Hkv + s.kvh) * p.page + (j & (p.page - 1))) * D +
+                                        c * 8) = val;
+                                }
+                            }
+                            *reinterpret_cast<uint4 *>(dst + tile_offset<D>(r, c)) = val;
+                        }
+                        ptx::fence_proxy_async_smem();
+                        __syncwarp();
+                        if (lane == 0) ptx::mbar_arrive(ptx::smem_u32(which ? &v_full[vslot] : &k_full[kslot]));
+                    }
+                } else {
+                    // cached tiles belong to the TMA producers; keep this warp's parities in lockstep (see there)
+                    ptx::mbar_wait(ptx::smem_u32(&k_empty[kslot]), kph ^ 1);
+                    ptx::mbar_wait(ptx::smem_u32(&v_empty[vslot]), vph ^ 1);
+                }
+                if (++kslot == kNK) {
+                    kslot = 0;
+                    kph ^= 1;
+                }
+                if (++vslot == p.nv) {
+                    vslot = 0;
+                    vph ^= 1;
+                }
+            }
+        }
+    } else if (warp == 1) {
+        // ===================== MMA issuer =====================
+        int kslot = 0, vslot = 0;
+        uint32_t kph = 0, vph = 0, qph = 0;
+        uint32_t pph[2] = {0, 0};
+        SegIter it(t0, t1);
+        Seg s;
+        while (it.next(p, s)) {
+            const int rows = s.u.ntok * G;
+            const int n_mt = rows > 128 ? 2 : 1;
+            const int n_tiles = s.te - s.tb;
+            const int n_items = n_tiles * n_mt;
+            ptx::mbar_wait(ptx::smem_u32(q_full), qph);
+            qph ^= 1;
+            ptx::tc_fence_after();
+
+            auto issue_qk = [&](int i) {
+                const int w = i & 1;
+                const int mt = (n_mt == 2) ? w : 0;
+                const bool first_use = (n_mt == 1) || w == 0;
+                const bool last_use = (n_mt == 1) || w == 1;
+                if (first_use) {
+                    ptx::mbar_wait(ptx::smem_u32(&k_full[kslot]), kph);
+                    ptx::tc_fence_after();
+                }
+                if (lane == 0) {
+                    const uint32_t qa = ptx::smem_u32(q_s + mt * kTileBytes);
+                    const uint32_t ka = ptx::smem_u32(k_s + kslot * kTileBytes);
+#pragma unroll
+                    for (int hf = 0; hf < kHalves; ++hf)
+#pragma unroll
+                        for (int ks = 0; ks < 4; ++ks) {
+                            const uint32_t off = hf * 1024 + ks * 32;
+                            ptx::umma_ss(tmem + kColS + w * 128, make_desc(qa + off, 16, kGroupStride),
+                                         make_desc(ka + off, 16, kGroupStride), kIdescQK, (hf | ks) != 0);
+                        }
+                    ptx::umma_commit(ptx::smem_u32(&s_full[w]));
+                    if (last_use) ptx::umma_commit(ptx::smem_u32(&k_empty[kslot]));
+                }
+                __syncwarp();
+                if (last_use) {
+                    if (++kslot == kNK) {
+                        kslot = 0;
+                        kph ^= 1;
+                    }
+                }
+            };
+
+            issue_qk(0);
+            if (n_items > 1) issue_qk(1);
+            for (int i = 0; i < n_items; ++i) {
+                const int w = i & 1;
+                const int t = s.tb + (n_mt == 2 ? (i >> 1) : i);
+                const bool first_use = (n_mt == 1) || w == 0;
+                const bool last_use = (n_mt == 1) || w == 1;
+                if (first_use) {
+                    ptx::mbar_wait(ptx::smem_u32(&v_full[vslot]), vph);
+                    // rows past the valid tokens of a ragged cached tile hold whatever the pool / the ring held:
+                    // P is exactly 0 there, but 0 * NaN would poison O, so zero them before the MMA reads them.
+                    if (t < s.u.n_cached_tiles) {
+                        const int valid = s.u.n_s - t * kTile;
+                        if (valid < kTile) {
+                            uint8_t *vb = v_s + vslot * kTileBytes;
+                            for (int idx = valid * (D / 8) + lane; idx < kTile * (D / 8); idx += 32) {
+                                const int r = idx / (D / 8), c = idx - r * (D / 8);
+                                *reinterpret_cast<uint4 *>(vb + tile_offset<D>(r, c)) = make_uint4(0, 0, 0, 0);
+                            }
+                            ptx::fence_proxy_async_smem();
+                            __syncwarp();
+                        }
+                    }
+                }
+                ptx::mbar_wait(ptx::smem_u32(&p_ready[w]), pph[w]);
+                pph[w] ^= 1;
+                ptx::tc_fence_after();
+                if (lane == 0) {
+                    const uint32_t va = ptx::smem_u32(v_s + vslot * kTileBytes);
+                    const bool first_pv = (i < 2);  // first PV of stream i & 1 in this segment overwrites O
+#pragma unroll
+                    for (int ks = 0; ks < kTile / 16; ++ks)
+                        ptx::umma_ts(tmem + kColO + w * D, tmem + kColS + w * 128 + ks * 8,
+                                     make_desc(va + ks * 2 * kGroupStride, 1024, kGroupStride), kIdescPV,
+                                     !(first_pv && ks == 0));
+                    if (last_use) ptx::umma_commit(ptx::smem_u32(&v_empty[vslot]));
+                }
+                __syncwarp();
+                if (last_use) {
+                    if (++vslot == p.nv) {
+                        vslot = 0;
+                        vph ^= 1;
+                    }
+                }
+                if (i + 2 < n_items) issue_qk(i + 2);
+            }
+            if (lane == 0) {
+                ptx::umma_commit(ptx::smem_u32(&o_done[0]));
+                ptx::umma_commit(ptx::smem_u32(&o_done[1]));
+            }
+            __syncwarp();
+        }
+    } else {
+        // ===================== softmax warpgroups (warps 4-7: stream 0, warps 8-11: stream 1) =====================
+        const int w = (warp - 4) >> 2;
+        const int row = ((warp & 3) << 5) | lane;              // TMEM lane == row within the M-tile
+        const uint32_t lane_addr = static_cast<uint32_t>((warp & 3) << 5) << 16;
+        const int st = threadIdx.x - 128;                      // 0..255 among softmax threads
+        uint32_t sph = 0, oph = 0;
+        SegIter it(t0, t1);
+        Seg s;
+        while (it.next(p, s)) {
+            const int rows = s.u.ntok * G;
+            const int n_mt = rows > 128 ? 2 : 1;
+            const int n_tiles = s.te - s.tb;
+            const int n_items = n_tiles * n_mt;
+            // ---- Q rows -> smem (swizzled K-major tiles; rows past the unit zero).  Row r of the unit is entry
+            // token tok0 + r / G, query head kvh * G + r % G.
+            {
+                constexpr int kChunks = D / 8;
+                const __nv_bfloat16 *qb = p.a.q + static_cast<size_t>(s.layer) * p.a.q_layer_stride;
+                for (int idx = st; idx < n_mt * 128 * kChunks; idx += 256) {
+                    const int r = idx / kChunks, c = idx - r * kChunks;
+                    uint4 val = make_uint4(0, 0, 0, 0);
+                    if (r < rows) {
+                        const int tok = s.u.tok0 + r / G, h = s.kvh * G + r % G;
+                        val = __ldg(reinterpret_cast<const uint4 *>(
+                            qb + (static_cast<size_t>(s.u.row0 + tok) * p.Hq + h) * D + c * 8));
+                    }
+                    *reinterpret_cast<uint4 *>(q_s + (r >> 7) * kTileBytes + tile_offset<D>(r & 127, c)) = val;
+                }
+                ptx::fence_proxy_async_smem();
+                ptx::tc_fence_before();  // epilogue TMEM reads of the previous segment precede this arrive
+                ptx::mbar_arrive(ptx::smem_u32(q_full));
+            }
+            const int mt = (n_mt == 2) ? w : 0;
+            const int urow = mt * 128 + row;                   // row within the unit
+            const int my_tok = s.u.tok0 + urow / G;            // entry token of this row (if urow < rows)
+            float m_used = -CUDART_INF_F, l_sum = 0.f;
+            bool have = false;
+            for (int i = w; i < n_items; i += 2) {
+                const int t = s.tb + (n_mt == 2 ? (i >> 1) : i);
+                // visible columns of this tile for this row
+                int limit = kTile;
+                if (t < s.u.n_cached_tiles) {
+                    const int valid = s.u.n_s - t * kTile;
+                    limit = valid < kTile ? valid : kTile;
+                } else {
+                    const int nb = (t - s.u.n_cached_tiles) * kTile;
+                    limit = (urow < rows) ? my_tok - nb + 1 : 1;   // causal among the entry tokens (reading Q5)
+                    limit = limit < 0 ? 0 : (limit > kTile ? kTile : limit);
+                }
+                ptx::mbar_wait(ptx::smem_u32(&s_full[w]), sph);
+                sph ^= 1;
+                ptx::tc_fence_after();
+                uint32_t sr[128];
+                {
+                    const uint32_t sa = tmem + lane_addr + kColS + w * 128;
+                    ptx::tmem_ld_32x32b_x32(sa, sr);
+                    ptx::tmem_ld_32x32b_x32(sa + 32, sr + 32);
+                    ptx::tmem_ld_32x32b_x32(sa + 64, sr + 64);
+                    ptx::tmem_ld_32x32b_x32(sa + 96, sr + 96);
+                    ptx::tmem_ld_wait();
+                }
+                float mx = -CUDART_INF_F;
+                if (limit >= kTile) {
+#pragma unroll
+                    for (int c = 0; c < 128; ++c) mx = fmaxf(mx, __uint_as_float(sr[c]));
+                } else {
+#pragma unroll
+                    for (int c = 0; c < 128; ++c) {
+                        const float v = (c < limit) ? __uint_as_float(sr[c]) : -CUDART_INF_F;
+                        sr[c] = __float_as_uint(v);
+                        mx = fmaxf(mx, v);
+                    }
+                }
+                const float m_new = fmaxf(m_used, mx * p.scale_log2);
+                // lazy rescale, warp-uniform because the TMEM round trip of O is warp-collective
+                const bool need = (m_new > m_used + kRescaleThreshold);
+                if (__any_sync(0xffffffffu, need)) {
+                    const float alpha = (m_used == -CUDART_INF_F) ? 0.f : exp2f(m_used - m_new);
+                    l_sum *= alpha;
+                    if (have) {
+                        const uint32_t oa = tmem + lane_addr + kColO + w * D;
+#pragma unroll
+                        for (int cb = 0; cb < D; cb += 32) {
+                            uint32_t o[32];
+                            ptx::tmem_ld_32x32b_x32(oa + cb, o);
+                            ptx::tmem_ld_wait();
+#pragma unroll
+                            for (int c = 0; c < 32; ++c) o[c] = __float_as_uint(__uint_as_float(o[c]) * alpha);
+                            ptx::tmem_st_32x32b_x32(oa + cb, o);
+                        }
+                    }
+                    m_used = m_new;
+                }
+                const float m_eff = (m_used == -CUDART_INF_F) ? 0.f : m_used;  // fully masked so far: p = 0
+                const float neg_m = -m_eff;
+                const uint32_t pa = tmem + lane_addr + kColS + w * 128;
+#pragma unroll
+                for (int cb = 0; cb < 128; cb += 64) {
+                    uint32_t pk[32];
+#pragma unroll
+                    for (int c = 0; c < 64; c += 2) {
+                        const float p0 = ptx::ex2(fmaf(__uint_as_float(sr[cb + c]), p.scale_log2, neg_m));
+                        const float p1 = ptx::ex2(fmaf(__uint_as_float(sr[cb + c + 1]), p.scale_log2, neg_m));
+                        l_sum += p0 + p1;
+                        pk[c >> 1] = pack_bf16(p0, p1);
+                    }
+                    ptx::tmem_st_32x32b_x32(pa + (cb >> 1), pk);
+                }
+                ptx::tmem_st_wait();
+                ptx::tc_fence_before();
+                ptx::mbar_arrive(ptx::smem_u32(&p_ready[w]));
+                have = true;
+            }
+            // ---- epilogue
+            ptx::mbar_wait(ptx::smem_u32(&o_done[w]), oph);
+            oph ^= 1;
+            ptx::tc_fence_after();
+            __nv_bfloat16 *ob = p.a.out + static_cast<size_t>(s.layer) * p.a.out_layer_stride;
+            float *slot = p.partials + static_cast<size_t>(2 * blockIdx.x + (s.first ? 0 : 1)) * (kAttnMaxRows * (D + 2));
+            if (n_mt == 2) {
+                // stream w owns M-tile w: rows urow, all D columns
+                const float inv = 1.f / l_sum;
+                const bool live = urow < rows;
+                const uint32_t oa = tmem + lane_addr + kColO + w * D;
+                __nv_bfloat16 *orow = ob + (static_cast<size_t>(s.u.row0 + my_tok) * p.Hq + s.kvh * G + urow % G) * D;
+#pragma unroll
+                for (int cb = 0; cb < D; cb += 32) {
+                    uint32_t o[32];
+                    ptx::tmem_ld_32x32b_x32(oa + cb, o);
+                    ptx::tmem_ld_wait();
+                    if (live) {
+                        if (s.direct) {
+#pragma unroll
+                            for (int c = 0; c < 32; c += 8) {
+                                uint4 v;
+                                v.x = pack_bf16(__uint_as_float(o[c]) * inv, __uint_as_float(o[c + 1]) * inv);
+                                v.y = pack_bf16(__uint_as_float(o[c + 2]) * inv, __uint_as_float(o[c + 3]) * inv);
+                                v.z = pack_bf16(__uint_as_float(o[c + 4]) * inv, __uint_as_float(o[c + 5]) * inv);
+                                v.w = pack_bf16(__uint_as_float(o[c + 6]) * inv, __uint_as_float(o[c + 7]) * inv);
+                                *reinterpret_cast<uint4 *>(orow + cb + c) = v;
+                            }
+                        } else {
+#pragma unroll
+                            for (int c = 0; c < 32; c += 4)
+                                *reinterpret_cast<float4 *>(slot + static_cast<size_t>(urow) * D + cb + c) =
+                                    make_float4(__uint_as_float(o[c]) * inv, __uint_as_float(o[c + 1]) * inv,
+                                                __uint_as_float(o[c + 2]) * inv, __uint_as_float(o[c + 3]) * inv);
+                        }
+                    }
+                }
+                if (live && !s.direct) slot[kAttnMaxRows * D + urow] = m_used + log2f(l_sum);
+            } else {
+                // both streams hold partial sums of the same rows: exchange (m, l), then WG w finishes columns
+                // [w * D/2, (w+1) * D/2) of the merged row
+                ml_x[w * 128 + row] = make_float2(m_used, l_sum);
+                ptx::bar_sync(1, 256);
+                const float2 a = ml_x[row], b = ml_x[128 + row];
+                const bool two = n_items > 1;
+                const float M = two ? fmaxf(a.x, b.x) : a.x;
+                const float wa = exp2f(a.x - M), wb = two ? exp2f(b.x - M) : 0.f;
+                const float L = wa * a.y + wb * b.y;
+                const float inv = 1.f / L;
+                const float fa = wa * inv, fb = wb * inv;
+                const bool live = row < rows;
+                constexpr int kHalfD = D / 2;
+                const uint32_t oa0 = tmem + lane_addr + kColO + w * kHalfD;
+                const uint32_t oa1 = tmem + lane_addr + kColO + D + w * kHalfD;
+                const int tok = s.u.tok0 + row / G;
+                __nv_bfloat16 *orow = ob + (static_cast<size_t>(s.u.row0 + tok) * p.Hq + s.kvh * G + row % G) * D + w * kHalfD;
+#pragma unroll
+                for (int cb = 0; cb < kHalfD; cb += 32) {
+                    uint32_t o0[32], o1[32];
+                    ptx::tmem_ld_32x32b_x32(oa0 + cb, o0);
+                    if (two) ptx::tmem_ld_32x32b_x32(oa1 + cb, o1);
+                    ptx::tmem_ld_wait();
+                    float f[32];
+#pragma unroll
+                    for (int c = 0; c < 32; ++c)
+                        f[c] = two ? fmaf(__uint_as_float(o0[c]), fa, __uint_as_float(o1[c]) * fb)
+                                   : __uint_as_float(o0[c]) * fa;
+                    if (live) {
+                        if (s.direct) {
+#pragma unroll
+                            for (int c = 0; c < 32; c += 8) {
+                                uint4 v;
+                                v.x = pack_bf16(f[c], f[c + 1]);
+                                v.y = pack_bf16(f[c + 2], f[c + 3]);
+                                v.z = pack_bf16(f[c + 4], f[c + 5]);
+                                v.w = pack_bf16(f[c + 6], f[c + 7]);
+                                *reinterpret_cast<uint4 *>(orow + cb + c) = v;
+                            }
+                        } else {
+#pragma unroll
+                            for (int c = 0; c < 32; c += 4)
+                                *reinterpret_cast<float4 *>(slot + static_cast<size_t>(row) * D + w * kHalfD + cb + c) =
+                                    make_float4(f[c], f[c + 1], f[c + 2], f[c + 3]);
+                        }
+                    }
+                }
+                if (live && !s.direct && w == 0) slot[kAttnMaxRows * D + row] = M + log2f(L);
+                ptx::bar_sync(1, 256);  // ml_x is reused by the next segment
+            }
+        }
+    }
+
+    ptx::tc_fence_before();
+    __syncthreads();
+    if (warp == 2) ptx::tmem_dealloc<512>(tmem);
+}
+
+// Combines the partials of every unit that was cut across CTAs.  grid (n_units, Hkv, layers), 128 threads.
+template <int D>
+__global__ void __launch_bounds__(128) attn_merge_kernel(const UmmaParams p, int main_grid)
+{
+    const AttnUnit u = p.units[blockIdx.x];
+    const int kvh = blockIdx.y, lz = blockIdx.z;
+    const int lh = lz * p.Hkv + kvh;
+    const int G = p.Hq / p.Hkv;
+    const int rows = u.ntok * G;
+    const long long U0 = static_cast<long long>(lh) * p.tiles_per_lh + u.tile_prefix;
+    const long long U1 = U0 + u.n_tiles;
+    // CTAs covering [U0, U1)
+    int c0 = static_cast<int>(U0 * main_grid / p.total_tiles);
+    while (c0 + 1 < main_grid && cta_begin(p.total_tiles, main_grid, c0 + 1) <= U0) ++c0;
+    while (c0 > 0 && cta_begin(p.total_tiles, main_grid, c0) > U0) --c0;
+    int c1 = c0;
+    while (c1 + 1 < main_grid && cta_begin(p.total_tiles, main_grid, c1 + 1) < U1) ++c1;
+    if (c0 == c1) return;  // written directly by its only CTA
+    const size_t slot_floats = static_cast<size_t>(kAttnMaxRows) * (D + 2);
+    __nv_bfloat16 *ob = p.a.out + static_cast<size_t>(p.a.layer_begin + lz) * p.a.out_layer_stride;
+    constexpr int kVec = D / 4;  // float4 per row
+    for (int idx = threadIdx.x; idx < rows * kVec; idx += blockDim.x) {
+        const int r = idx / kVec, v = idx - r * kVec;
+        float M = -CUDART_INF_F;
+        for (int c = c0; c <= c1; ++c) {
+            const float *slot = p.partials + (2 * static_cast<size_t>(c) + (cta_begin(p.total_tiles, main_grid, c) < U0 ? 1 : 0)) * slot_floats;
+            M = fmaxf(M, slot[kAttnMaxRows * D + r]);
+        }
+        float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
+        float wsum = 0.f;
+        for (int c = c0; c <= c1; ++c) {
+            const float *slot = p.partials + (2 * static_cast<size_t>(c) + (cta_begin(p.total_tiles, main_grid, c) < U0 ? 1 : 0)) * slot_floats;
+            const float wgt = exp2f(slot[kAttnMaxRows * D + r] - M);
+            const float4 o = *reinterpret_cast<const float4 *>(slot + static_cast<size_t>(r) * D + v * 4);
+            acc.x = fmaf(wgt, o.x, acc.x);
+            acc.y = fmaf(wgt, o.y, acc.y);
+            acc.z = fmaf(wgt, o.z, acc.z);
+            acc.w = fmaf(wgt, o.w, acc.w);
+            wsum += wgt;
+        }
+        const float inv = 1.f / wsum;
+        const int tok = u.tok0 + r / G, h = kvh * G + r % G;
+        uint2 pk;
+        pk.x = pack_bf16(acc.x * inv, acc.y * inv);
+        pk.y = pack_bf16(acc.z * inv, acc.w * inv);
+        *reinterpret_cast<uint2 *>(ob + (static_cast<size_t>(u.row0 + tok) * p.Hq + h) * D + v * 4) = pk;
+    }
+}
+
+typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
+                                  const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+int encode_pool_map(CUtensorMap *tm, void *pool, const prepos_model_shape &s, int64_t layer_stride, int64_t n_pages)
+{
+    EncodeTiledFn encode = reinterpret_cast<EncodeTiledFn>(prepos_get_encode_tiled());
+    if (!encode) return PREPOS_E_CUDA;
+    const int D = s.head_dim, halves = D / 64, groups = s.page_size / 8;
+    const cuuint64_t dims[5] = {64, 8, static_cast<cuuint64_t>(halves),
+                                static_cast<cuuint64_t>(n_pages) * s.n_kv_heads * groups,
+                                static_cast<cuuint64_t>(s.layers)};
+    const cuuint64_t strides[4] = {static_cast<cuuint64_t>(D) * 2, 128, static_cast<cuuint64_t>(8) * D * 2,
+                                   static_cast<cuuint64_t>(layer_stride) * 2};
+    const cuuint32_t box[5] = {64, 8, static_cast<cuuint32_t>(halves), static_cast<cuuint32_t>(groups), 1};
+    const cuuint32_t estr[5] = {1, 1, 1, 1, 1};
+    const CUresult r = encode(tm, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 5, pool, dims, strides, box, estr,
+                              CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
+                              CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) {
+        fprintf(stderr, "libprepos: cuTensorMapEncodeTiled(pool) failed: %d\n", static_cast<int>(r));
+        return PREPOS_E_CUDA;
+    }
+    return PREPOS_OK;
+}
+
+template <int D>
+int launch(prepos_ctx *ctx, const AttnArgs &a, int tiles_per_lh, cudaStream_t stream)
+{
+    UmmaParams p;
+    p.a = a;
+    p.units = ctx->attn_units;
+    p.Hq = ctx->shape.n_q_heads;
+    p.Hkv = ctx->shape.n_kv_heads;
+    p.page = ctx->shape.page_size;
+    p.page_shift = 0;
+    while ((1 << p.page_shift) < p.page) ++p.page_shift;
+    p.n_lh = (a.layer_end - a.layer_begin) * p.Hkv;
+    p.tiles_per_lh = tiles_per_lh;
+    p.total_tiles = static_cast<long long>(p.n_lh) * tiles_per_lh;
+    p.scale_log2 = a.scale * 1.4426950408889634f;
+    p.partials = ctx->attn_partials;
+    const int G = p.Hq / p.Hkv;
+    bool two = false;
+    for (const AttnUnit &u : ctx->plan_units) two |= (u.ntok * G > 128);
+    p.q_tiles = two ? 2 : 1;
+    p.nv = two ? 2 : 3;
+    if (D == 64) p.nv = 3;
+    constexpr int kTileBytes = kTile * D * 2;
+    const size_t smem = static_cast<size_t>(p.q_tiles + kNK + p.nv) * kTileBytes + 20 * 8 + 256 * 8 + 16;
+    // one CTA per SM; never more CTAs than tiles, never more than the partial slots provisioned
+    long long grid = ctx->num_sms;
+    if (grid > p.total_tiles) grid = p.total_tiles;
+    if (grid > kAttnMaxCtas) grid = kAttnMaxCtas;
+    if (ctx->tm_k_ptr != a.k_pool || ctx->tm_v_ptr != a.v_pool || ctx->tm_layer_stride != a.pool_layer_stride ||
+        ctx->tm_n_pages != a.n_pages) {
+        int st = encode_pool_map(&ctx->tm_k, a.k_pool, ctx->shape, a.pool_layer_stride, a.n_pages);
+        if (st == PREPOS_OK) st = encode_pool_map(&ctx->tm_v, a.v_pool, ctx->shape, a.pool_layer_stride, a.n_pages);
+        if (st != PREPOS_OK) return st;
+        ctx->tm_k_ptr = a.k_pool;
+        ctx->tm_v_ptr = a.v_pool;
+        ctx->tm_layer_stride = a.pool_layer_stride;
+        ctx->tm_n_pages = a.n_pages;
+    }
+    PREPOS_CUDA_TRY(cudaFuncSetAttribute(attn_umma_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                         static_cast<int>(smem)));
+    attn_umma_kernel<D><<<static_cast<int>(grid), kThreads, smem, stream>>>(ctx->tm_k, ctx->tm_v, p);
+    PREPOS_CUDA_TRY(cudaGetLastError());
+    ctx->launches += 1;
+    if (grid > 1) {
+        const dim3 mg(a.n_units, p.Hkv, a.layer_end - a.layer_begin);
+        attn_merge_kernel<D><<<mg, 128, 0, stream>>>(p, static_cast<int>(grid));
+        PREPOS_CUDA_TRY(cudaGetLastError());
+        ctx->launches += 1;
+    }
+    return PREPOS_OK;
+}
+
+}  // namespace
+
+bool prepos_attn_umma_supported(const prepos_ctx *ctx)
+{
+    const prepos_model_shape &s = ctx->shape;
+    return (s.head_dim == 64 || s.head_dim == 128) && s.page_size >= 8 && s.page_size <= kTile;
+}
+
+int prepos_launch_attn_umma(prepos_ctx *ctx, const AttnArgs &a, int tiles_per_lh, cudaStream_t stream)
+{
+    if (!prepos_attn_umma_supported(ctx)) return PREPOS_E_SHAPE;
+    if (ctx->shape.head_dim == 128) return launch<128>(ctx, a, tiles_per_lh, stream);
+    return launch<64>(ctx, a, tiles_per_lh, stream);
+}

@@ -23,6 +23,7 @@ static_assert(sizeof(prepos_record) == 48, "prepos_record must be 48 bytes");
     } while (0)
 
 void prepos_note_cuda_error(cudaError_t e, const char *what, const char *file, int line);
+void *prepos_get_encode_tiled();  // cuTensorMapEncodeTiled through the runtime's driver entry point (api.cu)
 
 constexpr int kMaxRdPartials = 1024;  // CTAs of a ready-dist launch (upper bound on its grid)
 constexpr int kRdMaxRows = 128;       // hidden rows reduced by one ready-dist launch

@@ -414,8 +414,6 @@ typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t
 
 }  // namespace
 
-void *prepos_get_encode_tiled();  // api.cu
-
 int prepos_launch_ready_dist(prepos_ctx *ctx, int n, const int32_t *session_ids, const __nv_bfloat16 *hidden,
                              const __nv_bfloat16 *w, const int64_t *position_p, const uint64_t *entry_hash,
                              const int32_t *skip_mask, prepos_record *records, const uint64_t *session_version,
