@@ -153,6 +153,8 @@ int prepos_ctx_create(prepos_ctx **out, const prepos_model_shape *shape, int max
     c->plan_inflight = false;
     c->tm_k_ptr = c->tm_v_ptr = nullptr;
     c->tm_layer_stride = c->tm_n_pages = 0;
+    c->tm_kn_ptr = c->tm_vn_ptr = nullptr;
+    c->tm_new_layer_stride = c->tm_new_rows = 0;
     // arrival counters start at zero and are reset by their last arriver
     cudaError_t e = cudaMemset(c->rd_counter, 0, sizeof(unsigned int) * (kRdMaxRows + 1));
     if (e == cudaSuccess) e = cudaMemset(c->attn_counters, 0, sizeof(unsigned int) * c->attn_counters_n);
@@ -286,6 +288,8 @@ int prepos_entry_attn(prepos_ctx *ctx, int layer_begin, int layer_end, int n_ses
     a.layer_begin = layer_begin;
     a.layer_end = layer_end;
     a.n_units = static_cast<int>(ctx->plan_units.size());
+    a.sum_rows = 0;
+    for (int i = 0; i < n_sessions; ++i) a.sum_rows += l_entry[i];
     a.q = static_cast<const __nv_bfloat16 *>(q);
     a.k_new = static_cast<const __nv_bfloat16 *>(k_new);
     a.v_new = static_cast<const __nv_bfloat16 *>(v_new);

@@ -8,14 +8,15 @@
 //   (layer, kv head) x units x 128-token tiles
 // cut into one contiguous range per persistent CTA (1 CTA / SM).  A CTA walks its range as segments
 // (= its part of one unit).  A unit covered by one segment is written directly; otherwise every
-// covering CTA writes a normalised fp32 partial + log-sum-exp and a small merge kernel combines them in
-// CTA order (deterministic for a fixed plan).
+// covering CTA writes a normalised fp32 partial + log-sum-exp, bumps the unit's arrival counter, and the
+// last CTA to arrive combines the partials in CTA order (the single cross-CTA pass; deterministic for a
+// fixed plan whoever arrives last).
 //
 // Inside a CTA (384 threads):
-//   warp 0  K producer: TMA (5-D map over the pool: one 4 KB box per page) into a ring of K tiles
-//   warp 3  V producer: same for V
-//   warp 2  TMEM allocator; loader of the entry-token tile (K_new/V_new -> swizzled smem) and the
-//           Append(E) writer (Alg. 1 l.5)
+//   warp 0  K producer: TMA into a ring of K tiles -- cached tiles through a 5-D map over the pool (one
+//           4 KB box per page), entry-token tiles through a 5-D map over K_new (one box per 8 tokens)
+//   warp 3  V producer: same for V (plus a zero fill of the rows of an entry tile no box covers)
+//   warp 2  TMEM allocator and the Append(E) writer (Alg. 1 l.5): K_new/V_new -> the session's pages
 //   warp 1  MMA issuer: S = Q K^T (SS, K-major SW128) into TMEM, O += P V (A = P from TMEM, B = V MN-major)
 //   warps 4-7 / 8-11  two softmax warpgroups, one TMEM lane (= query row) per thread: online softmax
 //           with lazy rescaling, P written back to TMEM as bf16 over S.
@@ -32,8 +33,9 @@ namespace {
 constexpr int kThreads = 384;
 constexpr int kTile = kAttnTileTokens;  // 128 tokens
 constexpr int kNK = 3;                  // K ring slots
-constexpr int kMaxNV = 3;               // V ring slots (3 when only one Q tile is resident, else 2)
 constexpr float kRescaleThreshold = 8.f;  // log2 units: lazy rescale (P <= 2^8)
+constexpr int kServiceRegs = 72;          // 128 * 72 + 256 * 216 = 384 * 168
+constexpr int kSoftmaxRegs = 216;
 
 struct UmmaParams {
     AttnArgs a;
@@ -46,11 +48,12 @@ struct UmmaParams {
     int nv;             // V ring slots
     float scale_log2;
     float *partials;    // [2 * grid] slots of kAttnMaxRows * (D + 2) floats: O [256][D], lse2 [256], pad [256]
+    unsigned int *counters;  // [n_lh][n_units] arrival counters of the cross-CTA pass (self-resetting)
 };
 
 struct Seg {
     AttnUnit u;
-    int unit_idx, layer, kvh;
+    int unit_idx, layer, kvh, lh;
     int tb, te;      // tile range within the unit
     int first;       // 1 = first segment of this CTA
     int direct;      // segment covers the whole unit
@@ -82,6 +85,7 @@ struct SegIter {
         prev_unit = lo;
         s.unit_idx = lo;
         s.u = p.units[lo];
+        s.lh = lh;
         s.layer = p.a.layer_begin + lh / p.Hkv;
         s.kvh = lh % p.Hkv;
         s.tb = off - s.u.tile_prefix;
@@ -99,6 +103,11 @@ struct SegIter {
 __device__ __forceinline__ long long cta_begin(long long total, int grid, int c)
 {
     return total * c / grid;
+}
+// the CTA whose range [cta_begin(c), cta_begin(c + 1)) holds tile t
+__device__ __forceinline__ int cta_of(long long total, int grid, long long t)
+{
+    return static_cast<int>(((t + 1) * grid + total - 1) / total) - 1;
 }
 
 // 64-bit UMMA shared-memory descriptor, SWIZZLE_128B, version 1 (sm_100)
@@ -133,6 +142,7 @@ __device__ __forceinline__ uint32_t pack_bf16(float lo, float hi)
 template <int D>
 __global__ void __launch_bounds__(kThreads, 1)
 attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__ CUtensorMap tm_v,
+                 const __grid_constant__ CUtensorMap tm_kn, const __grid_constant__ CUtensorMap tm_vn,
                  const UmmaParams p)
 {
     constexpr int kHalves = D / 64;
@@ -154,6 +164,7 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
     uint64_t *s_full = bars + 12, *p_ready = bars + 14, *o_done = bars + 16, *q_full = bars + 18;
     float2 *ml_x = reinterpret_cast<float2 *>(bars + 20);  // [2][128] (m_used, l) exchange
     uint32_t *tmem_slot = reinterpret_cast<uint32_t *>(ml_x + 256);
+    int *merge_info = reinterpret_cast<int *>(tmem_slot + 1);  // [3]: c0 (or -1 = not last), c1, c0's slot
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
 
@@ -188,18 +199,24 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
     const int page_bytes = p.page * D * 2;
     const int page_groups = p.page >> 3;
 
-    // register budget: the four service warps need few registers, the softmax threads hold a 128-wide score row
-    // (setmaxnreg tuning comes after correctness)
-
+    // register budget: launch gives 168 regs x 384 threads.  The four service warps (warpgroup 0) hand theirs
+    // down to kServiceRegs; each softmax thread, which holds a 128-wide score row, grows to kSoftmaxRegs.
+    if (warp < 4) {
+    ptx::setmaxnreg_dec<kServiceRegs>();
     if (warp == 0 || warp == 3) {
         // ===================== K (warp 0) / V (warp 3) TMA producers =====================
         const bool is_v = (warp == 3);
         const CUtensorMap *tm = is_v ? &tm_v : &tm_k;
+        const CUtensorMap *tmn = is_v ? &tm_vn : &tm_kn;
         uint64_t *full = is_v ? v_full : k_full, *empty = is_v ? v_empty : k_empty;
         uint8_t *ring = is_v ? v_s : k_s;
         const int n_slots = is_v ? p.nv : kNK;
-        if (lane == 0) ptx::prefetch_tmap(tm);
-        const uint64_t pol = ptx::policy_evict_first();
+        if (lane == 0) {
+            ptx::prefetch_tmap(tm);
+            ptx::prefetch_tmap(tmn);
+        }
+        const uint64_t pol = ptx::policy_evict_first();   // the cache is streamed once per pass
+        const uint64_t pol_new = ptx::policy_evict_last();  // entry K/V: just produced, re-read by every row chunk
         int slot = 0;
         uint32_t ph = 0;
         SegIter it(t0, t1);
@@ -207,27 +224,46 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
         while (it.next(p, s)) {
             const int n_pages_valid = (s.u.n_s + p.page - 1) >> p.page_shift;
             const int32_t *pt = p.a.page_table + static_cast<size_t>(s.u.session) * p.a.page_table_stride;
+            // this lane's page of tile t (page-table reads run one tile ahead of the TMA issue)
+            auto page_of = [&](int t) -> int {
+                const int idx = t * pages_per_tile + lane;
+                return (t < s.u.n_cached_tiles && lane < pages_per_tile && idx < n_pages_valid) ? __ldg(pt + idx) : -1;
+            };
+            int pg_next = page_of(s.tb);
             for (int t = s.tb; t < s.te; ++t) {
+                const int pg = pg_next;
+                if (t + 1 < s.te) pg_next = page_of(t + 1);
+                if (lane == 0) ptx::mbar_wait(ptx::smem_u32(&empty[slot]), ph ^ 1);
+                __syncwarp();
+                uint8_t *dst = ring + slot * kTileBytes;
+                const uint32_t fb = ptx::smem_u32(&full[slot]);
                 if (t < s.u.n_cached_tiles) {
-                    const int first_page = t * pages_per_tile;
-                    int nvp = n_pages_valid - first_page;
+                    int nvp = n_pages_valid - t * pages_per_tile;
                     nvp = nvp < pages_per_tile ? nvp : pages_per_tile;
-                    int pg = 0;
-                    if (lane < nvp) pg = __ldg(pt + first_page + lane);
-                    if (lane == 0) {
-                        ptx::mbar_wait(ptx::smem_u32(&empty[slot]), ph ^ 1);
-                        ptx::mbar_arrive_expect_tx(ptx::smem_u32(&full[slot]), nvp * page_bytes);
-                    }
+                    if (lane == 0) ptx::mbar_arrive_expect_tx(fb, nvp * page_bytes);
                     __syncwarp();
-                    if (lane < nvp)
-                        ptx::tma_load_5d(ptx::smem_u32(ring + slot * kTileBytes + lane * page_bytes), tm,
-                                         ptx::smem_u32(&full[slot]), 0, 0, 0, (pg * p.Hkv + s.kvh) * page_groups,
-                                         s.layer, pol);
+                    if (pg >= 0)
+                        ptx::tma_load_5d(ptx::smem_u32(dst + lane * page_bytes), tm, fb, 0, 0, 0,
+                                         (pg * p.Hkv + s.kvh) * page_groups, s.layer, pol);
                 } else {
-                    // entry-token tiles are filled by warp 2; wait all the same so that the phase parity this
-                    // warp tracks never falls two rounds behind the barrier
-                    if (lane == 0) ptx::mbar_wait(ptx::smem_u32(&empty[slot]), ph ^ 1);
+                    // entry-token tile: one box per 8 tokens straight from K_new / V_new.  Tokens past the ones this
+                    // unit can see (later tokens, the next session's, or out of bounds = zero) are finite and masked
+                    // by the softmax; V rows that no box covers are zeroed so that P = 0 never meets stale NaNs.
+                    const int nb = (t - s.u.n_cached_tiles) * kTile;  // first entry token of this tile
+                    int nvis = s.u.tok0 + s.u.ntok - nb;              // entry tokens this unit can see here
+                    nvis = nvis < kTile ? nvis : kTile;
+                    const int ng = (nvis + 7) >> 3;
+                    if (is_v) {
+                        for (int off = ng * kGroupStride + lane * 16; off < kTileBytes; off += 32 * 16)
+                            *reinterpret_cast<uint4 *>(dst + off) = make_uint4(0, 0, 0, 0);
+                        ptx::fence_proxy_async_smem();
+                        __syncwarp();
+                    }
+                    if (lane == 0) ptx::mbar_arrive_expect_tx(fb, ng * kGroupStride);
                     __syncwarp();
+                    if (lane < ng)
+                        ptx::tma_load_5d(ptx::smem_u32(dst + lane * kGroupStride), tmn, fb, 0, s.u.row0 + nb + lane * 8, 0,
+                                         s.kvh, s.layer, pol_new);
                 }
                 if (++slot == n_slots) {
                     slot = 0;
@@ -236,60 +272,46 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
             }
         }
     } else if (warp == 2) {
-        // ===================== entry-token tile loader + Append(E) =====================
-        int kslot = 0, vslot = 0;
-        uint32_t kph = 0, vph = 0;
+        // ===================== Append(E) (Alg. 1 l.5): K_new / V_new -> the session's pages =====================
+        // Owned by the CTA that runs the last tile of the session's last row chunk, once per (layer, kv head).
+        // Nothing in this launch reads cache positions >= n_s, so the copy needs no ordering with the tiles.
         SegIter it(t0, t1);
         Seg s;
         constexpr int kChunks = D / 8;  // 16-byte chunks per row
+        constexpr int kBatch = 4;
         while (it.next(p, s)) {
-            for (int t = s.tb; t < s.te; ++t) {
-                if (t >= s.u.n_cached_tiles) {
-                    const int nb = (t - s.u.n_cached_tiles) * kTile;      // first entry token of this tile
-                    int nvis = s.u.tok0 + s.u.ntok - nb;                   // entry tokens this unit can see here
-                    nvis = nvis < kTile ? nvis : kTile;
-                    const bool append = (s.u.tok0 + s.u.ntok == s.u.l_entry);  // last row chunk owns Append(E)
-                    const size_t lo = static_cast<size_t>(s.layer);
-                    const int32_t *pt = p.a.page_table + static_cast<size_t>(s.u.session) * p.a.page_table_stride;
-#pragma unroll 1
-                    for (int which = 0; which < 2; ++which) {
-                        const __nv_bfloat16 *src = (which ? p.a.v_new : p.a.k_new) + lo * p.a.kv_new_layer_stride;
-                        __nv_bfloat16 *pool = (which ? p.a.v_pool : p.a.k_pool) + lo * p.a.pool_layer_stride;
-                        uint8_t *dst = which ? v_s + vslot * kTileBytes : k_s + kslot * kTileBytes;
-                        ptx::mbar_wait(ptx::smem_u32(which ? &v_empty[vslot] : &k_empty[kslot]), (which ? vph : kph) ^ 1);
-                        for (int idx = lane; idx < kTile * kChunks; idx += 32) {
-                            const int r = idx / kChunks, c = idx - r * kChunks;
-                            uint4 val = make_uint4(0, 0, 0, 0);
-                            if (r < nvis) {
-                                const int tok = nb + r;
-                                val = *reinterpret_cast<const uint4 *>(
-                                    src + (static_cast<size_t>(s.u.row0 + tok) * p.Hkv + s.kvh) * D + c * 8);
-                                if (append) {
-                                    const int j = s.u.n_s + tok;
-                                    const int pg = __ldg(pt + (j >> p.page_shift));
-                                    *reinterpret_cast<uint4 *>(
-                                        pool + ((static_cast<size_t>(pg) * p.Hkv + s.kvh) * p.page + (j & (p.page - 1))) * D +
-                                        c * 8) = val;
-                                }
-                            }
-                            *reinterpret_cast<uint4 *>(dst + tile_offset<D>(r, c)) = val;
-                        }
-                        ptx::fence_proxy_async_smem();
-                        __syncwarp();
-                        if (lane == 0) ptx::mbar_arrive(ptx::smem_u32(which ? &v_full[vslot] : &k_full[kslot]));
+            if (s.u.tok0 + s.u.ntok != s.u.l_entry || s.te != s.u.n_tiles) continue;
+            const size_t lo = static_cast<size_t>(s.layer);
+            const int32_t *pt = p.a.page_table + static_cast<size_t>(s.u.session) * p.a.page_table_stride;
+            const __nv_bfloat16 *ksrc = p.a.k_new + lo * p.a.kv_new_layer_stride;
+            const __nv_bfloat16 *vsrc = p.a.v_new + lo * p.a.kv_new_layer_stride;
+            __nv_bfloat16 *kpool = p.a.k_pool + lo * p.a.pool_layer_stride;
+            __nv_bfloat16 *vpool = p.a.v_pool + lo * p.a.pool_layer_stride;
+            const int total = s.u.l_entry * kChunks;
+            for (int base = lane; base < total; base += 32 * kBatch) {
+                uint4 kv[kBatch], vv[kBatch];
+                int pg[kBatch];
+#pragma unroll
+                for (int u = 0; u < kBatch; ++u) {
+                    const int idx = base + u * 32;
+                    if (idx < total) {
+                        const int tok = idx / kChunks, c = idx - tok * kChunks;
+                        const size_t so = (static_cast<size_t>(s.u.row0 + tok) * p.Hkv + s.kvh) * D + c * 8;
+                        kv[u] = __ldg(reinterpret_cast<const uint4 *>(ksrc + so));
+                        vv[u] = __ldg(reinterpret_cast<const uint4 *>(vsrc + so));
+                        pg[u] = __ldg(pt + ((s.u.n_s + tok) >> p.page_shift));
                     }
-                } else {
-                    // cached tiles belong to the TMA producers; keep this warp's parities in lockstep (see there)
-                    ptx::mbar_wait(ptx::smem_u32(&k_empty[kslot]), kph ^ 1);
-                    ptx::mbar_wait(ptx::smem_u32(&v_empty[vslot]), vph ^ 1);
                 }
-                if (++kslot == kNK) {
-                    kslot = 0;
-                    kph ^= 1;
-                }
-                if (++vslot == p.nv) {
-                    vslot = 0;
-                    vph ^= 1;
+#pragma unroll
+                for (int u = 0; u < kBatch; ++u) {
+                    const int idx = base + u * 32;
+                    if (idx < total) {
+                        const int tok = idx / kChunks, c = idx - tok * kChunks;
+                        const int j = s.u.n_s + tok;
+                        const size_t po = ((static_cast<size_t>(pg[u]) * p.Hkv + s.kvh) * p.page + (j & (p.page - 1))) * D + c * 8;
+                        *reinterpret_cast<uint4 *>(kpool + po) = kv[u];
+                        *reinterpret_cast<uint4 *>(vpool + po) = vv[u];
+                    }
                 }
             }
         }
@@ -297,7 +319,7 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
         // ===================== MMA issuer =====================
         int kslot = 0, vslot = 0;
         uint32_t kph = 0, vph = 0, qph = 0;
-        uint32_t pph[2] = {0, 0};
+        uint32_t pph = 0;  // bit w = phase parity of p_ready[w]
         SegIter it(t0, t1);
         Seg s;
         while (it.next(p, s)) {
@@ -365,8 +387,8 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
                         }
                     }
                 }
-                ptx::mbar_wait(ptx::smem_u32(&p_ready[w]), pph[w]);
-                pph[w] ^= 1;
+                ptx::mbar_wait(ptx::smem_u32(&p_ready[w]), (pph >> w) & 1u);
+                pph ^= 1u << w;
                 ptx::tc_fence_after();
                 if (lane == 0) {
                     const uint32_t va = ptx::smem_u32(v_s + vslot * kTileBytes);
@@ -393,7 +415,9 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
             }
             __syncwarp();
         }
+    }
     } else {
+        ptx::setmaxnreg_inc<kSoftmaxRegs>();
         // ===================== softmax warpgroups (warps 4-7: stream 0, warps 8-11: stream 1) =====================
         const int w = (warp - 4) >> 2;
         const int row = ((warp & 3) << 5) | lane;              // TMEM lane == row within the M-tile
@@ -596,61 +620,62 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
                 if (live && !s.direct && w == 0) slot[kAttnMaxRows * D + row] = M + log2f(L);
                 ptx::bar_sync(1, 256);  // ml_x is reused by the next segment
             }
+            // ---- the single cross-CTA pass: the last CTA to deliver its partial of a cut unit combines them
+            if (!s.direct) {
+                __threadfence();
+                ptx::bar_sync(1, 256);
+                if (st == 0) {
+                    const long long U0 = static_cast<long long>(s.lh) * p.tiles_per_lh + s.u.tile_prefix;
+                    const int c0 = cta_of(p.total_tiles, gridDim.x, U0);
+                    const int c1 = cta_of(p.total_tiles, gridDim.x, U0 + s.u.n_tiles - 1);
+                    unsigned int *cnt = p.counters + static_cast<size_t>(s.lh) * p.a.n_units + s.unit_idx;
+                    const unsigned int prev = atomicAdd(cnt, 1u);
+                    const bool last = (prev == static_cast<unsigned int>(c1 - c0));
+                    if (last) *cnt = 0u;  // self-reset for the next launch
+                    merge_info[0] = last ? c0 : -1;
+                    merge_info[1] = c1;
+                    merge_info[2] = (cta_begin(p.total_tiles, gridDim.x, c0) < U0) ? 1 : 0;  // c0's slot for this unit
+                }
+                ptx::bar_sync(1, 256);
+                const int c0 = merge_info[0], c1 = merge_info[1], c0_slot = merge_info[2];
+                if (c0 >= 0) {
+                    __threadfence();
+                    constexpr int kVec = D / 4;  // float4 per row
+                    constexpr size_t kSlotFloats = static_cast<size_t>(kAttnMaxRows) * (D + 2);
+                    const float *base0 = p.partials + (2 * static_cast<size_t>(c0) + c0_slot) * kSlotFloats;
+                    for (int idx = st; idx < rows * kVec; idx += 256) {
+                        const int r = idx / kVec, v = idx - r * kVec;
+                        float M = __ldcg(base0 + kAttnMaxRows * D + r);
+                        for (int c = c0 + 1; c <= c1; ++c)
+                            M = fmaxf(M, __ldcg(p.partials + 2 * static_cast<size_t>(c) * kSlotFloats + kAttnMaxRows * D + r));
+                        float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
+                        float wsum = 0.f;
+                        for (int c = c0; c <= c1; ++c) {
+                            const float *sl = (c == c0) ? base0 : p.partials + 2 * static_cast<size_t>(c) * kSlotFloats;
+                            const float wgt = exp2f(__ldcg(sl + kAttnMaxRows * D + r) - M);
+                            const float4 o = __ldcg(reinterpret_cast<const float4 *>(sl + static_cast<size_t>(r) * D) + v);
+                            acc.x = fmaf(wgt, o.x, acc.x);
+                            acc.y = fmaf(wgt, o.y, acc.y);
+                            acc.z = fmaf(wgt, o.z, acc.z);
+                            acc.w = fmaf(wgt, o.w, acc.w);
+                            wsum += wgt;
+                        }
+                        const float inv = 1.f / wsum;
+                        const int tok = s.u.tok0 + r / G, h = s.kvh * G + r % G;
+                        uint2 pk;
+                        pk.x = pack_bf16(acc.x * inv, acc.y * inv);
+                        pk.y = pack_bf16(acc.z * inv, acc.w * inv);
+                        *reinterpret_cast<uint2 *>(ob + (static_cast<size_t>(s.u.row0 + tok) * p.Hq + h) * D + v * 4) = pk;
+                    }
+                }
+                ptx::bar_sync(1, 256);  // merge_info is reused by the next segment
+            }
         }
     }
 
     ptx::tc_fence_before();
     __syncthreads();
     if (warp == 2) ptx::tmem_dealloc<512>(tmem);
-}
-
-// Combines the partials of every unit that was cut across CTAs.  grid (n_units, Hkv, layers), 128 threads.
-template <int D>
-__global__ void __launch_bounds__(128) attn_merge_kernel(const UmmaParams p, int main_grid)
-{
-    const AttnUnit u = p.units[blockIdx.x];
-    const int kvh = blockIdx.y, lz = blockIdx.z;
-    const int lh = lz * p.Hkv + kvh;
-    const int G = p.Hq / p.Hkv;
-    const int rows = u.ntok * G;
-    const long long U0 = static_cast<long long>(lh) * p.tiles_per_lh + u.tile_prefix;
-    const long long U1 = U0 + u.n_tiles;
-    // CTAs covering [U0, U1)
-    int c0 = static_cast<int>(U0 * main_grid / p.total_tiles);
-    while (c0 + 1 < main_grid && cta_begin(p.total_tiles, main_grid, c0 + 1) <= U0) ++c0;
-    while (c0 > 0 && cta_begin(p.total_tiles, main_grid, c0) > U0) --c0;
-    int c1 = c0;
-    while (c1 + 1 < main_grid && cta_begin(p.total_tiles, main_grid, c1 + 1) < U1) ++c1;
-    if (c0 == c1) return;  // written directly by its only CTA
-    const size_t slot_floats = static_cast<size_t>(kAttnMaxRows) * (D + 2);
-    __nv_bfloat16 *ob = p.a.out + static_cast<size_t>(p.a.layer_begin + lz) * p.a.out_layer_stride;
-    constexpr int kVec = D / 4;  // float4 per row
-    for (int idx = threadIdx.x; idx < rows * kVec; idx += blockDim.x) {
-        const int r = idx / kVec, v = idx - r * kVec;
-        float M = -CUDART_INF_F;
-        for (int c = c0; c <= c1; ++c) {
-            const float *slot = p.partials + (2 * static_cast<size_t>(c) + (cta_begin(p.total_tiles, main_grid, c) < U0 ? 1 : 0)) * slot_floats;
-            M = fmaxf(M, slot[kAttnMaxRows * D + r]);
-        }
-        float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
-        float wsum = 0.f;
-        for (int c = c0; c <= c1; ++c) {
-            const float *slot = p.partials + (2 * static_cast<size_t>(c) + (cta_begin(p.total_tiles, main_grid, c) < U0 ? 1 : 0)) * slot_floats;
-            const float wgt = exp2f(slot[kAttnMaxRows * D + r] - M);
-            const float4 o = *reinterpret_cast<const float4 *>(slot + static_cast<size_t>(r) * D + v * 4);
-            acc.x = fmaf(wgt, o.x, acc.x);
-            acc.y = fmaf(wgt, o.y, acc.y);
-            acc.z = fmaf(wgt, o.z, acc.z);
-            acc.w = fmaf(wgt, o.w, acc.w);
-            wsum += wgt;
-        }
-        const float inv = 1.f / wsum;
-        const int tok = u.tok0 + r / G, h = kvh * G + r % G;
-        uint2 pk;
-        pk.x = pack_bf16(acc.x * inv, acc.y * inv);
-        pk.y = pack_bf16(acc.z * inv, acc.w * inv);
-        *reinterpret_cast<uint2 *>(ob + (static_cast<size_t>(u.row0 + tok) * p.Hq + h) * D + v * 4) = pk;
-    }
 }
 
 typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
@@ -674,6 +699,31 @@ int encode_pool_map(CUtensorMap *tm, void *pool, const prepos_model_shape &s, in
                               CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) {
         fprintf(stderr, "libprepos: cuTensorMapEncodeTiled(pool) failed: %d\n", static_cast<int>(r));
+        return PREPOS_E_CUDA;
+    }
+    return PREPOS_OK;
+}
+
+// K_new / V_new [layer][sum_L][Hkv][d]: a box is 8 consecutive tokens of one kv head, laid out like one 8-row group
+// of a pool tile ([64-column half][8 rows][128 B], 128-byte swizzle); tokens past sum_L read as zero.
+int encode_new_map(CUtensorMap *tm, const void *base, const prepos_model_shape &s, int64_t layer_stride, int64_t sum_rows)
+{
+    EncodeTiledFn encode = reinterpret_cast<EncodeTiledFn>(prepos_get_encode_tiled());
+    if (!encode) return PREPOS_E_CUDA;
+    const int D = s.head_dim, halves = D / 64;
+    const cuuint64_t tok_stride = static_cast<cuuint64_t>(s.n_kv_heads) * D * 2;
+    // a one-layer tensor may come with any layer stride: give the (unused) dimension a valid one
+    const cuuint64_t lstride = (s.layers > 1) ? static_cast<cuuint64_t>(layer_stride) * 2 : tok_stride * static_cast<cuuint64_t>(sum_rows);
+    const cuuint64_t dims[5] = {64, static_cast<cuuint64_t>(sum_rows), static_cast<cuuint64_t>(halves),
+                                static_cast<cuuint64_t>(s.n_kv_heads), static_cast<cuuint64_t>(s.layers)};
+    const cuuint64_t strides[4] = {tok_stride, 128, static_cast<cuuint64_t>(D) * 2, lstride};
+    const cuuint32_t box[5] = {64, 8, static_cast<cuuint32_t>(halves), 1, 1};
+    const cuuint32_t estr[5] = {1, 1, 1, 1, 1};
+    const CUresult r = encode(tm, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 5, const_cast<void *>(base), dims, strides, box, estr,
+                              CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
+                              CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) {
+        fprintf(stderr, "libprepos: cuTensorMapEncodeTiled(entry K/V) failed: %d\n", static_cast<int>(r));
         return PREPOS_E_CUDA;
     }
     return PREPOS_OK;
@@ -717,17 +767,24 @@ int launch(prepos_ctx *ctx, const AttnArgs &a, int tiles_per_lh, cudaStream_t st
         ctx->tm_layer_stride = a.pool_layer_stride;
         ctx->tm_n_pages = a.n_pages;
     }
+    // entry K/V maps: they follow the call's K_new / V_new pointers
+    if (ctx->tm_kn_ptr != a.k_new || ctx->tm_vn_ptr != a.v_new || ctx->tm_new_layer_stride != a.kv_new_layer_stride ||
+        ctx->tm_new_rows != a.sum_rows) {
+        int st = encode_new_map(&ctx->tm_kn, a.k_new, ctx->shape, a.kv_new_layer_stride, a.sum_rows);
+        if (st == PREPOS_OK) st = encode_new_map(&ctx->tm_vn, a.v_new, ctx->shape, a.kv_new_layer_stride, a.sum_rows);
+        if (st != PREPOS_OK) return st;
+        ctx->tm_kn_ptr = a.k_new;
+        ctx->tm_vn_ptr = a.v_new;
+        ctx->tm_new_layer_stride = a.kv_new_layer_stride;
+        ctx->tm_new_rows = a.sum_rows;
+    }
+    if (static_cast<size_t>(p.n_lh) * a.n_units > ctx->attn_counters_n) return PREPOS_E_WORKSPACE;
+    p.counters = ctx->attn_counters;
     PREPOS_CUDA_TRY(cudaFuncSetAttribute(attn_umma_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                          static_cast<int>(smem)));
-    attn_umma_kernel<D><<<static_cast<int>(grid), kThreads, smem, stream>>>(ctx->tm_k, ctx->tm_v, p);
+    attn_umma_kernel<D><<<static_cast<int>(grid), kThreads, smem, stream>>>(ctx->tm_k, ctx->tm_v, ctx->tm_kn, ctx->tm_vn, p);
     PREPOS_CUDA_TRY(cudaGetLastError());
     ctx->launches += 1;
-    if (grid > 1) {
-        const dim3 mg(a.n_units, p.Hkv, a.layer_end - a.layer_begin);
-        attn_merge_kernel<D><<<mg, 128, 0, stream>>>(p, static_cast<int>(grid));
-        PREPOS_CUDA_TRY(cudaGetLastError());
-        ctx->launches += 1;
-    }
     return PREPOS_OK;
 }
 

@@ -87,6 +87,10 @@ struct prepos_ctx {
     void *tm_k_ptr, *tm_v_ptr;
     int64_t tm_layer_stride, tm_n_pages;
     CUtensorMap tm_k, tm_v;
+    // ... and for the call's entry K/V
+    const void *tm_kn_ptr, *tm_vn_ptr;
+    int64_t tm_new_layer_stride, tm_new_rows;
+    CUtensorMap tm_kn, tm_vn;
 };
 
 // ---- per-file launchers (all return a PREPOS_* status) -------------------------------------------
@@ -104,6 +108,7 @@ int prepos_launch_invalidate(prepos_ctx *ctx, int n, const int32_t *session_ids,
 
 struct AttnArgs {
     int layer_begin, layer_end, n_units;
+    int sum_rows;  // rows of the packed sum_L axis of q / k_new / v_new / out
     const __nv_bfloat16 *q, *k_new, *v_new;
     __nv_bfloat16 *k_pool, *v_pool, *out;
     int64_t q_layer_stride, kv_new_layer_stride, pool_layer_stride, out_layer_stride, n_pages;
