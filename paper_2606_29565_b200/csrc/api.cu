@@ -155,6 +155,8 @@ int prepos_ctx_create(prepos_ctx **out, const prepos_model_shape *shape, int max
     c->tm_layer_stride = c->tm_n_pages = 0;
     c->tm_kn_ptr = c->tm_vn_ptr = nullptr;
     c->tm_new_layer_stride = c->tm_new_rows = 0;
+    c->tm_q_ptr = nullptr;
+    c->tm_q_layer_stride = c->tm_q_rows = 0;
     // arrival counters start at zero and are reset by their last arriver
     cudaError_t e = cudaMemset(c->rd_counter, 0, sizeof(unsigned int) * (kRdMaxRows + 1));
     if (e == cudaSuccess) e = cudaMemset(c->attn_counters, 0, sizeof(unsigned int) * c->attn_counters_n);

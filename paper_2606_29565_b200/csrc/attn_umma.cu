@@ -25,6 +25,8 @@
 #include <math_constants.h>
 #include <stdio.h>
 
+#include <type_traits>
+
 #include "common.cuh"
 #include "ptx.cuh"
 
@@ -55,47 +57,75 @@ struct Seg {
     AttnUnit u;
     int unit_idx, layer, kvh, lh;
     int tb, te;      // tile range within the unit
-    int first;       // 1 = first segment of this CTA
+    int slot;        // partial slot of this CTA used when the segment is cut: 0 = starts at the CTA's first tile
     int direct;      // segment covers the whole unit
 };
 
-// Walks the CTA's contiguous range [t0, t1) of the global tile space as segments.
+// Walks the CTA's contiguous range [t0, t1) of the global tile space as segments (= the CTA's part of one
+// unit).  Processing order: when the range ends inside a unit, that cut head segment goes FIRST, then the rest
+// in natural order.  A cut unit's head (end of CTA c's range) and tail (start of CTA c+1's range) are then both
+// delivered early in the kernel, so the cross-CTA merge never sits in the kernel's tail.
 struct SegIter {
-    long long t, t1;
-    int first, prev_unit;
-    __device__ SegIter(long long t0_, long long t1_) : t(t0_), t1(t1_), first(1), prev_unit(-1) {}
-    __device__ bool next(const UmmaParams &p, Seg &s)
+    long long t0, t, t_stop, t1;
+    long long tl;     // start of the end-cut segment emitted first (or -1)
+    int prev_unit;
+    __device__ SegIter(const UmmaParams &p, long long t0_, long long t1_) : t0(t0_), t(t0_), t_stop(t1_), t1(t1_), tl(-1), prev_unit(-1)
     {
-        if (t >= t1) return false;
-        const int lh = static_cast<int>(t / p.tiles_per_lh);
-        const int off = static_cast<int>(t - static_cast<long long>(lh) * p.tiles_per_lh);
-        int lo;
-        if (prev_unit < 0) {
-            // first segment: binary search for the last unit with tile_prefix <= off
-            lo = 0;
-            int hi = p.a.n_units - 1;
-            while (lo < hi) {
-                const int mid = (lo + hi + 1) >> 1;
-                if (p.units[mid].tile_prefix <= off) lo = mid;
-                else hi = mid - 1;
-            }
-        } else {
-            lo = (prev_unit + 1 == p.a.n_units) ? 0 : prev_unit + 1;  // segments end on unit boundaries
+        if (t1 <= t0) return;
+        const long long last = t1 - 1;
+        const int lh = static_cast<int>(last / p.tiles_per_lh);
+        const int off = static_cast<int>(last - static_cast<long long>(lh) * p.tiles_per_lh);
+        const int ui = find_unit(p, off);
+        const AttnUnit u = p.units[ui];
+        const long long U0 = static_cast<long long>(lh) * p.tiles_per_lh + u.tile_prefix;
+        if (U0 + u.n_tiles > t1 && U0 > t0) {  // cut at the end, and not the CTA's only segment
+            tl = U0;
+            t_stop = U0;
         }
-        prev_unit = lo;
-        s.unit_idx = lo;
-        s.u = p.units[lo];
+    }
+    __device__ static int find_unit(const UmmaParams &p, int off)
+    {
+        // the last unit with tile_prefix <= off
+        int lo = 0, hi = p.a.n_units - 1;
+        while (lo < hi) {
+            const int mid = (lo + hi + 1) >> 1;
+            if (p.units[mid].tile_prefix <= off) lo = mid;
+            else hi = mid - 1;
+        }
+        return lo;
+    }
+    __device__ void fill(const UmmaParams &p, Seg &s, long long from, long long limit, int ui, int lh, int off)
+    {
+        s.unit_idx = ui;
+        s.u = p.units[ui];
         s.lh = lh;
         s.layer = p.a.layer_begin + lh / p.Hkv;
         s.kvh = lh % p.Hkv;
         s.tb = off - s.u.tile_prefix;
         const long long unit_end = static_cast<long long>(lh) * p.tiles_per_lh + s.u.tile_prefix + s.u.n_tiles;
-        const long long end = unit_end < t1 ? unit_end : t1;
-        s.te = s.tb + static_cast<int>(end - t);
-        s.first = first;
+        const long long end = unit_end < limit ? unit_end : limit;
+        s.te = s.tb + static_cast<int>(end - from);
+        s.slot = (from == t0) ? 0 : 1;
         s.direct = (s.tb == 0 && s.te == s.u.n_tiles);
-        first = 0;
-        t = end;
+    }
+    __device__ bool next(const UmmaParams &p, Seg &s)
+    {
+        if (tl >= 0) {
+            const int lh = static_cast<int>(tl / p.tiles_per_lh);
+            const int off = static_cast<int>(tl - static_cast<long long>(lh) * p.tiles_per_lh);
+            fill(p, s, tl, t1, find_unit(p, off), lh, off);
+            tl = -1;
+            return true;
+        }
+        if (t >= t_stop) return false;
+        const int lh = static_cast<int>(t / p.tiles_per_lh);
+        const int off = static_cast<int>(t - static_cast<long long>(lh) * p.tiles_per_lh);
+        int ui;
+        if (prev_unit < 0) ui = find_unit(p, off);
+        else ui = (prev_unit + 1 == p.a.n_units) ? 0 : prev_unit + 1;  // segments end on unit boundaries
+        prev_unit = ui;
+        fill(p, s, t, t_stop, ui, lh, off);
+        t += s.te - s.tb;
         return true;
     }
 };
@@ -122,6 +152,17 @@ __device__ __forceinline__ uint64_t make_desc(uint32_t saddr, uint32_t lbo_bytes
     return d;
 }
 
+// the same descriptor as two words: low = start address and leading byte offset, high = stride byte offset,
+// version and swizzle (the high word is one constant per tile layout)
+__device__ __forceinline__ uint32_t desc_lo(uint32_t saddr, uint32_t lbo_bytes)
+{
+    return ((saddr >> 4) & 0x3fffu) | (((lbo_bytes >> 4) & 0x3fffu) << 16);
+}
+__host__ __device__ constexpr uint32_t desc_hi(uint32_t sbo_bytes)
+{
+    return ((sbo_bytes >> 4) & 0x3fffu) | (1u << 14) | (2u << 29);
+}
+
 // byte offset of (row r, 16-byte chunk c of a D-wide bf16 row) in a tile laid out
 // [row group of 8][64-column half][8 rows][128 B] with the 128-byte swizzle (chunk ^= row % 8)
 template <int D>
@@ -139,10 +180,52 @@ __device__ __forceinline__ uint32_t pack_bf16(float lo, float hi)
     return r;
 }
 
+// Append(E) for one (session, layer, kv head), by one warp
+template <int D>
+__device__ __forceinline__ void append_entry(const UmmaParams &p, const Seg &s, int lane)
+{
+    constexpr int kChunks = D / 8;  // 16-byte chunks per row
+    constexpr int kBatch = 4;
+    const size_t lo = static_cast<size_t>(s.layer);
+    const int32_t *pt = p.a.page_table + static_cast<size_t>(s.u.session) * p.a.page_table_stride;
+    const __nv_bfloat16 *ksrc = p.a.k_new + lo * p.a.kv_new_layer_stride;
+    const __nv_bfloat16 *vsrc = p.a.v_new + lo * p.a.kv_new_layer_stride;
+    __nv_bfloat16 *kpool = p.a.k_pool + lo * p.a.pool_layer_stride;
+    __nv_bfloat16 *vpool = p.a.v_pool + lo * p.a.pool_layer_stride;
+    const int total = s.u.l_entry * kChunks;
+    for (int base = lane; base < total; base += 32 * kBatch) {
+        uint4 kv[kBatch], vv[kBatch];
+        int pg[kBatch];
+#pragma unroll
+        for (int u = 0; u < kBatch; ++u) {
+            const int idx = base + u * 32;
+            if (idx < total) {
+                const int tok = idx / kChunks, c = idx - tok * kChunks;
+                const size_t so = (static_cast<size_t>(s.u.row0 + tok) * p.Hkv + s.kvh) * D + c * 8;
+                kv[u] = __ldg(reinterpret_cast<const uint4 *>(ksrc + so));
+                vv[u] = __ldg(reinterpret_cast<const uint4 *>(vsrc + so));
+                pg[u] = __ldg(pt + ((s.u.n_s + tok) >> p.page_shift));
+            }
+        }
+#pragma unroll
+        for (int u = 0; u < kBatch; ++u) {
+            const int idx = base + u * 32;
+            if (idx < total) {
+                const int tok = idx / kChunks, c = idx - tok * kChunks;
+                const int j = s.u.n_s + tok;
+                const size_t po = ((static_cast<size_t>(pg[u]) * p.Hkv + s.kvh) * p.page + (j & (p.page - 1))) * D + c * 8;
+                *reinterpret_cast<uint4 *>(kpool + po) = kv[u];
+                *reinterpret_cast<uint4 *>(vpool + po) = vv[u];
+            }
+        }
+    }
+}
+
 template <int D>
 __global__ void __launch_bounds__(kThreads, 1)
 attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__ CUtensorMap tm_v,
                  const __grid_constant__ CUtensorMap tm_kn, const __grid_constant__ CUtensorMap tm_vn,
+                 const __grid_constant__ CUtensorMap tm_q,
                  const UmmaParams p)
 {
     constexpr int kHalves = D / 64;
@@ -150,6 +233,7 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
     constexpr int kGroupStride = kHalves * 1024;      // bytes between 8-row groups
     constexpr uint32_t kIdescQK = (1u << 4) | (1u << 7) | (1u << 10) | ((kTile >> 3) << 17) | ((128u >> 4) << 24);
     constexpr uint32_t kIdescPV = (1u << 4) | (1u << 7) | (1u << 10) | (1u << 16) | ((D >> 3) << 17) | ((128u >> 4) << 24);
+    constexpr uint32_t kDescHi = desc_hi(kGroupStride);
     constexpr int kColS = 0;        // S_w at columns w * 128 (P_w aliases its first 64 columns)
     constexpr int kColO = 256;      // O_w at columns 256 + w * D
 
@@ -162,6 +246,7 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
     uint64_t *bars = reinterpret_cast<uint64_t *>(tail);
     uint64_t *k_full = bars, *k_empty = bars + 3, *v_full = bars + 6, *v_empty = bars + 9;
     uint64_t *s_full = bars + 12, *p_ready = bars + 14, *o_done = bars + 16, *q_full = bars + 18;
+    uint64_t *q_empty = bars + 19;    // the segment's last QK has read Q: the loader may overwrite it
     float2 *ml_x = reinterpret_cast<float2 *>(bars + 20);  // [2][128] (m_used, l) exchange
     uint32_t *tmem_slot = reinterpret_cast<uint32_t *>(ml_x + 256);
     int *merge_info = reinterpret_cast<int *>(tmem_slot + 1);  // [3]: c0 (or -1 = not last), c1, c0's slot
@@ -180,7 +265,8 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
             ptx::mbar_init(ptx::smem_u32(&p_ready[i]), 128);
             ptx::mbar_init(ptx::smem_u32(&o_done[i]), 1);
         }
-        ptx::mbar_init(ptx::smem_u32(q_full), 256);
+        ptx::mbar_init(ptx::smem_u32(q_full), 1);
+        ptx::mbar_init(ptx::smem_u32(q_empty), 1);
         ptx::fence_mbar_init();
     }
     if (warp == 2) {
@@ -219,7 +305,7 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
         const uint64_t pol_new = ptx::policy_evict_last();  // entry K/V: just produced, re-read by every row chunk
         int slot = 0;
         uint32_t ph = 0;
-        SegIter it(t0, t1);
+        SegIter it(p, t0, t1);
         Seg s;
         while (it.next(p, s)) {
             const int n_pages_valid = (s.u.n_s + p.page - 1) >> p.page_shift;
@@ -272,55 +358,54 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
             }
         }
     } else if (warp == 2) {
-        // ===================== Append(E) (Alg. 1 l.5): K_new / V_new -> the session's pages =====================
-        // Owned by the CTA that runs the last tile of the session's last row chunk, once per (layer, kv head).
-        // Nothing in this launch reads cache positions >= n_s, so the copy needs no ordering with the tiles.
-        SegIter it(t0, t1);
+        // ===================== service warp: Q loader, Append(E), cross-CTA merge =====================
+        SegIter it(p, t0, t1);
         Seg s;
-        constexpr int kChunks = D / 8;  // 16-byte chunks per row
-        constexpr int kBatch = 4;
+        // rows of an M-tile that no box covers are never written: clear the buffer once so they stay finite
+        for (int off = lane * 16; off < p.q_tiles * kTileBytes; off += 32 * 16)
+            *reinterpret_cast<uint4 *>(q_s + off) = make_uint4(0, 0, 0, 0);
+        ptx::fence_proxy_async_smem();
+        __syncwarp();
+        if (lane == 0) ptx::prefetch_tmap(&tm_q);
+        const uint64_t pol_q = ptx::policy_evict_last();  // Q is re-read by every CTA that shares the unit
+        int k = 0;
         while (it.next(p, s)) {
-            if (s.u.tok0 + s.u.ntok != s.u.l_entry || s.te != s.u.n_tiles) continue;
-            const size_t lo = static_cast<size_t>(s.layer);
-            const int32_t *pt = p.a.page_table + static_cast<size_t>(s.u.session) * p.a.page_table_stride;
-            const __nv_bfloat16 *ksrc = p.a.k_new + lo * p.a.kv_new_layer_stride;
-            const __nv_bfloat16 *vsrc = p.a.v_new + lo * p.a.kv_new_layer_stride;
-            __nv_bfloat16 *kpool = p.a.k_pool + lo * p.a.pool_layer_stride;
-            __nv_bfloat16 *vpool = p.a.v_pool + lo * p.a.pool_layer_stride;
-            const int total = s.u.l_entry * kChunks;
-            for (int base = lane; base < total; base += 32 * kBatch) {
-                uint4 kv[kBatch], vv[kBatch];
-                int pg[kBatch];
-#pragma unroll
-                for (int u = 0; u < kBatch; ++u) {
-                    const int idx = base + u * 32;
-                    if (idx < total) {
-                        const int tok = idx / kChunks, c = idx - tok * kChunks;
-                        const size_t so = (static_cast<size_t>(s.u.row0 + tok) * p.Hkv + s.kvh) * D + c * 8;
-                        kv[u] = __ldg(reinterpret_cast<const uint4 *>(ksrc + so));
-                        vv[u] = __ldg(reinterpret_cast<const uint4 *>(vsrc + so));
-                        pg[u] = __ldg(pt + ((s.u.n_s + tok) >> p.page_shift));
+            // ---- Q rows -> smem (swizzled K-major tiles) by TMA, as soon as the previous segment's last QK has read
+            // the buffer.  Row r of the unit is entry token tok0 + r / G, query
+            // head kvh * G + r % G; rows past the unit hold other tokens' Q or zeros and are never written out.
+            if (k > 0) ptx::mbar_wait(ptx::smem_u32(q_empty), (k - 1) & 1);
+            {
+                // one TMA box per 8-row group: gbox = min(G, 8) heads x 8 / gbox tokens x both 64-column halves
+                const int rows = s.u.ntok * G;
+                const int ng = (rows + 7) >> 3;
+                if (lane == 0) ptx::mbar_arrive_expect_tx(ptx::smem_u32(q_full), ng * kGroupStride);
+                __syncwarp();
+                for (int g = lane; g < ng; g += 32) {
+                    int tok, head;
+                    if (G <= 8) {
+                        tok = s.u.tok0 + g * (8 / G);
+                        head = s.kvh * G;
+                    } else {
+                        const int gpt = G >> 3;
+                        tok = s.u.tok0 + g / gpt;
+                        head = s.kvh * G + (g % gpt) * 8;
                     }
-                }
-#pragma unroll
-                for (int u = 0; u < kBatch; ++u) {
-                    const int idx = base + u * 32;
-                    if (idx < total) {
-                        const int tok = idx / kChunks, c = idx - tok * kChunks;
-                        const int j = s.u.n_s + tok;
-                        const size_t po = ((static_cast<size_t>(pg[u]) * p.Hkv + s.kvh) * p.page + (j & (p.page - 1))) * D + c * 8;
-                        *reinterpret_cast<uint4 *>(kpool + po) = kv[u];
-                        *reinterpret_cast<uint4 *>(vpool + po) = vv[u];
-                    }
+                    ptx::tma_load_5d(ptx::smem_u32(q_s + (g >> 4) * kTileBytes + (g & 15) * kGroupStride), &tm_q,
+                                     ptx::smem_u32(q_full), 0, head, s.u.row0 + tok, 0, s.layer, pol_q);
                 }
             }
+            ++k;
+            // ---- Append(E) (Alg. 1 l.5): K_new / V_new -> the session's pages.  Owned by the CTA that runs the last
+            // tile of the session's last row chunk, once per (layer, kv head).  Nothing in this launch reads cache
+            // positions >= n_s, so the copy needs no ordering with the tiles.
+            if (s.u.tok0 + s.u.ntok == s.u.l_entry && s.te == s.u.n_tiles) append_entry<D>(p, s, lane);
         }
     } else if (warp == 1) {
         // ===================== MMA issuer =====================
         int kslot = 0, vslot = 0;
         uint32_t kph = 0, vph = 0, qph = 0;
         uint32_t pph = 0;  // bit w = phase parity of p_ready[w]
-        SegIter it(t0, t1);
+        SegIter it(p, t0, t1);
         Seg s;
         while (it.next(p, s)) {
             const int rows = s.u.ntok * G;
@@ -340,19 +425,24 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
                     ptx::mbar_wait(ptx::smem_u32(&k_full[kslot]), kph);
                     ptx::tc_fence_after();
                 }
-                if (lane == 0) {
-                    const uint32_t qa = ptx::smem_u32(q_s + mt * kTileBytes);
-                    const uint32_t ka = ptx::smem_u32(k_s + kslot * kTileBytes);
+                // descriptor words are warp-uniform and computed by the whole warp; only the tcgen05 instructions sit
+                // under elect (a lane-0 branch would drag every operand through ELECT + R2UR per MMA)
+                const uint32_t qlo = desc_lo(ptx::smem_u32(q_s + mt * kTileBytes), 16);
+                const uint32_t klo = desc_lo(ptx::smem_u32(k_s + kslot * kTileBytes), 16);
+                const uint32_t sd = tmem + kColS + w * 128;
+                const uint32_t sfb = ptx::smem_u32(&s_full[w]), keb = ptx::smem_u32(&k_empty[kslot]);
+                const bool q_last = (i == n_items - 1);
+                if (ptx::elect_one()) {
 #pragma unroll
                     for (int hf = 0; hf < kHalves; ++hf)
 #pragma unroll
                         for (int ks = 0; ks < 4; ++ks) {
-                            const uint32_t off = hf * 1024 + ks * 32;
-                            ptx::umma_ss(tmem + kColS + w * 128, make_desc(qa + off, 16, kGroupStride),
-                                         make_desc(ka + off, 16, kGroupStride), kIdescQK, (hf | ks) != 0);
+                            const uint32_t off = (hf * 1024 + ks * 32) >> 4;
+                            ptx::umma_ss2(sd, qlo + off, klo + off, kDescHi, kIdescQK, (hf | ks) != 0);
                         }
-                    ptx::umma_commit(ptx::smem_u32(&s_full[w]));
-                    if (last_use) ptx::umma_commit(ptx::smem_u32(&k_empty[kslot]));
+                    ptx::umma_commit(sfb);
+                    if (last_use) ptx::umma_commit(keb);
+                    if (q_last) ptx::umma_commit(ptx::smem_u32(q_empty));  // Q may be overwritten
                 }
                 __syncwarp();
                 if (last_use) {
@@ -390,15 +480,16 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
                 ptx::mbar_wait(ptx::smem_u32(&p_ready[w]), (pph >> w) & 1u);
                 pph ^= 1u << w;
                 ptx::tc_fence_after();
-                if (lane == 0) {
-                    const uint32_t va = ptx::smem_u32(v_s + vslot * kTileBytes);
-                    const bool first_pv = (i < 2);  // first PV of stream i & 1 in this segment overwrites O
+                const uint32_t vlo = desc_lo(ptx::smem_u32(v_s + vslot * kTileBytes), 1024);
+                const uint32_t od = tmem + kColO + w * D, pa = tmem + kColS + w * 128;
+                const uint32_t veb = ptx::smem_u32(&v_empty[vslot]);
+                const uint32_t first_pv = (i < 2) ? 0u : 1u;  // first PV of stream i & 1 in this segment overwrites O
+                if (ptx::elect_one()) {
 #pragma unroll
                     for (int ks = 0; ks < kTile / 16; ++ks)
-                        ptx::umma_ts(tmem + kColO + w * D, tmem + kColS + w * 128 + ks * 8,
-                                     make_desc(va + ks * 2 * kGroupStride, 1024, kGroupStride), kIdescPV,
-                                     !(first_pv && ks == 0));
-                    if (last_use) ptx::umma_commit(ptx::smem_u32(&v_empty[vslot]));
+                        ptx::umma_ts2(od, pa + ks * 8, vlo + ((ks * 2 * kGroupStride) >> 4), kDescHi, kIdescPV,
+                                      ks == 0 ? first_pv : 1u);
+                    if (last_use) ptx::umma_commit(veb);
                 }
                 __syncwarp();
                 if (last_use) {
@@ -409,7 +500,7 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
                 }
                 if (i + 2 < n_items) issue_qk(i + 2);
             }
-            if (lane == 0) {
+            if (ptx::elect_one()) {
                 ptx::umma_commit(ptx::smem_u32(&o_done[0]));
                 ptx::umma_commit(ptx::smem_u32(&o_done[1]));
             }
@@ -424,32 +515,13 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
         const uint32_t lane_addr = static_cast<uint32_t>((warp & 3) << 5) << 16;
         const int st = threadIdx.x - 128;                      // 0..255 among softmax threads
         uint32_t sph = 0, oph = 0;
-        SegIter it(t0, t1);
+        SegIter it(p, t0, t1);
         Seg s;
         while (it.next(p, s)) {
             const int rows = s.u.ntok * G;
             const int n_mt = rows > 128 ? 2 : 1;
             const int n_tiles = s.te - s.tb;
             const int n_items = n_tiles * n_mt;
-            // ---- Q rows -> smem (swizzled K-major tiles; rows past the unit zero).  Row r of the unit is entry
-            // token tok0 + r / G, query head kvh * G + r % G.
-            {
-                constexpr int kChunks = D / 8;
-                const __nv_bfloat16 *qb = p.a.q + static_cast<size_t>(s.layer) * p.a.q_layer_stride;
-                for (int idx = st; idx < n_mt * 128 * kChunks; idx += 256) {
-                    const int r = idx / kChunks, c = idx - r * kChunks;
-                    uint4 val = make_uint4(0, 0, 0, 0);
-                    if (r < rows) {
-                        const int tok = s.u.tok0 + r / G, h = s.kvh * G + r % G;
-                        val = __ldg(reinterpret_cast<const uint4 *>(
-                            qb + (static_cast<size_t>(s.u.row0 + tok) * p.Hq + h) * D + c * 8));
-                    }
-                    *reinterpret_cast<uint4 *>(q_s + (r >> 7) * kTileBytes + tile_offset<D>(r & 127, c)) = val;
-                }
-                ptx::fence_proxy_async_smem();
-                ptx::tc_fence_before();  // epilogue TMEM reads of the previous segment precede this arrive
-                ptx::mbar_arrive(ptx::smem_u32(q_full));
-            }
             const int mt = (n_mt == 2) ? w : 0;
             const int urow = mt * 128 + row;                   // row within the unit
             const int my_tok = s.u.tok0 + urow / G;            // entry token of this row (if urow < rows)
@@ -470,62 +542,79 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
                 ptx::mbar_wait(ptx::smem_u32(&s_full[w]), sph);
                 sph ^= 1;
                 ptx::tc_fence_after();
-                uint32_t sr[128];
-                {
-                    const uint32_t sa = tmem + lane_addr + kColS + w * 128;
-                    ptx::tmem_ld_32x32b_x32(sa, sr);
-                    ptx::tmem_ld_32x32b_x32(sa + 32, sr + 32);
-                    ptx::tmem_ld_32x32b_x32(sa + 64, sr + 64);
-                    ptx::tmem_ld_32x32b_x32(sa + 96, sr + 96);
-                    ptx::tmem_ld_wait();
-                }
-                float mx = -CUDART_INF_F;
-                if (limit >= kTile) {
-#pragma unroll
-                    for (int c = 0; c < 128; ++c) mx = fmaxf(mx, __uint_as_float(sr[c]));
-                } else {
-#pragma unroll
-                    for (int c = 0; c < 128; ++c) {
-                        const float v = (c < limit) ? __uint_as_float(sr[c]) : -CUDART_INF_F;
-                        sr[c] = __float_as_uint(v);
-                        mx = fmaxf(mx, v);
+                // The tile body exists twice (all columns visible / masked at `limit`): one body with a branch
+                // around the masking makes the compiler copy the whole 128-register score row at the join.
+                auto tile_body = [&](auto masked_tag) {
+                    constexpr bool kMasked = decltype(masked_tag)::value;
+                    uint32_t sr[128];
+                    {
+                        const uint32_t sa = tmem + lane_addr + kColS + w * 128;
+                        ptx::tmem_ld_32x32b_x32(sa, sr);
+                        ptx::tmem_ld_32x32b_x32(sa + 32, sr + 32);
+                        ptx::tmem_ld_32x32b_x32(sa + 64, sr + 64);
+                        ptx::tmem_ld_32x32b_x32(sa + 96, sr + 96);
+                        ptx::tmem_ld_wait();
                     }
-                }
-                const float m_new = fmaxf(m_used, mx * p.scale_log2);
-                // lazy rescale, warp-uniform because the TMEM round trip of O is warp-collective
-                const bool need = (m_new > m_used + kRescaleThreshold);
-                if (__any_sync(0xffffffffu, need)) {
-                    const float alpha = (m_used == -CUDART_INF_F) ? 0.f : exp2f(m_used - m_new);
-                    l_sum *= alpha;
-                    if (have) {
-                        const uint32_t oa = tmem + lane_addr + kColO + w * D;
+                    float mx = -CUDART_INF_F;
+                    if constexpr (kMasked) {
 #pragma unroll
-                        for (int cb = 0; cb < D; cb += 32) {
-                            uint32_t o[32];
-                            ptx::tmem_ld_32x32b_x32(oa + cb, o);
-                            ptx::tmem_ld_wait();
-#pragma unroll
-                            for (int c = 0; c < 32; ++c) o[c] = __float_as_uint(__uint_as_float(o[c]) * alpha);
-                            ptx::tmem_st_32x32b_x32(oa + cb, o);
+                        for (int c = 0; c < 128; ++c) {
+                            const float v = (c < limit) ? __uint_as_float(sr[c]) : -CUDART_INF_F;
+                            sr[c] = __float_as_uint(v);
+                            mx = fmaxf(mx, v);
                         }
-                    }
-                    m_used = m_new;
-                }
-                const float m_eff = (m_used == -CUDART_INF_F) ? 0.f : m_used;  // fully masked so far: p = 0
-                const float neg_m = -m_eff;
-                const uint32_t pa = tmem + lane_addr + kColS + w * 128;
+                    } else {
 #pragma unroll
-                for (int cb = 0; cb < 128; cb += 64) {
-                    uint32_t pk[32];
-#pragma unroll
-                    for (int c = 0; c < 64; c += 2) {
-                        const float p0 = ptx::ex2(fmaf(__uint_as_float(sr[cb + c]), p.scale_log2, neg_m));
-                        const float p1 = ptx::ex2(fmaf(__uint_as_float(sr[cb + c + 1]), p.scale_log2, neg_m));
-                        l_sum += p0 + p1;
-                        pk[c >> 1] = pack_bf16(p0, p1);
+                        for (int c = 0; c < 128; ++c) mx = fmaxf(mx, __uint_as_float(sr[c]));
                     }
-                    ptx::tmem_st_32x32b_x32(pa + (cb >> 1), pk);
-                }
+                    const float m_new = fmaxf(m_used, mx * p.scale_log2);
+                    // lazy rescale, warp-uniform because the TMEM round trip of O is warp-collective
+                    const bool need = (m_new > m_used + kRescaleThreshold);
+                    if (__any_sync(0xffffffffu, need)) {
+                        const float alpha = (m_used == -CUDART_INF_F) ? 0.f : exp2f(m_used - m_new);
+                        l_sum *= alpha;
+                        if (have) {
+                            const uint32_t oa = tmem + lane_addr + kColO + w * D;
+#pragma unroll 1
+                            for (int cb = 0; cb < D; cb += 32) {
+                                uint32_t o[32];
+                                ptx::tmem_ld_32x32b_x32(oa + cb, o);
+                                ptx::tmem_ld_wait();
+#pragma unroll
+                                for (int c = 0; c < 32; ++c) o[c] = __float_as_uint(__uint_as_float(o[c]) * alpha);
+                                ptx::tmem_st_32x32b_x32(oa + cb, o);
+                            }
+                        }
+                        m_used = m_new;
+                    }
+                    const float m_eff = (m_used == -CUDART_INF_F) ? 0.f : m_used;  // fully masked so far: p = 0
+                    const float neg_m = -m_eff;
+                    const uint32_t pa = tmem + lane_addr + kColS + w * 128;
+                    // packed fp32 pairs: one FFMA2 scales two scores, one FADD2 adds two probabilities to the row sum
+                    const uint64_t sc2 = ptx::pack_f32x2(p.scale_log2, p.scale_log2), nm2 = ptx::pack_f32x2(neg_m, neg_m);
+                    uint64_t acc_a = 0ull, acc_b = 0ull;
+#pragma unroll
+                    for (int cb = 0; cb < 128; cb += 32) {
+                        uint32_t pk[16];
+#pragma unroll
+                        for (int c = 0; c < 32; c += 2) {
+                            const uint64_t x2 = ptx::fma_f32x2(
+                                ptx::pack_f32x2(__uint_as_float(sr[cb + c]), __uint_as_float(sr[cb + c + 1])), sc2, nm2);
+                            float x0, x1;
+                            ptx::unpack_f32x2(x2, x0, x1);
+                            const float p0 = ptx::ex2(x0), p1 = ptx::ex2(x1);
+                            if (c & 2) acc_b = ptx::add_f32x2(acc_b, ptx::pack_f32x2(p0, p1));
+                            else acc_a = ptx::add_f32x2(acc_a, ptx::pack_f32x2(p0, p1));
+                            pk[c >> 1] = pack_bf16(p0, p1);
+                        }
+                        ptx::tmem_st_32x32b_x16(pa + (cb >> 1), pk);
+                    }
+                    float a0, a1;
+                    ptx::unpack_f32x2(ptx::add_f32x2(acc_a, acc_b), a0, a1);
+                    l_sum += a0 + a1;
+                };
+                if (limit >= kTile) tile_body(std::false_type{});
+                else tile_body(std::true_type{});
                 ptx::tmem_st_wait();
                 ptx::tc_fence_before();
                 ptx::mbar_arrive(ptx::smem_u32(&p_ready[w]));
@@ -536,7 +625,7 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
             oph ^= 1;
             ptx::tc_fence_after();
             __nv_bfloat16 *ob = p.a.out + static_cast<size_t>(s.layer) * p.a.out_layer_stride;
-            float *slot = p.partials + static_cast<size_t>(2 * blockIdx.x + (s.first ? 0 : 1)) * (kAttnMaxRows * (D + 2));
+            float *slot = p.partials + static_cast<size_t>(2 * blockIdx.x + s.slot) * (kAttnMaxRows * (D + 2));
             if (n_mt == 2) {
                 // stream w owns M-tile w: rows urow, all D columns
                 const float inv = 1.f / l_sum;
@@ -729,6 +818,31 @@ int encode_new_map(CUtensorMap *tm, const void *base, const prepos_model_shape &
     return PREPOS_OK;
 }
 
+// Q [layer][sum_L][Hq][d]: a box is one 8-row group of a unit's Q tile, rows ordered (token, head within the kv
+// group): min(G, 8) heads x 8 / min(G, 8) tokens, laid out [64-column half][8 rows][128 B] with the 128-byte swizzle
+int encode_q_map(CUtensorMap *tm, const void *base, const prepos_model_shape &s, int64_t layer_stride, int64_t sum_rows)
+{
+    EncodeTiledFn encode = reinterpret_cast<EncodeTiledFn>(prepos_get_encode_tiled());
+    if (!encode) return PREPOS_E_CUDA;
+    const int D = s.head_dim, halves = D / 64, G = s.n_q_heads / s.n_kv_heads;
+    const int gbox = G < 8 ? G : 8, tbox = 8 / gbox;
+    const cuuint64_t tok_stride = static_cast<cuuint64_t>(s.n_q_heads) * D * 2;
+    const cuuint64_t lstride = (s.layers > 1) ? static_cast<cuuint64_t>(layer_stride) * 2 : tok_stride * static_cast<cuuint64_t>(sum_rows);
+    const cuuint64_t dims[5] = {64, static_cast<cuuint64_t>(s.n_q_heads), static_cast<cuuint64_t>(sum_rows),
+                                static_cast<cuuint64_t>(halves), static_cast<cuuint64_t>(s.layers)};
+    const cuuint64_t strides[4] = {static_cast<cuuint64_t>(D) * 2, tok_stride, 128, lstride};
+    const cuuint32_t box[5] = {64, static_cast<cuuint32_t>(gbox), static_cast<cuuint32_t>(tbox), static_cast<cuuint32_t>(halves), 1};
+    const cuuint32_t estr[5] = {1, 1, 1, 1, 1};
+    const CUresult r = encode(tm, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 5, const_cast<void *>(base), dims, strides, box, estr,
+                              CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
+                              CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) {
+        fprintf(stderr, "libprepos: cuTensorMapEncodeTiled(Q) failed: %d\n", static_cast<int>(r));
+        return PREPOS_E_CUDA;
+    }
+    return PREPOS_OK;
+}
+
 template <int D>
 int launch(prepos_ctx *ctx, const AttnArgs &a, int tiles_per_lh, cudaStream_t stream)
 {
@@ -778,11 +892,18 @@ int launch(prepos_ctx *ctx, const AttnArgs &a, int tiles_per_lh, cudaStream_t st
         ctx->tm_new_layer_stride = a.kv_new_layer_stride;
         ctx->tm_new_rows = a.sum_rows;
     }
+    if (ctx->tm_q_ptr != a.q || ctx->tm_q_layer_stride != a.q_layer_stride || ctx->tm_q_rows != a.sum_rows) {
+        const int st = encode_q_map(&ctx->tm_q, a.q, ctx->shape, a.q_layer_stride, a.sum_rows);
+        if (st != PREPOS_OK) return st;
+        ctx->tm_q_ptr = a.q;
+        ctx->tm_q_layer_stride = a.q_layer_stride;
+        ctx->tm_q_rows = a.sum_rows;
+    }
     if (static_cast<size_t>(p.n_lh) * a.n_units > ctx->attn_counters_n) return PREPOS_E_WORKSPACE;
     p.counters = ctx->attn_counters;
     PREPOS_CUDA_TRY(cudaFuncSetAttribute(attn_umma_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                          static_cast<int>(smem)));
-    attn_umma_kernel<D><<<static_cast<int>(grid), kThreads, smem, stream>>>(ctx->tm_k, ctx->tm_v, ctx->tm_kn, ctx->tm_vn, p);
+    attn_umma_kernel<D><<<static_cast<int>(grid), kThreads, smem, stream>>>(ctx->tm_k, ctx->tm_v, ctx->tm_kn, ctx->tm_vn, ctx->tm_q, p);
     PREPOS_CUDA_TRY(cudaGetLastError());
     ctx->launches += 1;
     return PREPOS_OK;
@@ -793,7 +914,9 @@ int launch(prepos_ctx *ctx, const AttnArgs &a, int tiles_per_lh, cudaStream_t st
 bool prepos_attn_umma_supported(const prepos_ctx *ctx)
 {
     const prepos_model_shape &s = ctx->shape;
-    return (s.head_dim == 64 || s.head_dim == 128) && s.page_size >= 8 && s.page_size <= kTile;
+    const int G = s.n_q_heads / s.n_kv_heads;
+    return (s.head_dim == 64 || s.head_dim == 128) && s.page_size >= 8 && s.page_size <= kTile &&
+           (G & (G - 1)) == 0;  // the Q boxes take whole 8-row groups of (token, head) rows
 }
 
 int prepos_launch_attn_umma(prepos_ctx *ctx, const AttnArgs &a, int tiles_per_lh, cudaStream_t stream)

@@ -91,6 +91,10 @@ struct prepos_ctx {
     const void *tm_kn_ptr, *tm_vn_ptr;
     int64_t tm_new_layer_stride, tm_new_rows;
     CUtensorMap tm_kn, tm_vn;
+    // ... and for the call's Q
+    const void *tm_q_ptr;
+    int64_t tm_q_layer_stride, tm_q_rows;
+    CUtensorMap tm_q;
 };
 
 // ---- per-file launchers (all return a PREPOS_* status) -------------------------------------------
