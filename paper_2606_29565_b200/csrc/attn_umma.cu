@@ -711,16 +711,20 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
             }
             // ---- the single cross-CTA pass: the last CTA to deliver its partial of a cut unit combines them
             if (!s.direct) {
-                __threadfence();
+                // the barrier orders every thread's partial stores before thread 0's release fence + ticket
                 ptx::bar_sync(1, 256);
                 if (st == 0) {
                     const long long U0 = static_cast<long long>(s.lh) * p.tiles_per_lh + s.u.tile_prefix;
                     const int c0 = cta_of(p.total_tiles, gridDim.x, U0);
                     const int c1 = cta_of(p.total_tiles, gridDim.x, U0 + s.u.n_tiles - 1);
                     unsigned int *cnt = p.counters + static_cast<size_t>(s.lh) * p.a.n_units + s.unit_idx;
+                    ptx::fence_acq_rel_gpu();
                     const unsigned int prev = atomicAdd(cnt, 1u);
                     const bool last = (prev == static_cast<unsigned int>(c1 - c0));
-                    if (last) *cnt = 0u;  // self-reset for the next launch
+                    if (last) {
+                        *cnt = 0u;  // self-reset for the next launch
+                        ptx::fence_acq_rel_gpu();
+                    }
                     merge_info[0] = last ? c0 : -1;
                     merge_info[1] = c1;
                     merge_info[2] = (cta_begin(p.total_tiles, gridDim.x, c0) < U0) ? 1 : 0;  // c0's slot for this unit
@@ -728,26 +732,54 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
                 ptx::bar_sync(1, 256);
                 const int c0 = merge_info[0], c1 = merge_info[1], c0_slot = merge_info[2];
                 if (c0 >= 0) {
-                    __threadfence();
                     constexpr int kVec = D / 4;  // float4 per row
+                    constexpr int kMaxC = 4;     // partials combined with all loads in flight; more take the loop
                     constexpr size_t kSlotFloats = static_cast<size_t>(kAttnMaxRows) * (D + 2);
                     const float *base0 = p.partials + (2 * static_cast<size_t>(c0) + c0_slot) * kSlotFloats;
+                    const int nc = c1 - c0 + 1;
                     for (int idx = st; idx < rows * kVec; idx += 256) {
                         const int r = idx / kVec, v = idx - r * kVec;
-                        float M = __ldcg(base0 + kAttnMaxRows * D + r);
-                        for (int c = c0 + 1; c <= c1; ++c)
-                            M = fmaxf(M, __ldcg(p.partials + 2 * static_cast<size_t>(c) * kSlotFloats + kAttnMaxRows * D + r));
                         float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
                         float wsum = 0.f;
-                        for (int c = c0; c <= c1; ++c) {
-                            const float *sl = (c == c0) ? base0 : p.partials + 2 * static_cast<size_t>(c) * kSlotFloats;
-                            const float wgt = exp2f(__ldcg(sl + kAttnMaxRows * D + r) - M);
-                            const float4 o = __ldcg(reinterpret_cast<const float4 *>(sl + static_cast<size_t>(r) * D) + v);
-                            acc.x = fmaf(wgt, o.x, acc.x);
-                            acc.y = fmaf(wgt, o.y, acc.y);
-                            acc.z = fmaf(wgt, o.z, acc.z);
-                            acc.w = fmaf(wgt, o.w, acc.w);
-                            wsum += wgt;
+                        if (nc <= kMaxC) {
+                            float lse[kMaxC];
+                            float4 o[kMaxC];
+#pragma unroll
+                            for (int j = 0; j < kMaxC; ++j) {
+                                const float *sl = (j == 0) ? base0 : p.partials + 2 * static_cast<size_t>(c0 + j) * kSlotFloats;
+                                lse[j] = -CUDART_INF_F;
+                                o[j] = make_float4(0.f, 0.f, 0.f, 0.f);
+                                if (j < nc) {
+                                    lse[j] = __ldcg(sl + kAttnMaxRows * D + r);
+                                    o[j] = __ldcg(reinterpret_cast<const float4 *>(sl + static_cast<size_t>(r) * D) + v);
+                                }
+                            }
+                            float M = lse[0];
+#pragma unroll
+                            for (int j = 1; j < kMaxC; ++j) M = fmaxf(M, lse[j]);
+#pragma unroll
+                            for (int j = 0; j < kMaxC; ++j) {  // CTA order
+                                const float wgt = (j < nc) ? exp2f(lse[j] - M) : 0.f;
+                                acc.x = fmaf(wgt, o[j].x, acc.x);
+                                acc.y = fmaf(wgt, o[j].y, acc.y);
+                                acc.z = fmaf(wgt, o[j].z, acc.z);
+                                acc.w = fmaf(wgt, o[j].w, acc.w);
+                                wsum += wgt;
+                            }
+                        } else {
+                            float M = __ldcg(base0 + kAttnMaxRows * D + r);
+                            for (int c = c0 + 1; c <= c1; ++c)
+                                M = fmaxf(M, __ldcg(p.partials + 2 * static_cast<size_t>(c) * kSlotFloats + kAttnMaxRows * D + r));
+                            for (int c = c0; c <= c1; ++c) {
+                                const float *sl = (c == c0) ? base0 : p.partials + 2 * static_cast<size_t>(c) * kSlotFloats;
+                                const float wgt = exp2f(__ldcg(sl + kAttnMaxRows * D + r) - M);
+                                const float4 o = __ldcg(reinterpret_cast<const float4 *>(sl + static_cast<size_t>(r) * D) + v);
+                                acc.x = fmaf(wgt, o.x, acc.x);
+                                acc.y = fmaf(wgt, o.y, acc.y);
+                                acc.z = fmaf(wgt, o.z, acc.z);
+                                acc.w = fmaf(wgt, o.w, acc.w);
+                                wsum += wgt;
+                            }
                         }
                         const float inv = 1.f / wsum;
                         const int tok = s.u.tok0 + r / G, h = s.kvh * G + r % G;

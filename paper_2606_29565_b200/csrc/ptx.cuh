@@ -62,6 +62,12 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)
     }
 }
 
+// release / acquire at GPU scope (lighter than __threadfence(), which is sequentially consistent)
+__device__ __forceinline__ void fence_acq_rel_gpu()
+{
+    asm volatile("fence.acq_rel.gpu;" ::: "memory");
+}
+
 // generic-proxy smem writes -> visible to the async proxy (TMA / UMMA)
 __device__ __forceinline__ void fence_proxy_async_smem()
 {
