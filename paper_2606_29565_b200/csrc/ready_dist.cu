@@ -175,6 +175,35 @@ struct RdParams {
     unsigned int *counter;
 };
 
+// The single cross-CTA pass: the last CTA to arrive merges the per-CTA partials of every hidden row in CTA order
+// and writes the records (Alg. 1 l.10-12: position, dist (here: argmax, gamma, max, lse), decoded/valid).
+// Called by all threads of the CTA after their partials are stored (and fenced).
+__device__ __forceinline__ void finalize_records(const RdParams &p, int warp, int lane, int n_warps)
+{
+    __shared__ int s_is_last;
+    if (threadIdx.x == 0) {
+        const unsigned int prev = atomicAdd(p.counter, 1u);
+        s_is_last = (prev == gridDim.x - 1);
+    }
+    __syncthreads();
+    if (!s_is_last) return;
+    __threadfence();
+    for (int row = warp; row < p.n; row += n_warps) {
+        const Top2Lse t = merge_partials_warp(p.partials, row, gridDim.x, lane);
+        if (lane == 0 && !(p.skip_mask && p.skip_mask[row])) {
+            const int sid = p.session_ids[row];
+            prepos_record *rec = p.records + sid;
+            write_record_fields(rec, t);
+            rec->entry_hash = p.entry_hash ? p.entry_hash[row] : 0ull;
+            rec->position = p.position_p ? p.position_p[row] : 0ll;
+            rec->version = p.session_version[sid];
+            __threadfence();  // payload before the valid bit
+            rec->flags = PREPOS_FLAG_VALID | (t.nonfinite ? PREPOS_FLAG_NONFINITE : 0u);
+        }
+    }
+    if (threadIdx.x == 0) *p.counter = 0u;  // self-reset for the next launch on this stream
+}
+
 __global__ void __launch_bounds__(kThreads, 1)
 ready_dist_kernel(const __grid_constant__ CUtensorMap tm_w, const RdParams p)
 {
@@ -189,8 +218,6 @@ ready_dist_kernel(const __grid_constant__ CUtensorMap tm_w, const RdParams p)
     uint64_t *full_bar = bars;
     uint64_t *empty_bar = bars + kMaxStages;
     RdPartial *warp_part = reinterpret_cast<RdPartial *>(bars + 2 * kMaxStages);  // [kConsumerWarps][kNB]
-    __shared__ int s_is_last;
-
     const int warp = threadIdx.x >> 5;
     const int lane = threadIdx.x & 31;
     const int n_tiles = (p.V + kTileRows - 1) / kTileRows;
@@ -324,28 +351,172 @@ ready_dist_kernel(const __grid_constant__ CUtensorMap tm_w, const RdParams p)
         __threadfence();
     }
     __syncthreads();
+    finalize_records(p, warp, lane, kThreads / 32);
+}
+
+// ---- a3 + a4 for a batch of sessions (9..128 hidden rows per launch): one pass over W for all of them ----------
+// With more than a handful of hidden rows the LM head is a real contraction [n x H] . [H x V]: tcgen05.mma with the
+// hidden rows as the M operand (rows past n are zero-filled by TMA or never read back), a 128-row vocabulary tile
+// as the N operand, fp32 accumulators in TMEM.  D[session][vocab row]: TMEM lane = session, so one epilogue thread
+// owns one session and scans its 128 new logits per tile into ONE (top1, top2, max, sum-exp) state -- no cross-lane
+// reduction at all.  Still a pure HBM stream of W: the [x_rows x 128] slice of the hidden rows that rides along in
+// each stage comes from L2.
+constexpr int kBThreads = 192;  // warp 0: TMA, warp 1: MMA issue + TMEM, warps 2-5: epilogue (one TMEM quadrant each)
+constexpr int kBMaxStages = 5;
+
+__device__ __forceinline__ uint32_t rd_desc_lo(uint32_t saddr) { return ((saddr >> 4) & 0x3fffu) | (1u << 16); }
+constexpr uint32_t kRdDescHi = (1024u >> 4) | (1u << 14) | (2u << 29);  // SBO 1024 B, version 1, SWIZZLE_128B
+constexpr uint32_t kRdIdesc = (1u << 4) | (1u << 7) | (1u << 10) | ((128u >> 3) << 17) | ((128u >> 4) << 24);
+
+__global__ void __launch_bounds__(kBThreads, 1)
+ready_dist_batch_kernel(const __grid_constant__ CUtensorMap tm_w, const __grid_constant__ CUtensorMap tm_x,
+                        const RdParams p)
+{
+    extern __shared__ __align__(1024) uint8_t smem_raw[];
+    uint8_t *smem = reinterpret_cast<uint8_t *>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
+    const int x_box_bytes = p.x_rows * kBoxCols * 2;          // one 64-column box of the hidden rows
+    const int stage_bytes = kStageBytes + 2 * x_box_bytes;    // W [128 x 128] + X [x_rows x 128]
+    // the M = 128 MMA reads 128 rows of the hidden-row boxes: with x_rows < 128 it runs past the last stage into
+    // this pad (garbage rows of D that no thread reads back), which keeps the reads inside the CTA's allocation
+    const int pad_bytes = kBoxBytes - x_box_bytes;
+    uint64_t *bars = reinterpret_cast<uint64_t *>(smem + static_cast<size_t>(p.n_stages) * stage_bytes + pad_bytes);
+    uint64_t *full_bar = bars, *empty_bar = bars + kBMaxStages;
+    uint64_t *d_full = bars + 2 * kBMaxStages, *d_empty = d_full + 2;
+    uint32_t *tmem_slot = reinterpret_cast<uint32_t *>(d_empty + 2);
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int n_tiles = (p.V + kTileRows - 1) / kTileRows;
+    const int n_kc = p.H / kStageCols;
+
     if (threadIdx.x == 0) {
-        const unsigned int prev = atomicAdd(p.counter, 1u);
-        s_is_last = (prev == gridDim.x - 1);
+        for (int s = 0; s < p.n_stages; ++s) {
+            ptx::mbar_init(ptx::smem_u32(&full_bar[s]), 1);
+            ptx::mbar_init(ptx::smem_u32(&empty_bar[s]), 1);
+        }
+        for (int b = 0; b < 2; ++b) {
+            ptx::mbar_init(ptx::smem_u32(&d_full[b]), 1);
+            ptx::mbar_init(ptx::smem_u32(&d_empty[b]), 128);
+        }
+        ptx::fence_mbar_init();
     }
+    if (warp == 1) {
+        ptx::tmem_alloc<256>(ptx::smem_u32(tmem_slot));
+        ptx::tmem_relinquish();
+    }
+    ptx::tc_fence_before();
     __syncthreads();
-    if (!s_is_last) return;
-    __threadfence();
-    if (warp < p.n) {
-        const Top2Lse t = merge_partials_warp(p.partials, warp, gridDim.x, lane);
-        if (lane == 0 && !(p.skip_mask && p.skip_mask[warp])) {
-            const int sid = p.session_ids[warp];
-            prepos_record *rec = p.records + sid;
-            // Alg. 1 l.10-12: position, dist (here: argmax, gamma, max, lse), decoded/valid.
-            write_record_fields(rec, t);
-            rec->entry_hash = p.entry_hash ? p.entry_hash[warp] : 0ull;
-            rec->position = p.position_p ? p.position_p[warp] : 0ll;
-            rec->version = p.session_version[sid];
-            __threadfence();  // payload before the valid bit
-            rec->flags = PREPOS_FLAG_VALID | (t.nonfinite ? PREPOS_FLAG_NONFINITE : 0u);
+    ptx::tc_fence_after();
+    const uint32_t tmem = *tmem_slot;
+
+    if (warp == 0) {
+        // ===== TMA producer: W stage (two 64-column boxes) + the matching columns of the hidden rows =====
+        if (lane == 0) {
+            ptx::prefetch_tmap(&tm_w);
+            ptx::prefetch_tmap(&tm_x);
+            const uint64_t pol_w = ptx::policy_evict_first();  // W is read once per pass
+            const uint64_t pol_x = ptx::policy_evict_last();   // the hidden rows are re-read by every tile
+            int stage = 0;
+            uint32_t phase = 0;
+            for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+                for (int kc = 0; kc < n_kc; ++kc) {
+                    ptx::mbar_wait(ptx::smem_u32(&empty_bar[stage]), phase ^ 1);
+                    const uint32_t fb = ptx::smem_u32(&full_bar[stage]);
+                    ptx::mbar_arrive_expect_tx(fb, stage_bytes);
+                    const uint32_t dst = ptx::smem_u32(smem + static_cast<size_t>(stage) * stage_bytes);
+                    ptx::tma_load_2d(dst, &tm_w, fb, kc * kStageCols, tile * kTileRows, pol_w);
+                    ptx::tma_load_2d(dst + kBoxBytes, &tm_w, fb, kc * kStageCols + kBoxCols, tile * kTileRows, pol_w);
+                    ptx::tma_load_2d(dst + kStageBytes, &tm_x, fb, kc * kStageCols, 0, pol_x);
+                    ptx::tma_load_2d(dst + kStageBytes + x_box_bytes, &tm_x, fb, kc * kStageCols + kBoxCols, 0, pol_x);
+                    if (++stage == p.n_stages) {
+                        stage = 0;
+                        phase ^= 1;
+                    }
+                }
+            }
+        }
+    } else if (warp == 1) {
+        // ===== MMA issuer: D[buf] = X . W_tile^T over H, 8 x k16 per stage =====
+        int stage = 0, it = 0;
+        uint32_t phase = 0;
+        for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x, ++it) {
+            const int buf = it & 1;
+            ptx::mbar_wait(ptx::smem_u32(&d_empty[buf]), ((it >> 1) & 1) ^ 1);
+            ptx::tc_fence_after();
+            const uint32_t d = tmem + buf * 128;
+            for (int kc = 0; kc < n_kc; ++kc) {
+                ptx::mbar_wait(ptx::smem_u32(&full_bar[stage]), phase);
+                ptx::tc_fence_after();
+                const uint32_t sb = ptx::smem_u32(smem + static_cast<size_t>(stage) * stage_bytes);
+                const uint32_t wlo = rd_desc_lo(sb), xlo = rd_desc_lo(sb + kStageBytes);
+                const uint32_t xbox = static_cast<uint32_t>(x_box_bytes) >> 4;
+                const uint32_t eb = ptx::smem_u32(&empty_bar[stage]), fb = ptx::smem_u32(&d_full[buf]);
+                const uint32_t acc0 = (kc != 0);
+                const bool last = (kc == n_kc - 1);
+                if (ptx::elect_one()) {
+#pragma unroll
+                    for (int ks = 0; ks < 8; ++ks) {
+                        const uint32_t koff = ((ks & 3) * 32) >> 4;
+                        ptx::umma_ss2(d, xlo + (ks >> 2) * xbox + koff, wlo + (ks >> 2) * (kBoxBytes >> 4) + koff, kRdDescHi,
+                                      kRdIdesc, ks == 0 ? acc0 : 1u);
+                    }
+                    ptx::umma_commit(eb);
+                    if (last) ptx::umma_commit(fb);
+                }
+                __syncwarp();
+                if (++stage == p.n_stages) {
+                    stage = 0;
+                    phase ^= 1;
+                }
+            }
+        }
+    } else {
+        // ===== epilogue: thread = session (TMEM lane), scans the tile's 128 logits =====
+        const int sess = ((warp & 3) << 5) | lane;
+        const uint32_t lane_addr = static_cast<uint32_t>((warp & 3) << 5) << 16;
+        const bool live = sess < p.n;
+        Top2Lse st = t2_init();
+        int it = 0;
+        for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x, ++it) {
+            const int buf = it & 1;
+            ptx::mbar_wait(ptx::smem_u32(&d_full[buf]), (it >> 1) & 1);
+            ptx::tc_fence_after();
+            const int v0 = tile * kTileRows;
+            const int nv = (p.V - v0 < kTileRows) ? p.V - v0 : kTileRows;
+#pragma unroll 1
+            for (int cb = 0; cb < kTileRows; cb += 32) {
+                uint32_t r[32];
+                ptx::tmem_ld_32x32b_x32(tmem + lane_addr + buf * 128 + cb, r);
+                ptx::tmem_ld_wait();
+                if (live) {
+#pragma unroll
+                    for (int c = 0; c < 32; ++c)
+                        if (cb + c < nv) t2_push(st, __uint_as_float(r[c]), v0 + cb + c);
+                    if (p.logits_out) {
+                        float *lo = p.logits_out + static_cast<size_t>(sess) * p.V + v0 + cb;
+                        if (cb + 32 <= nv && ((reinterpret_cast<uintptr_t>(lo) & 15) == 0)) {
+#pragma unroll
+                            for (int c = 0; c < 32; c += 4)
+                                *reinterpret_cast<uint4 *>(lo + c) = make_uint4(r[c], r[c + 1], r[c + 2], r[c + 3]);
+                        } else {
+#pragma unroll
+                            for (int c = 0; c < 32; ++c)
+                                if (cb + c < nv) lo[c] = __uint_as_float(r[c]);
+                        }
+                    }
+                }
+            }
+            ptx::tc_fence_before();
+            ptx::mbar_arrive(ptx::smem_u32(&d_empty[buf]));
+        }
+        if (live) {
+            t2_store(p.partials + static_cast<size_t>(sess) * kMaxRdPartials + blockIdx.x, st);
+            __threadfence();
         }
     }
-    if (threadIdx.x == 0) *p.counter = 0u;  // self-reset for the next launch on this stream
+    ptx::tc_fence_before();
+    __syncthreads();
+    if (warp == 1) ptx::tmem_dealloc<256>(tmem);
+    finalize_records(p, warp, lane, kBThreads / 32);
 }
 
 // ---- a4': scan of stored fp32 logits ---------------------------------------------------------------
@@ -434,6 +605,45 @@ int prepos_launch_ready_dist(prepos_ctx *ctx, int n, const int32_t *session_ids,
 
     const int n_tiles = (V + kTileRows - 1) / kTileRows;
     const int grid = n_tiles < ctx->num_sms ? n_tiles : ctx->num_sms;
+    if (n > kNB) {
+        // a batch of sessions: one pass over W per 128 hidden rows on the tensor cores
+        for (int r0 = 0; r0 < n; r0 += kRdMaxRows) {
+            RdParams p;
+            p.n = (n - r0 < kRdMaxRows) ? n - r0 : kRdMaxRows;
+            p.H = H;
+            p.V = V;
+            p.x_rows = p.n <= 32 ? 32 : (p.n <= 64 ? 64 : 128);
+            CUtensorMap tmx;
+            const cuuint64_t xdims[2] = {static_cast<cuuint64_t>(H), static_cast<cuuint64_t>(p.n)};
+            const cuuint32_t xbox[2] = {kBoxCols, static_cast<cuuint32_t>(p.x_rows)};
+            if (encode(&tmx, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<__nv_bfloat16 *>(hidden + static_cast<size_t>(r0) * H),
+                       xdims, strides, xbox, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
+                       CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+                return PREPOS_E_CUDA;
+            const int stage_bytes = kStageBytes + 2 * p.x_rows * kBoxCols * 2;
+            const size_t fixed = 1024 + (kBoxBytes - p.x_rows * kBoxCols * 2) + (2 * kBMaxStages + 4) * 8 + 16;
+            int stages = static_cast<int>((232448 - fixed) / stage_bytes);
+            if (stages > kBMaxStages) stages = kBMaxStages;
+            p.n_stages = stages;
+            p.hidden = hidden + static_cast<size_t>(r0) * H;
+            p.session_ids = session_ids + r0;
+            p.position_p = position_p ? position_p + r0 : nullptr;
+            p.entry_hash = entry_hash ? entry_hash + r0 : nullptr;
+            p.skip_mask = skip_mask ? skip_mask + r0 : nullptr;
+            p.records = records;
+            p.session_version = session_version;
+            p.logits_out = logits_out ? logits_out + static_cast<size_t>(r0) * V : nullptr;
+            p.partials = ctx->rd_partials;
+            p.counter = ctx->rd_counter;
+            const size_t smem = fixed + static_cast<size_t>(stages) * stage_bytes;
+            PREPOS_CUDA_TRY(cudaFuncSetAttribute(ready_dist_batch_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                                 static_cast<int>(smem)));
+            ready_dist_batch_kernel<<<grid, kBThreads, smem, stream>>>(tm, tmx, p);
+            PREPOS_CUDA_TRY(cudaGetLastError());
+            ctx->launches += 1;
+        }
+        return PREPOS_OK;
+    }
     for (int r0 = 0; r0 < n; r0 += kNB) {
         RdParams p;
         p.n = (n - r0 < kNB) ? n - r0 : kNB;

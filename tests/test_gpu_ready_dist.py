@@ -61,9 +61,13 @@ def test_config1_many_seeds_records_and_gate(prepos, oracle):
     assert 20 <= served <= 100      # planted rows with realised gap >= 3 fire; unplanted never
 
 
-@pytest.mark.parametrize("V,H,n", [(1000, 128, 3), (130, 384, 1), (257, 256, 9), (4096, 1024, 8), (2, 128, 1)])
+@pytest.mark.parametrize("V,H,n", [(1000, 128, 3), (130, 384, 1), (257, 256, 9), (4096, 1024, 8), (2, 128, 1),
+                                   (1000, 128, 33), (513, 256, 64), (300, 384, 100), (4096, 1024, 128), (200, 128, 130),
+                                   (20000, 512, 17)])
 def test_ragged_vocab_and_batches(prepos, oracle, V, H, n):
-    """V not a multiple of the 128-row tile, H with a single stage, n crossing the 8-row pass."""
+    """V not a multiple of the 128-row tile, H with a single stage, n crossing the 8-row pass (streaming kernel)
+    into the batched tensor-core kernel (9..128 rows per launch: 32-, 64- and 128-row hidden boxes, a ragged last
+    tile, more tiles than CTAs, and n > 128 = two launches)."""
     shape = synth.Shape("r", layers=1, Hq=4, Hkv=2, d=64, H=H, V=V, fast_set=2)
     w = synth.make_w_vocab(shape, 5)
     hidden = synth.randn_bf16((n, H), synth.gen(6))
