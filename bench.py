@@ -218,33 +218,57 @@ class Workload:
 
 
 def run_device_timed(wl, steps, warmup, dist_ctx):
-    """K steps with inputs resident in HBM.  Per-step and per-call CUDA events on the launch stream."""
+    """K steps with inputs resident in HBM, timed with CUDA events on the launch stream.
+
+    Pass A (the reported `value`): the K steps back to back with one event before the first and one after the
+    last call -- nothing between the four calls of a step, so that each kernel's prologue may overlap its
+    predecessor's tail (programmatic dependent launch) exactly as in a caller's stream.  With an L2 flush between
+    steps (c1) the events bracket each step instead and the flushes stay outside.
+    Pass B (the per-kernel breakdown and the roofline): the same K steps again with an event between the calls;
+    a kernel's duration is the mean over those K launches."""
     flush = torch.empty(2 * L2_BYTES, dtype=torch.uint8, device=wl.dev) if wl.spec["flush_l2"] else None
     for i in range(warmup):
         wl.step(i)
     torch.cuda.synchronize()
-    evs = [[torch.cuda.Event(enable_timing=True) for _ in range(5)] for _ in range(steps)]
     launches0 = wl.ctx.launch_count()
     dist_ctx.barrier()
     torch.cuda.synchronize()
     t_wall0 = time.perf_counter()
     with ClockSampler(torch.cuda.current_device()) as clk:
-        for i in range(steps):
-            if flush is not None:
+        if flush is None:
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            for i in range(steps):
+                wl.step(warmup + i)
+            e1.record()
+            torch.cuda.synchronize()
+            total_ms = e0.elapsed_time(e1)
+            per_step = [total_ms / steps] * steps
+        else:
+            ev = [[torch.cuda.Event(enable_timing=True) for _ in range(2)] for _ in range(steps)]
+            for i in range(steps):
                 flush.fill_(i & 0xFF)  # evict L2 between timed iterations (outside the per-step events)
-            wl.step(warmup + i, evs[i])
-        torch.cuda.synchronize()
+                ev[i][0].record()
+                wl.step(warmup + i)
+                ev[i][1].record()
+            torch.cuda.synchronize()
+            per_step = [a.elapsed_time(b) for a, b in ev]
+            total_ms = sum(per_step)
     dist_ctx.barrier()
     wall = time.perf_counter() - t_wall0
     launches = wl.ctx.launch_count() - launches0
-    per_step = [e[0].elapsed_time(e[4]) for e in evs]
-    if flush is None:
-        total_ms = evs[0][0].elapsed_time(evs[-1][4])  # whole region incl. inter-step gaps
-    else:
-        total_ms = sum(per_step)
+    # pass B: per-call events
+    evs = [[torch.cuda.Event(enable_timing=True) for _ in range(5)] for _ in range(steps)]
+    with ClockSampler(torch.cuda.current_device()) as clk_b:
+        for i in range(steps):
+            if flush is not None:
+                flush.fill_(i & 0xFF)
+            wl.step(warmup + steps + i, evs[i])
+        torch.cuda.synchronize()
     calls = {name: statistics.fmean(e[a].elapsed_time(e[b]) for e in evs)
              for name, a, b in (("invalidate", 0, 1), ("entry_attn", 1, 2), ("ready_dist", 2, 3), ("gate_serve", 3, 4))}
-    return dict(total_ms=total_ms, per_step=per_step, calls=calls, launches=launches, wall_s=wall, clocks=clk.summary())
+    return dict(total_ms=total_ms, per_step=per_step, calls=calls, launches=launches, wall_s=wall, clocks=clk.summary(),
+                clocks_per_call_pass=clk_b.summary())
 
 
 def run_e2e(wl, steps, warmup, dist_ctx):
@@ -548,6 +572,7 @@ def main():
                                     "frac_of_8tbs_nominal": round(step_gbs / 8000.0, 4)},
             "kernels": kern,
             "clocks": res["clocks"],
+            "clocks_per_call_pass": res["clocks_per_call_pass"],
             "gpu_launches": res["launches"],
         }
         if e2e:

@@ -277,6 +277,10 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
     __syncthreads();
     ptx::tc_fence_after();
     const uint32_t tmem = *tmem_slot;
+    // everything above touched only this CTA's shared memory and TMEM; from here on the kernel reads what earlier
+    // kernels in the stream wrote (the plan, the pools, Q)
+    ptx::griddep_wait();
+    ptx::griddep_launch();
 
     const long long t0 = cta_begin(p.total_tiles, gridDim.x, blockIdx.x);
     const long long t1 = cta_begin(p.total_tiles, gridDim.x, blockIdx.x + 1);
@@ -935,8 +939,8 @@ int launch(prepos_ctx *ctx, const AttnArgs &a, int tiles_per_lh, cudaStream_t st
     p.counters = ctx->attn_counters;
     PREPOS_CUDA_TRY(cudaFuncSetAttribute(attn_umma_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                          static_cast<int>(smem)));
-    attn_umma_kernel<D><<<static_cast<int>(grid), kThreads, smem, stream>>>(ctx->tm_k, ctx->tm_v, ctx->tm_kn, ctx->tm_vn, ctx->tm_q, p);
-    PREPOS_CUDA_TRY(cudaGetLastError());
+    PREPOS_CUDA_TRY(prepos_launch_pdl(attn_umma_kernel<D>, dim3(static_cast<unsigned>(grid)), dim3(kThreads), smem, stream,
+                                      ctx->tm_k, ctx->tm_v, ctx->tm_kn, ctx->tm_vn, ctx->tm_q, p));
     ctx->launches += 1;
     return PREPOS_OK;
 }

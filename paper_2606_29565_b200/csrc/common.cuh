@@ -25,6 +25,28 @@ static_assert(sizeof(prepos_record) == 48, "prepos_record must be 48 bytes");
 void prepos_note_cuda_error(cudaError_t e, const char *what, const char *file, int line);
 void *prepos_get_encode_tiled();  // cuTensorMapEncodeTiled through the runtime's driver entry point (api.cu)
 
+// Every libprepos kernel is launched with programmatic stream serialization: its prologue (barrier init, TMEM
+// allocation, tensor-map prefetch, and -- for the LM head -- the first W_vocab stages, which no libprepos kernel
+// writes) may overlap the tail of the previous libprepos kernel in the stream; each kernel executes
+// griddepcontrol.wait before it touches anything a predecessor can have written.  After a kernel that never
+// triggers early (anything that is not ours) the launch behaves exactly like an ordinary one.
+template <typename... KArgs, typename... Args>
+inline cudaError_t prepos_launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t stream,
+                                     Args &&...args)
+{
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid;
+    cfg.blockDim = block;
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, kernel, static_cast<KArgs>(args)...);
+}
+
 constexpr int kMaxRdPartials = 1024;  // CTAs of a ready-dist launch (upper bound on its grid)
 constexpr int kRdMaxRows = 128;       // hidden rows reduced by one ready-dist launch
 constexpr int kAttnTileTokens = 128;  // KV tokens per tile of the tcgen05 attention kernel

@@ -2,6 +2,7 @@
 // PAPER.md:111) and invalidation (Sec. 3.6).  Both are a handful of bytes per
 // request: launch-latency bound, one thread per request.
 #include "common.cuh"
+#include "ptx.cuh"
 
 namespace {
 
@@ -15,6 +16,8 @@ __global__ void __launch_bounds__(128) gate_serve_kernel(int n, const int32_t *_
                                                          int strict_gt, int32_t *__restrict__ decision,
                                                          int32_t *__restrict__ token)
 {
+    ptx::griddep_wait();
+    ptx::griddep_launch();
     const int r = blockIdx.x * blockDim.x + threadIdx.x;
     if (r >= n) return;
     const int sid = session_ids[r];
@@ -51,6 +54,8 @@ __global__ void __launch_bounds__(128) invalidate_kernel(int n, const int32_t *_
                                                          unsigned long long *__restrict__ session_version,
                                                          prepos_record *__restrict__ records)
 {
+    ptx::griddep_wait();
+    ptx::griddep_launch();
     const int r = blockIdx.x * blockDim.x + threadIdx.x;
     if (r >= n) return;
     const int sid = session_ids[r];
@@ -68,9 +73,9 @@ int prepos_launch_gate_serve(prepos_ctx *ctx, int n, const int32_t *session_ids,
 {
     if (n == 0) return PREPOS_OK;
     const int threads = 128;
-    gate_serve_kernel<<<(n + threads - 1) / threads, threads, 0, stream>>>(
-        n, session_ids, req_hash, records, session_version, bitmap, ctx->shape.vocab, tau, strict_gt, decision, token);
-    PREPOS_CUDA_TRY(cudaGetLastError());
+    PREPOS_CUDA_TRY(prepos_launch_pdl(gate_serve_kernel, dim3((n + threads - 1) / threads), dim3(threads), 0, stream, n,
+                                      session_ids, req_hash, records, session_version, bitmap, ctx->shape.vocab, tau,
+                                      strict_gt, decision, token));
     ctx->launches += 1;
     return PREPOS_OK;
 }
@@ -80,9 +85,8 @@ int prepos_launch_invalidate(prepos_ctx *ctx, int n, const int32_t *session_ids,
 {
     if (n == 0) return PREPOS_OK;
     const int threads = 128;
-    invalidate_kernel<<<(n + threads - 1) / threads, threads, 0, stream>>>(
-        n, session_ids, reinterpret_cast<unsigned long long *>(session_version), records);
-    PREPOS_CUDA_TRY(cudaGetLastError());
+    PREPOS_CUDA_TRY(prepos_launch_pdl(invalidate_kernel, dim3((n + threads - 1) / threads), dim3(threads), 0, stream, n,
+                                      session_ids, reinterpret_cast<unsigned long long *>(session_version), records));
     ctx->launches += 1;
     return PREPOS_OK;
 }

@@ -62,6 +62,18 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)
     }
 }
 
+// Programmatic dependent launch: `griddep_wait` blocks until the kernels this launch depends on have completed and
+// their writes are visible (a no-op for a launch without the attribute); `griddep_launch` lets the next kernel in
+// the stream start its own prologue while this one is still running.
+__device__ __forceinline__ void griddep_wait()
+{
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+}
+__device__ __forceinline__ void griddep_launch()
+{
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+}
+
 // release / acquire at GPU scope (lighter than __threadfence(), which is sequentially consistent)
 __device__ __forceinline__ void fence_acq_rel_gpu()
 {

@@ -230,20 +230,12 @@ ready_dist_kernel(const __grid_constant__ CUtensorMap tm_w, const RdParams p)
         }
         ptx::fence_mbar_init();
     }
-    // hidden rows -> smem (row x_rows-1 is zero when n < 8; lanes of absent rows read it)
-    {
-        const int chunks_per_row = p.H / 8;
-        for (int idx = threadIdx.x; idx < p.x_rows * chunks_per_row; idx += kThreads) {
-            const int r = idx / chunks_per_row, c = idx - r * chunks_per_row;
-            uint4 v = make_uint4(0, 0, 0, 0);
-            if (r < p.n) v = *reinterpret_cast<const uint4 *>(p.hidden + static_cast<size_t>(r) * p.H + c * 8);
-            *reinterpret_cast<uint4 *>(xs + static_cast<size_t>(r) * x_stride + c * 8) = v;
-        }
-    }
     __syncthreads();
+    ptx::griddep_launch();
 
     if (warp == kConsumerWarps) {
-        // ===== TMA producer =====
+        // ===== TMA producer =====  W_vocab is never written by a libprepos kernel: its first stages are fetched
+        // while the previous kernel in the stream (the entry attention) is still draining
         if (lane == 0) {
             ptx::prefetch_tmap(&tm_w);
             const uint64_t pol = ptx::policy_evict_first();  // W is read once per pass
@@ -264,8 +256,22 @@ ready_dist_kernel(const __grid_constant__ CUtensorMap tm_w, const RdParams p)
                 }
             }
         }
+        ptx::griddep_wait();  // the cross-CTA pass below reads and writes what earlier kernels own
     } else {
         // ===== consumers: 16 vocabulary rows per warp =====
+        // hidden rows -> smem (row x_rows-1 is zero when n < 8; lanes of absent rows read it): the first access
+        // to memory an earlier kernel may have written
+        ptx::griddep_wait();
+        {
+            const int chunks_per_row = p.H / 8;
+            for (int idx = threadIdx.x; idx < p.x_rows * chunks_per_row; idx += kConsumerWarps * 32) {
+                const int r = idx / chunks_per_row, c = idx - r * chunks_per_row;
+                uint4 v = make_uint4(0, 0, 0, 0);
+                if (r < p.n) v = *reinterpret_cast<const uint4 *>(p.hidden + static_cast<size_t>(r) * p.H + c * 8);
+                *reinterpret_cast<uint4 *>(xs + static_cast<size_t>(r) * x_stride + c * 8) = v;
+            }
+        }
+        ptx::bar_sync(1, kConsumerWarps * 32);
         Top2Lse st[2];
         st[0] = t2_init();
         st[1] = t2_init();
@@ -407,6 +413,8 @@ ready_dist_batch_kernel(const __grid_constant__ CUtensorMap tm_w, const __grid_c
     __syncthreads();
     ptx::tc_fence_after();
     const uint32_t tmem = *tmem_slot;
+    ptx::griddep_wait();  // the hidden rows ride in every stage: nothing useful to fetch before the predecessor ends
+    ptx::griddep_launch();
 
     if (warp == 0) {
         // ===== TMA producer: W stage (two 64-column boxes) + the matching columns of the hidden rows =====
@@ -638,8 +646,7 @@ int prepos_launch_ready_dist(prepos_ctx *ctx, int n, const int32_t *session_ids,
             const size_t smem = fixed + static_cast<size_t>(stages) * stage_bytes;
             PREPOS_CUDA_TRY(cudaFuncSetAttribute(ready_dist_batch_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                                  static_cast<int>(smem)));
-            ready_dist_batch_kernel<<<grid, kBThreads, smem, stream>>>(tm, tmx, p);
-            PREPOS_CUDA_TRY(cudaGetLastError());
+            PREPOS_CUDA_TRY(prepos_launch_pdl(ready_dist_batch_kernel, dim3(grid), dim3(kBThreads), smem, stream, tm, tmx, p));
             ctx->launches += 1;
         }
         return PREPOS_OK;
@@ -669,8 +676,7 @@ int prepos_launch_ready_dist(prepos_ctx *ctx, int n, const int32_t *session_ids,
         const size_t smem = fixed + static_cast<size_t>(stages) * kStageBytes;
         PREPOS_CUDA_TRY(cudaFuncSetAttribute(ready_dist_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                              static_cast<int>(smem)));
-        ready_dist_kernel<<<grid, kThreads, smem, stream>>>(tm, p);
-        PREPOS_CUDA_TRY(cudaGetLastError());
+        PREPOS_CUDA_TRY(prepos_launch_pdl(ready_dist_kernel, dim3(grid), dim3(kThreads), smem, stream, tm, p));
         ctx->launches += 1;
     }
     return PREPOS_OK;
