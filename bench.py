@@ -90,6 +90,18 @@ def attention_flops(spec):
     return f * s.layers
 
 
+# DRAM bytes (dram__bytes_read.sum + dram__bytes_write.sum) of ONE launch of the dominant kernel, from the committed
+# `ncu --set full` captures (profiles/r01_ncu_full_final.md); None where no capture of that workload exists.
+NCU_TRAFFIC = {
+    ("c2", "entry_attn"): 546406000 + 9566208,
+    ("c2", "ready_dist"): 1050731000 + 3184640,
+    ("c3", "ready_dist"): 1050731000 + 3184640,   # same launch (V, H) as c2
+    ("c4", "entry_attn"): 71075419000 + 1655495000,
+    ("c4", "ready_dist"): 1051255000 + 3249000,
+    ("c5", "entry_attn"): 5424826000 + 54921984,
+}
+
+
 def peaks():
     p = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(p):
@@ -551,10 +563,22 @@ def main():
         kern["invalidate"] = {"ms": round(calls["invalidate"], 5)}
         kern["gate_serve"] = {"ms": round(calls["gate_serve"], 5), "requests": spec["serves"]}
         dom = max(("entry_attn", "ready_dist"), key=lambda k: calls[k])
-        roofline = {"kernel": "attn_umma_kernel" if dom == "entry_attn" else "ready_dist_kernel", "bound": "hbm",
-                    "achieved": kern[dom]["achieved_gbs"], "peak": pk["hbm"], "unit": "GB/s",
-                    "frac": kern[dom]["frac_of_measured_hbm"], "traffic": None, "peak_source": pk["source"],
-                    "share_of_step": round(calls[dom] / sum(calls.values()), 4)}
+        s_ = spec["shape"]
+        intensity = fl / max(1, ab["entry_attn"])   # flop per algorithmic byte of the attention call
+        ridge = pk["bf16"] * 1e12 / (pk["hbm"] * 1e9)
+        kname = "attn_umma_kernel" if dom == "entry_attn" else (
+            "ready_dist_batch_kernel" if n_sess > 8 else "ready_dist_kernel")
+        if dom == "entry_attn" and intensity >= 0.9 * ridge:
+            # G * L_entry at or above the ridge: the attention is a tensor-bound dense contraction;
+            # the kernel is timed alone between events: burst peak
+            roofline = {"kernel": kname, "bound": "tensor", "achieved": kern[dom]["tflops"], "peak": pk["bf16"],
+                        "unit": "TFLOP/s", "frac": kern[dom]["frac_of_measured_bf16"]}
+        else:
+            roofline = {"kernel": kname, "bound": "hbm", "achieved": kern[dom]["achieved_gbs"], "peak": pk["hbm"],
+                        "unit": "GB/s", "frac": kern[dom]["frac_of_measured_hbm"]}
+        roofline.update({"traffic": NCU_TRAFFIC.get((args.config, dom)), "algorithmic_bytes": ab[dom],
+                         "flop_per_byte": round(intensity, 1) if dom == "entry_attn" else round(2.0 * n_sess, 1),
+                         "peak_source": pk["source"], "share_of_step": round(calls[dom] / sum(calls.values()), 4)})
         step_bytes = ab["entry_attn"] + ab["ready_dist"]
         step_gbs = step_bytes / (ms_per_step * 1e-3) / 1e9
         line = {
