@@ -207,3 +207,57 @@ def test_config4_like_batch_sampled(prepos, oracle, path):
                 worst = max(worst, float(np.abs(got - o).max()))
     assert worst <= ATTN_ATOL, worst
     _check_append(sb, kp, vp, before, status, range(2))
+
+
+def _full_size_spec(name):
+    seed = synth.SEED_BASE + int(name[1])
+    if name == "c2":
+        return synth.C2, [4096], [24], seed
+    if name == "c3":
+        return synth.C3, [32768], [16], seed
+    if name == "c4":
+        return synth.C4, synth.lognormal_ns(64, seed), synth.uniform_l(64, seed), seed
+    return synth.C5, [16384], [32], seed
+
+
+@pytest.mark.parametrize("name", ["c2", "c3", "c4", "c5"])
+def test_full_size_configs_sampled(prepos, oracle, name):
+    """BASELINE configs 2-5 at FULL size in the launch configuration bench.py times (default path, every layer
+    in one launch, inputs generated on the device with bench.py's seeds): sampled (layer, session, head, entry
+    row) outputs against the oracle, which computes each sampled row from the same bits, plus the Append(E)
+    post-condition on the sampled (layer, session) pairs."""
+    shape, n_s, l_e, seed = _full_size_spec(name)
+    sb = synth.make_sessions(shape, n_s, l_e, seed=seed, device="cuda")
+    n = len(n_s)
+    ctx = prepos.Context(shape.layers, shape.Hq, shape.Hkv, shape.d, shape.H, shape.V, shape.page, max_sessions=n)
+    out = torch.full(sb.q.shape, float("nan"), dtype=torch.bfloat16, device="cuda")
+    status = ctx.entry_attn(sb.q, sb.k_new, sb.v_new, sb.k_pool, sb.v_pool, sb.page_table, sb.n_s, sb.l_entry,
+                            sb.capacity, out)
+    ctx.sync()
+    assert status == [0] * n
+    assert torch.isfinite(out.float()).all()
+    rng = np.random.default_rng(seed)
+    sessions = list(range(n)) if n <= 8 else sorted(set(int(x) for x in rng.choice(n, 8, replace=False)) |
+                                                     {int(np.argmax(n_s)), int(np.argmax(l_e))})
+    worst = 0.0
+    for s in sessions:
+        # a single session: first, last and one random layer; a batch: one random layer per sampled session
+        layers = sorted({0, shape.layers - 1, int(rng.integers(0, shape.layers))}) if n == 1 else [
+            int(rng.integers(0, shape.layers))]
+        for l in layers:
+            L = l_e[s]
+            picks = [(int(rng.integers(0, shape.Hq)), int(rng.integers(0, L))) for _ in range(2)]
+            picks += [(shape.Hq - 1, L - 1), (0, 0)]
+            ref = oracle_attn_rows(oracle, sb, l, s, picks)
+            for (h, i), o in ref.items():
+                got = out[l, sb.row_offset[s] + i, h].cpu().to(torch.float64).numpy()
+                worst = max(worst, float(np.abs(got - o).max()))
+            # Append(E): the session's new cache positions hold K_new / V_new bit for bit
+            pt = sb.page_table[s].cpu()
+            for jp in (0, L // 2, L - 1):
+                j = n_s[s] + jp
+                pg, sl = int(pt[j // shape.page]), j % shape.page
+                r = sb.row_offset[s] + jp
+                assert torch.equal(sb.k_pool[l, pg, :, sl].view(torch.int16), sb.k_new[l, r].view(torch.int16))
+                assert torch.equal(sb.v_pool[l, pg, :, sl].view(torch.int16), sb.v_new[l, r].view(torch.int16))
+    assert worst <= ATTN_ATOL, worst
