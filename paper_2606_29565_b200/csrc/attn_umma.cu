@@ -140,20 +140,8 @@ __device__ __forceinline__ int cta_of(long long total, int grid, long long t)
     return static_cast<int>(((t + 1) * grid + total - 1) / total) - 1;
 }
 
-// 64-bit UMMA shared-memory descriptor, SWIZZLE_128B, version 1 (sm_100)
-__device__ __forceinline__ uint64_t make_desc(uint32_t saddr, uint32_t lbo_bytes, uint32_t sbo_bytes)
-{
-    uint64_t d = 0;
-    d |= static_cast<uint64_t>((saddr >> 4) & 0x3fff);
-    d |= static_cast<uint64_t>((lbo_bytes >> 4) & 0x3fff) << 16;
-    d |= static_cast<uint64_t>((sbo_bytes >> 4) & 0x3fff) << 32;
-    d |= 1ull << 46;  // descriptor version
-    d |= 2ull << 61;  // SWIZZLE_128B
-    return d;
-}
-
-// the same descriptor as two words: low = start address and leading byte offset, high = stride byte offset,
-// version and swizzle (the high word is one constant per tile layout)
+// 64-bit UMMA shared-memory descriptor, SWIZZLE_128B, version 1 (sm_100), as two words: low = start address and
+// leading byte offset, high = stride byte offset, version and swizzle (the high word is one constant per tile layout)
 __device__ __forceinline__ uint32_t desc_lo(uint32_t saddr, uint32_t lbo_bytes)
 {
     return ((saddr >> 4) & 0x3fffu) | (((lbo_bytes >> 4) & 0x3fffu) << 16);
@@ -281,6 +269,10 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
     // kernels in the stream wrote (the plan, the pools, Q)
     ptx::griddep_wait();
     ptx::griddep_launch();
+#ifdef PREPOS_CTA_TIMES
+    long long dbg_t0 = 0;
+    if (threadIdx.x == 0) asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(dbg_t0));
+#endif
 
     const long long t0 = cta_begin(p.total_tiles, gridDim.x, blockIdx.x);
     const long long t1 = cta_begin(p.total_tiles, gridDim.x, blockIdx.x + 1);
@@ -741,39 +733,65 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
                     constexpr size_t kSlotFloats = static_cast<size_t>(kAttnMaxRows) * (D + 2);
                     const float *base0 = p.partials + (2 * static_cast<size_t>(c0) + c0_slot) * kSlotFloats;
                     const int nc = c1 - c0 + 1;
-                    for (int idx = st; idx < rows * kVec; idx += 256) {
+                    constexpr int kU = 4;  // rows x float4 columns per thread and pass: kU * 2 * nc loads in flight
+                    const int total = rows * kVec;
+                    auto store_row = [&](int idx, const float4 &acc, float wsum) {
                         const int r = idx / kVec, v = idx - r * kVec;
-                        float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
-                        float wsum = 0.f;
-                        if (nc <= kMaxC) {
-                            float lse[kMaxC];
-                            float4 o[kMaxC];
+                        const float inv = 1.f / wsum;
+                        const int tok = s.u.tok0 + r / G, h = s.kvh * G + r % G;
+                        uint2 pk;
+                        pk.x = pack_bf16(acc.x * inv, acc.y * inv);
+                        pk.y = pack_bf16(acc.z * inv, acc.w * inv);
+                        *reinterpret_cast<uint2 *>(ob + (static_cast<size_t>(s.u.row0 + tok) * p.Hq + h) * D + v * 4) = pk;
+                    };
+                    if (nc <= kMaxC) {
+                        for (int idx0 = st; idx0 < total; idx0 += 256 * kU) {
+                            float lse[kU][kMaxC];
+                            float4 o[kU][kMaxC];
 #pragma unroll
-                            for (int j = 0; j < kMaxC; ++j) {
-                                const float *sl = (j == 0) ? base0 : p.partials + 2 * static_cast<size_t>(c0 + j) * kSlotFloats;
-                                lse[j] = -CUDART_INF_F;
-                                o[j] = make_float4(0.f, 0.f, 0.f, 0.f);
-                                if (j < nc) {
-                                    lse[j] = __ldcg(sl + kAttnMaxRows * D + r);
-                                    o[j] = __ldcg(reinterpret_cast<const float4 *>(sl + static_cast<size_t>(r) * D) + v);
+                            for (int u = 0; u < kU; ++u) {
+                                const int idx = idx0 + u * 256;
+                                const int r = idx / kVec, v = idx - r * kVec;
+#pragma unroll
+                                for (int j = 0; j < kMaxC; ++j) {
+                                    const float *sl = (j == 0) ? base0 : p.partials + 2 * static_cast<size_t>(c0 + j) * kSlotFloats;
+                                    lse[u][j] = -CUDART_INF_F;
+                                    o[u][j] = make_float4(0.f, 0.f, 0.f, 0.f);
+                                    if (j < nc && idx < total) {
+                                        lse[u][j] = __ldcg(sl + kAttnMaxRows * D + r);
+                                        o[u][j] = __ldcg(reinterpret_cast<const float4 *>(sl + static_cast<size_t>(r) * D) + v);
+                                    }
                                 }
                             }
-                            float M = lse[0];
 #pragma unroll
-                            for (int j = 1; j < kMaxC; ++j) M = fmaxf(M, lse[j]);
+                            for (int u = 0; u < kU; ++u) {
+                                const int idx = idx0 + u * 256;
+                                if (idx >= total) continue;
+                                float M = lse[u][0];
 #pragma unroll
-                            for (int j = 0; j < kMaxC; ++j) {  // CTA order
-                                const float wgt = (j < nc) ? exp2f(lse[j] - M) : 0.f;
-                                acc.x = fmaf(wgt, o[j].x, acc.x);
-                                acc.y = fmaf(wgt, o[j].y, acc.y);
-                                acc.z = fmaf(wgt, o[j].z, acc.z);
-                                acc.w = fmaf(wgt, o[j].w, acc.w);
-                                wsum += wgt;
+                                for (int j = 1; j < kMaxC; ++j) M = fmaxf(M, lse[u][j]);
+                                float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
+                                float wsum = 0.f;
+#pragma unroll
+                                for (int j = 0; j < kMaxC; ++j) {  // CTA order
+                                    const float wgt = (j < nc) ? exp2f(lse[u][j] - M) : 0.f;
+                                    acc.x = fmaf(wgt, o[u][j].x, acc.x);
+                                    acc.y = fmaf(wgt, o[u][j].y, acc.y);
+                                    acc.z = fmaf(wgt, o[u][j].z, acc.z);
+                                    acc.w = fmaf(wgt, o[u][j].w, acc.w);
+                                    wsum += wgt;
+                                }
+                                store_row(idx, acc, wsum);
                             }
-                        } else {
+                        }
+                    } else {
+                        for (int idx = st; idx < total; idx += 256) {
+                            const int r = idx / kVec, v = idx - r * kVec;
                             float M = __ldcg(base0 + kAttnMaxRows * D + r);
                             for (int c = c0 + 1; c <= c1; ++c)
                                 M = fmaxf(M, __ldcg(p.partials + 2 * static_cast<size_t>(c) * kSlotFloats + kAttnMaxRows * D + r));
+                            float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
+                            float wsum = 0.f;
                             for (int c = c0; c <= c1; ++c) {
                                 const float *sl = (c == c0) ? base0 : p.partials + 2 * static_cast<size_t>(c) * kSlotFloats;
                                 const float wgt = exp2f(__ldcg(sl + kAttnMaxRows * D + r) - M);
@@ -784,13 +802,8 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
                                 acc.w = fmaf(wgt, o.w, acc.w);
                                 wsum += wgt;
                             }
+                            store_row(idx, acc, wsum);
                         }
-                        const float inv = 1.f / wsum;
-                        const int tok = s.u.tok0 + r / G, h = s.kvh * G + r % G;
-                        uint2 pk;
-                        pk.x = pack_bf16(acc.x * inv, acc.y * inv);
-                        pk.y = pack_bf16(acc.z * inv, acc.w * inv);
-                        *reinterpret_cast<uint2 *>(ob + (static_cast<size_t>(s.u.row0 + tok) * p.Hq + h) * D + v * 4) = pk;
                     }
                 }
                 ptx::bar_sync(1, 256);  // merge_info is reused by the next segment
@@ -801,6 +814,20 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
     ptx::tc_fence_before();
     __syncthreads();
     if (warp == 2) ptx::tmem_dealloc<512>(tmem);
+#ifdef PREPOS_CTA_TIMES
+    if (threadIdx.x == 0) {
+        long long dbg_t1;
+        asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(dbg_t1));
+        int nseg = 0, ncut = 0;
+        SegIter it(p, t0, t1);
+        Seg s;
+        while (it.next(p, s)) {
+            ++nseg;
+            ncut += !s.direct;
+        }
+        printf("CTA %d start %lld dur %lld tiles %lld nseg %d ncut %d\n", blockIdx.x, dbg_t0, dbg_t1 - dbg_t0, t1 - t0, nseg, ncut);
+    }
+#endif
 }
 
 typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
