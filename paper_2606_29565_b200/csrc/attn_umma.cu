@@ -744,16 +744,20 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
                         pk.y = pack_bf16(acc.z * inv, acc.w * inv);
                         *reinterpret_cast<uint2 *>(ob + (static_cast<size_t>(s.u.row0 + tok) * p.Hq + h) * D + v * 4) = pk;
                     };
-                    if (nc <= kMaxC) {
-                        for (int idx0 = st; idx0 < total; idx0 += 256 * kU) {
-                            float lse[kU][kMaxC];
-                            float4 o[kU][kMaxC];
+                    // all loads of a pass are issued before the first use: one L2 round trip (~2 us under a full HBM
+                    // stream) per pass.  Two partials (the common cut) take 12 rows per thread and pass, i.e. one pass
+                    // for up to 96 rows; up to four partials take 4.
+                    auto merge_pass = [&](auto ku_tag, auto kc_tag) {
+                        constexpr int kU_ = decltype(ku_tag)::value, kC_ = decltype(kc_tag)::value;
+                        for (int idx0 = st; idx0 < total; idx0 += 256 * kU_) {
+                            float lse[kU_][kC_];
+                            float4 o[kU_][kC_];
 #pragma unroll
-                            for (int u = 0; u < kU; ++u) {
+                            for (int u = 0; u < kU_; ++u) {
                                 const int idx = idx0 + u * 256;
                                 const int r = idx / kVec, v = idx - r * kVec;
 #pragma unroll
-                                for (int j = 0; j < kMaxC; ++j) {
+                                for (int j = 0; j < kC_; ++j) {
                                     const float *sl = (j == 0) ? base0 : p.partials + 2 * static_cast<size_t>(c0 + j) * kSlotFloats;
                                     lse[u][j] = -CUDART_INF_F;
                                     o[u][j] = make_float4(0.f, 0.f, 0.f, 0.f);
@@ -764,16 +768,16 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
                                 }
                             }
 #pragma unroll
-                            for (int u = 0; u < kU; ++u) {
+                            for (int u = 0; u < kU_; ++u) {
                                 const int idx = idx0 + u * 256;
                                 if (idx >= total) continue;
                                 float M = lse[u][0];
 #pragma unroll
-                                for (int j = 1; j < kMaxC; ++j) M = fmaxf(M, lse[u][j]);
+                                for (int j = 1; j < kC_; ++j) M = fmaxf(M, lse[u][j]);
                                 float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
                                 float wsum = 0.f;
 #pragma unroll
-                                for (int j = 0; j < kMaxC; ++j) {  // CTA order
+                                for (int j = 0; j < kC_; ++j) {  // CTA order
                                     const float wgt = (j < nc) ? exp2f(lse[u][j] - M) : 0.f;
                                     acc.x = fmaf(wgt, o[u][j].x, acc.x);
                                     acc.y = fmaf(wgt, o[u][j].y, acc.y);
@@ -784,6 +788,11 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
                                 store_row(idx, acc, wsum);
                             }
                         }
+                    };
+                    if (nc <= 2) {
+                        merge_pass(std::integral_constant<int, 12>{}, std::integral_constant<int, 2>{});
+                    } else if (nc <= kMaxC) {
+                        merge_pass(std::integral_constant<int, kU>{}, std::integral_constant<int, kMaxC>{});
                     } else {
                         for (int idx = st; idx < total; idx += 256) {
                             const int r = idx / kVec, v = idx - r * kVec;
