@@ -371,6 +371,35 @@ def run_gate_serve(wl, prepos, reps=200):
     return res
 
 
+def run_fall_through(wl, reps=20):
+    """SURVEY.md 8(f) NEXT-1, the step after a gate miss (Eq. 5): prepos_entry_attn with a delta of
+    8 tokens, and with the single decode token, over the same cached sessions (all layers, one launch each).
+    G * L is 32 / 4 rows per KV head here: the streaming-HBM regime of the same kernel."""
+    res = {}
+    ab = algorithmic_bytes(wl.spec)
+    s = wl.spec["shape"]
+    kv_bytes = sum(wl.spec["n_s"]) * s.layers * s.Hkv * s.d * 2 * 2
+    for L in (8, 1):
+        if min(wl.spec["l_entry"]) < L or wl.n != 1:
+            continue
+        l_h = [L] * wl.n
+        ev = []
+        for i in range(reps + 3):
+            st = wl.sets[i % len(wl.sets)]
+            sb = st["sb"]
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            wl.ctx.entry_attn(sb.q[:, :L], sb.k_new[:, :L], sb.v_new[:, :L], sb.k_pool, sb.v_pool, sb.page_table,
+                              wl.n_s_h, l_h, wl.cap_h, st["out"][:, :L])
+            e1.record()
+            ev.append((e0, e1))
+        torch.cuda.synchronize()
+        ms = statistics.fmean(a.elapsed_time(b) for a, b in ev[3:])
+        res[f"L{L}"] = {"attn_ms": round(ms, 5), "kv_gbs": round(kv_bytes / (ms * 1e-3) / 1e9, 1),
+                        "frac_of_measured_hbm": round(kv_bytes / (ms * 1e-3) / 1e9 / peaks()["hbm"], 4)}
+    return res
+
+
 # ----------------------------------------------------------------------------------------------------
 # the CPU oracle, timed on a bounded sample (cpu_baseline leg and --impl reference)
 # ----------------------------------------------------------------------------------------------------
@@ -602,6 +631,9 @@ def main():
         if e2e:
             line["e2e"] = e2e
         line["gate_serve"] = run_gate_serve(wl, prepos)
+        ft = run_fall_through(wl)
+        if ft:
+            line["fall_through"] = ft
         if not args.no_cpu_baseline:
             osmp = OracleSample(spec)
             units, rows = osmp.plan(15.0)

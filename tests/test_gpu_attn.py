@@ -261,3 +261,59 @@ def test_full_size_configs_sampled(prepos, oracle, name):
                 assert torch.equal(sb.k_pool[l, pg, :, sl].view(torch.int16), sb.k_new[l, r].view(torch.int16))
                 assert torch.equal(sb.v_pool[l, pg, :, sl].view(torch.int16), sb.v_new[l, r].view(torch.int16))
     assert worst <= ATTN_ATOL, worst
+
+
+def test_fall_through_delta_resume_full_size(prepos, oracle):
+    """The fall-through path after a gate miss (Eq. 5; Alg. 2 l.8-9) on BASELINE
+    config 2 at full size: pre-position L = 24 entry tokens, then resume with a delta of 8 tokens on top of the
+    pre-positioned cache (n_s' = n_s + 24), then one decode step (L = 1, n_s'' = n_s + 32).  Each call's sampled
+    rows against the oracle (which reads the cache the previous calls appended to), and two-step consistency at
+    scale: rows of the first two calls == one call with all 32 tokens over the original cache."""
+    from dataclasses import replace
+    shape, seed = synth.C2, synth.SEED_BASE + 1
+    n_s0, L1, L2 = 4096, 24, 8
+    sb = synth.make_sessions(shape, [n_s0], [L1 + L2], seed=seed, device="cuda", extra_pages=1)
+    k0, v0 = sb.k_pool.clone(), sb.v_pool.clone()
+    ctx = prepos.Context(shape.layers, shape.Hq, shape.Hkv, shape.d, shape.H, shape.V, shape.page, max_sessions=1)
+
+    def run(view, pools):
+        out = torch.full(view.q.shape, float("nan"), dtype=torch.bfloat16, device="cuda")
+        st = ctx.entry_attn(view.q, view.k_new, view.v_new, pools[0], pools[1], view.page_table, view.n_s,
+                            view.l_entry, view.capacity, out)
+        ctx.sync()
+        assert st == [0]
+        return out
+
+    def sample(view, out, rng, layers):
+        worst = 0.0
+        L = view.l_entry[0]
+        for l in layers:
+            picks = [(int(rng.integers(0, shape.Hq)), int(rng.integers(0, L))) for _ in range(2)] + [(shape.Hq - 1, L - 1)]
+            for (h, i), o in oracle_attn_rows(oracle, view, l, 0, picks).items():
+                worst = max(worst, float(np.abs(out[l, i, h].cpu().to(torch.float64).numpy() - o).max()))
+        return worst
+
+    rng = np.random.default_rng(seed)
+    layers = [0, int(rng.integers(1, shape.layers - 1)), shape.layers - 1]
+    # one call with all 32 tokens over the original cache (on copies of the pools)
+    joint = run(sb, (k0, v0))
+    # call 1: the pre-position
+    v1 = replace(sb, l_entry=[L1], q=sb.q[:, :L1], k_new=sb.k_new[:, :L1], v_new=sb.v_new[:, :L1])
+    o1 = run(v1, (sb.k_pool, sb.v_pool))
+    assert sample(v1, o1, rng, layers) <= ATTN_ATOL
+    # call 2: the delta on top of the pre-positioned entry
+    v2 = replace(sb, n_s=[n_s0 + L1], l_entry=[L2], q=sb.q[:, L1:], k_new=sb.k_new[:, L1:], v_new=sb.v_new[:, L1:])
+    o2 = run(v2, (sb.k_pool, sb.v_pool))
+    assert sample(v2, o2, rng, layers) <= ATTN_ATOL
+    # two-step consistency: same rows as the joint call, and the same cache contents afterwards
+    both = torch.cat([o1, o2], dim=1).float()
+    assert float((both - joint.float()).abs().max()) <= 2 * ATTN_ATOL
+    assert torch.equal(sb.k_pool.view(torch.int16), k0.view(torch.int16))
+    assert torch.equal(sb.v_pool.view(torch.int16), v0.view(torch.int16))
+    # call 3: one decode step over everything appended so far
+    g = synth.gen(seed + 999, "cuda")
+    v3 = replace(sb, n_s=[n_s0 + L1 + L2], l_entry=[1], q=synth.randn_bf16((shape.layers, 1, shape.Hq, shape.d), g),
+                 k_new=synth.randn_bf16((shape.layers, 1, shape.Hkv, shape.d), g),
+                 v_new=synth.randn_bf16((shape.layers, 1, shape.Hkv, shape.d), g))
+    o3 = run(v3, (sb.k_pool, sb.v_pool))
+    assert sample(v3, o3, rng, layers) <= ATTN_ATOL
