@@ -10,6 +10,7 @@ marshals arrays, and loops the single-session / single-layer C calls over sessio
 from __future__ import annotations
 
 import ctypes as C
+import math
 import os
 import subprocess
 from dataclasses import dataclass
@@ -186,3 +187,60 @@ class SessionTable:
             return gate(0.0, -1, False, 0, 0, int(self.version[sid]), 0, request_hash, bitmap, V, tau, strict_gt)
         return gate(r.gap, r.top1, bool(self.rec_valid[sid]), r.nonfinite, int(self.rec_version[sid]),
                     int(self.version[sid]), int(self.rec_hash[sid]), request_hash, bitmap, V, tau, strict_gt)
+
+
+# ---- O6: risk-coverage sweep of the gate (Sec. 2.4) -------------------
+# Plain definitions in fp64; pinned in tests/test_oracle_calibration.py by the counts and intervals the paper prints
+# for its own calibration run (121 of 128 served at tau = 2.0, 16 false accepts).
+Z95 = 1.959963984540054  # two-sided 95% normal quantile
+
+
+def wilson(k: int, n: int, z: float = Z95):
+    """Wilson score interval of k successes in n trials (the paper's "Wilson 95% interval").
+    (0, 1) for n = 0."""
+    if n <= 0:
+        return 0.0, 1.0
+    p = k / n
+    den = 1.0 + z * z / n
+    centre = (p + z * z / (2.0 * n)) / den
+    half = z * math.sqrt(p * (1.0 - p) / n + z * z / (4.0 * n * n)) / den
+    return centre - half, centre + half
+
+
+@dataclass
+class SweepPoint:
+    tau: float
+    accepted: int        # requests the gate accepts: gamma > tau (or >=) and argmax in A       (Eq. 13 numerator)
+    false_accepts: int   # accepted whose served token differs from the full-path token          (Eq. 14 numerator)
+    coverage: float      # c(tau) = accepted / n                                                 (Eq. 13)
+    far: float           # r(tau) = false_accepts / accepted, 0 when nothing is accepted         (Eq. 14)
+    cov_lo: float
+    cov_hi: float
+    far_lo: float
+    far_hi: float
+
+
+def risk_coverage(gap, servable, top1, full_path_token, taus, strict_gt=False):
+    """For each tau: Eq. 13 / Eq. 14 over n decision points.  gap[i], top1[i] from the ready-distribution record,
+    servable[i] = record valid, fresh and argmax in A (everything of Eq. 12 but the threshold), full_path_token[i]
+    the model's own full-path output.  A non-finite gap never accepts."""
+    gap = np.asarray(gap, dtype=np.float64)
+    servable = np.asarray(servable).astype(bool)
+    wrong = np.asarray(top1) != np.asarray(full_path_token)
+    n = int(gap.shape[0])
+    out = []
+    for tau in taus:
+        acc = servable & ((gap > tau) if strict_gt else (gap >= tau)) & np.isfinite(gap)
+        a = int(acc.sum())
+        f = int((acc & wrong).sum())
+        clo, chi = wilson(a, n)
+        flo, fhi = wilson(f, a)
+        out.append(SweepPoint(float(tau), a, f, a / n if n else 0.0, f / a if a else 0.0, clo, chi, flo, fhi))
+    return out
+
+
+def calibrate_tau(points, r_max: float):
+    """"selects the smallest tau such that r(tau) <= r_max" over the swept thresholds; None when no
+    swept threshold meets the budget."""
+    ok = [p.tau for p in points if p.far <= r_max]
+    return min(ok) if ok else None
