@@ -197,6 +197,32 @@ int prepos_gate_serve(prepos_ctx *ctx, int n_requests, const int32_t *session_id
 int prepos_invalidate(prepos_ctx *ctx, int n, const int32_t *session_ids,
                       uint64_t *session_version, prepos_record *records, void *stream);
 
+/*
+ * Risk-coverage sweep of the gate (Sec. 2.4, Eq. 13-14; the calibration measurement of
+ * PAPER.md:254): for each threshold taus[t], over the n decision points records[0..n):
+ *   accepted       = #{ i : records[i] VALID, finite, fresh (version == session_version[i]), top1 in A,
+ *                        gap >= tau (strict_gt: gap > tau) }                       -- the numerator of c(tau), Eq. 13
+ *   false_accepts  = #{ accepted i : records[i].top1 != full_path_token[i] }       -- the numerator of r(tau), Eq. 14
+ *   coverage = accepted / n, far = false_accepts / accepted (0 when nothing is accepted), and the Wilson 95%
+ *   score intervals of both ((0, 1) for an empty denominator), all in fp64.
+ * "Calibration selects the smallest tau such that r(tau) <= r_max" is one pass of the caller over
+ * out[].  records, session_version, fast_set_bitmap, full_path_token [n] int32, taus [n_tau] float and
+ * out [n_tau] are DEVICE pointers; out is fully overwritten.  One CTA per threshold.
+ */
+typedef struct {
+    float tau;
+    int32_t n;
+    int32_t accepted;
+    int32_t false_accepts;
+    double coverage, far;
+    double cov_lo, cov_hi;
+    double far_lo, far_hi;
+} prepos_sweep_point; /* 64 bytes */
+
+int prepos_gate_sweep(prepos_ctx *ctx, int n, const prepos_record *records, const uint64_t *session_version,
+                      const uint32_t *fast_set_bitmap, const int32_t *full_path_token, int n_tau,
+                      const float *taus, int strict_gt, prepos_sweep_point *out, void *stream);
+
 /* HOST helper: A as a bitmap.  ids HOST int32 [n]; bitmap_host HOST uint32 [ceil(V/32)] (overwritten). */
 int prepos_fastset_build(const int32_t *ids, int n, int V, uint32_t *bitmap_host);
 

@@ -358,6 +358,19 @@ int prepos_invalidate(prepos_ctx *ctx, int n, const int32_t *session_ids, uint64
     return prepos_launch_invalidate(ctx, n, session_ids, session_version, records, static_cast<cudaStream_t>(stream));
 }
 
+int prepos_gate_sweep(prepos_ctx *ctx, int n, const prepos_record *records, const uint64_t *session_version,
+                      const uint32_t *fast_set_bitmap, const int32_t *full_path_token, int n_tau, const float *taus,
+                      int strict_gt, prepos_sweep_point *out, void *stream)
+{
+    if (!ctx || n < 0 || n_tau < 0) return PREPOS_E_INVALID_ARG;
+    if (n_tau == 0) return PREPOS_OK;
+    if (!taus || !out || (n > 0 && (!records || !session_version || !fast_set_bitmap || !full_path_token)))
+        return PREPOS_E_INVALID_ARG;
+    if (!aligned16(records) || (reinterpret_cast<uintptr_t>(out) & 7)) return PREPOS_E_ALIGN;
+    return prepos_launch_gate_sweep(ctx, n, records, session_version, fast_set_bitmap, full_path_token, n_tau, taus,
+                                    strict_gt, out, static_cast<cudaStream_t>(stream));
+}
+
 int prepos_fastset_build(const int32_t *ids, int n, int V, uint32_t *bitmap_host)
 {
     if (!bitmap_host || V <= 0 || n < 0 || (n > 0 && !ids)) return PREPOS_E_INVALID_ARG;

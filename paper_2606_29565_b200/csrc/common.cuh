@@ -129,6 +129,9 @@ int prepos_launch_gate_serve(prepos_ctx *ctx, int n, const int32_t *session_ids,
                              const prepos_record *records, const uint64_t *session_version,
                              const uint32_t *bitmap, float tau, int strict_gt, int32_t *decision, int32_t *token,
                              cudaStream_t stream);
+int prepos_launch_gate_sweep(prepos_ctx *ctx, int n, const prepos_record *records, const uint64_t *session_version,
+                             const uint32_t *bitmap, const int32_t *full_path_token, int n_tau, const float *taus,
+                             int strict_gt, prepos_sweep_point *out, cudaStream_t stream);
 int prepos_launch_invalidate(prepos_ctx *ctx, int n, const int32_t *session_ids, uint64_t *session_version,
                              prepos_record *records, cudaStream_t stream);
 

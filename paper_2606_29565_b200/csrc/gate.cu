@@ -64,7 +64,92 @@ __global__ void __launch_bounds__(128) invalidate_kernel(int n, const int32_t *_
     atomicAdd(&session_version[sid], 1ull);
 }
 
+// Wilson score interval of k successes in n trials, fp64 (z = the two-sided 95% normal quantile)
+__device__ __forceinline__ void wilson95(int k, int n, double &lo, double &hi)
+{
+    if (n <= 0) {
+        lo = 0.0;
+        hi = 1.0;
+        return;
+    }
+    const double z = 1.959963984540054;
+    const double p = static_cast<double>(k) / n;
+    const double den = 1.0 + z * z / n;
+    const double centre = (p + z * z / (2.0 * n)) / den;
+    const double half = z * sqrt(p * (1.0 - p) / n + z * z / (4.0 * static_cast<double>(n) * n)) / den;
+    lo = centre - half;
+    hi = centre + half;
+}
+
+// Eq. 13-14 for one threshold per CTA: two integer counts over the n records, then the rates and intervals.
+__global__ void __launch_bounds__(256) gate_sweep_kernel(int n, const prepos_record *__restrict__ records,
+                                                         const uint64_t *__restrict__ session_version,
+                                                         const uint32_t *__restrict__ bitmap, int vocab,
+                                                         const int32_t *__restrict__ full_path_token,
+                                                         const float *__restrict__ taus, int strict_gt,
+                                                         prepos_sweep_point *__restrict__ out)
+{
+    ptx::griddep_wait();
+    ptx::griddep_launch();
+    const float tau = taus[blockIdx.x];
+    int acc = 0, bad = 0;
+    for (int i = threadIdx.x; i < n; i += blockDim.x) {
+        const uint4 *p = reinterpret_cast<const uint4 *>(records + i);
+        const uint4 w0 = p[0];  // max_logit, lse, top1, top2
+        const uint4 w1 = p[1];  // gap, flags, version
+        const int32_t top1 = static_cast<int32_t>(w0.z);
+        const float gap = __uint_as_float(w1.x);
+        const uint32_t flags = w1.y;
+        const uint64_t rec_version = (static_cast<uint64_t>(w1.w) << 32) | w1.z;
+        const bool servable = (flags & PREPOS_FLAG_VALID) && !(flags & PREPOS_FLAG_NONFINITE) &&
+                              rec_version == session_version[i] && top1 >= 0 && top1 < vocab &&
+                              ((bitmap[top1 >> 5] >> (top1 & 31)) & 1u);
+        const bool a = servable && (strict_gt ? (gap > tau) : (gap >= tau)) && (fabsf(gap) <= 3.0e38f);
+        acc += a;
+        bad += a && (top1 != full_path_token[i]);
+    }
+    __shared__ int s_acc[8], s_bad[8];
+#pragma unroll
+    for (int m = 16; m > 0; m >>= 1) {
+        acc += __shfl_xor_sync(0xffffffffu, acc, m);
+        bad += __shfl_xor_sync(0xffffffffu, bad, m);
+    }
+    if ((threadIdx.x & 31) == 0) {
+        s_acc[threadIdx.x >> 5] = acc;
+        s_bad[threadIdx.x >> 5] = bad;
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        int a = 0, f = 0;
+        for (int w = 0; w < static_cast<int>(blockDim.x >> 5); ++w) {
+            a += s_acc[w];
+            f += s_bad[w];
+        }
+        prepos_sweep_point r;
+        r.tau = tau;
+        r.n = n;
+        r.accepted = a;
+        r.false_accepts = f;
+        r.coverage = n > 0 ? static_cast<double>(a) / n : 0.0;
+        r.far = a > 0 ? static_cast<double>(f) / a : 0.0;
+        wilson95(a, n, r.cov_lo, r.cov_hi);
+        wilson95(f, a, r.far_lo, r.far_hi);
+        out[blockIdx.x] = r;
+    }
+}
+
 }  // namespace
+
+int prepos_launch_gate_sweep(prepos_ctx *ctx, int n, const prepos_record *records, const uint64_t *session_version,
+                             const uint32_t *bitmap, const int32_t *full_path_token, int n_tau, const float *taus,
+                             int strict_gt, prepos_sweep_point *out, cudaStream_t stream)
+{
+    if (n_tau == 0) return PREPOS_OK;
+    PREPOS_CUDA_TRY(prepos_launch_pdl(gate_sweep_kernel, dim3(n_tau), dim3(256), 0, stream, n, records, session_version,
+                                      bitmap, ctx->shape.vocab, full_path_token, taus, strict_gt, out));
+    ctx->launches += 1;
+    return PREPOS_OK;
+}
 
 int prepos_launch_gate_serve(prepos_ctx *ctx, int n, const int32_t *session_ids, const uint64_t *req_hash,
                              const prepos_record *records, const uint64_t *session_version,

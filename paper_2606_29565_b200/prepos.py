@@ -24,7 +24,8 @@ RECORD_BYTES = 48
 EXPORTS = [
     "prepos_strerror", "prepos_version", "prepos_workspace_bytes", "prepos_ctx_create", "prepos_ctx_destroy",
     "prepos_ctx_sync", "prepos_ctx_launch_count", "prepos_ctx_set_attn_path", "prepos_entry_attn",
-    "prepos_ready_dist", "prepos_scan_logits", "prepos_gate_serve", "prepos_invalidate", "prepos_fastset_build",
+    "prepos_ready_dist", "prepos_scan_logits", "prepos_gate_serve", "prepos_invalidate", "prepos_gate_sweep",
+    "prepos_fastset_build",
 ]
 
 
@@ -77,6 +78,8 @@ def lib() -> C.CDLL:
         L.prepos_gate_serve.argtypes = [vp, i32, vp, vp, vp, vp, vp, f32, i32, vp, vp, vp]
         L.prepos_invalidate.restype = i32
         L.prepos_invalidate.argtypes = [vp, i32, vp, vp, vp, vp]
+        L.prepos_gate_sweep.restype = i32
+        L.prepos_gate_sweep.argtypes = [vp, i32, vp, vp, vp, vp, i32, vp, i32, vp, vp]
         L.prepos_fastset_build.restype = i32
         L.prepos_fastset_build.argtypes = [vp, i32, i32, vp]
         _lib = L
@@ -133,6 +136,20 @@ def unpack_records(records: torch.Tensor) -> dict:
     return {"max_logit": f[:, 0].clone(), "lse": f[:, 1].clone(), "top1": i[:, 2].clone(), "top2": i[:, 3].clone(),
             "gap": f[:, 4].clone(), "flags": i[:, 5].clone(), "version": q[:, 3].clone(),
             "entry_hash": q[:, 4].clone(), "position": q[:, 5].clone()}
+
+
+SWEEP_POINT_BYTES = 64
+
+
+def unpack_sweep(points: torch.Tensor) -> dict:
+    """prepos_sweep_point table -> dict of host tensors (field views; no arithmetic)."""
+    r = points.detach().cpu().contiguous()
+    f = r.view(torch.float32).view(-1, 16)
+    i = r.view(torch.int32).view(-1, 16)
+    d = r.view(torch.float64).view(-1, 8)
+    return {"tau": f[:, 0].clone(), "n": i[:, 1].clone(), "accepted": i[:, 2].clone(), "false_accepts": i[:, 3].clone(),
+            "coverage": d[:, 2].clone(), "far": d[:, 3].clone(), "cov_lo": d[:, 4].clone(), "cov_hi": d[:, 5].clone(),
+            "far_lo": d[:, 6].clone(), "far_hi": d[:, 7].clone()}
 
 
 class Context:
@@ -221,6 +238,17 @@ class Context:
                                        _p(records), _p(session_version), _p(fast_set_bitmap), float(tau),
                                        int(bool(strict_gt)), _p(decision_out), _p(token_out), _stream()),
                "prepos_gate_serve")
+
+    def gate_sweep(self, records, session_version, fast_set_bitmap, full_path_token, taus, strict_gt=False):
+        """prepos_gate_sweep over all records: returns the [n_tau] device buffer of prepos_sweep_point (64 B each);
+        `unpack_sweep` turns it into host arrays."""
+        assert full_path_token.dtype == torch.int32 and taus.dtype == torch.float32 and taus.is_cuda
+        n = full_path_token.numel()
+        out = torch.zeros(taus.numel() * SWEEP_POINT_BYTES, dtype=torch.uint8, device=taus.device)
+        _check(lib().prepos_gate_sweep(self._h, n, _p(records), _p(session_version), _p(fast_set_bitmap),
+                                       _p(full_path_token), taus.numel(), _p(taus), int(bool(strict_gt)), _p(out),
+                                       _stream()), "prepos_gate_sweep")
+        return out
 
     def invalidate(self, session_ids, session_version, records):
         assert session_ids.dtype == torch.int32 and session_version.dtype == torch.int64

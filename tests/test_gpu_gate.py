@@ -145,3 +145,51 @@ def test_config3_trace_invalidate_never_serves_stale(prepos, oracle):
     ctx.sync()
     assert ver.cpu().tolist() == [1, sum(bumps) + 2]
     assert prepos.unpack_records(recs)["flags"].tolist() == [0, 0]
+
+
+def test_gate_sweep_matches_oracle_risk_coverage(prepos, oracle):
+    """prepos_gate_sweep (Eq. 13-14) on records the GPU produced itself: 512 sessions of the
+    tiny config with planted margins, a third of them invalidated, full-path tokens that disagree on some rows;
+    counts bit-exact against oracle O6 (fed with the GPU's own gap / top-1, so no fp decision differs), rates and
+    Wilson intervals to 1e-12, under both inequality modes, including gamma == tau and an empty sweep."""
+    shape, seed, n = synth.C1, synth.SEED_BASE + 40, 512
+    w = synth.make_w_vocab(shape, seed, "cuda")
+    fast = synth.make_fast_set(shape, seed)
+    hidden, _, _ = synth.make_hidden(shape, n, w, fast.cuda(), seed, planted_frac=0.8)
+    ctx = prepos.Context(shape.layers, shape.Hq, shape.Hkv, shape.d, shape.H, shape.V, shape.page, max_sessions=n)
+    sid = torch.arange(n, dtype=torch.int32, device="cuda")
+    recs = prepos.new_records(n)
+    ver = torch.zeros(n, dtype=torch.int64, device="cuda")
+    ctx.ready_dist(sid, hidden, w, recs, ver)
+    stale = torch.arange(0, n, 3, dtype=torch.int32, device="cuda")
+    ctx.invalidate(stale, ver, recs)                     # these records must never count as accepted
+    bm = prepos.fastset_build(fast, shape.V).cuda()
+    rec = prepos.unpack_records(recs)
+    g = synth.gen(seed + 1)
+    full = rec["top1"].clone().to(torch.int32)
+    flip = torch.rand(n, generator=g) < 0.15
+    full[flip] = (full[flip] + 1) % shape.V
+    gap = rec["gap"].numpy().astype(np.float64)
+    taus = [0.0, 1.0, 2.0, 3.0, float(rec["gap"][1]), 4.5, 6.0, 1e9]   # one threshold exactly on a record's gap
+    in_set = np.isin(rec["top1"].numpy(), fast.numpy())
+    servable = in_set & (np.arange(n) % 3 != 0)
+    for strict in (False, True):
+        out = ctx.gate_sweep(recs, ver, bm, full.cuda(), torch.tensor(taus, dtype=torch.float32, device="cuda"), strict)
+        ctx.sync()
+        got = prepos.unpack_sweep(out)
+        ref = oracle.risk_coverage(gap, servable, rec["top1"].numpy(), full.numpy(),
+                                   [float(np.float32(t)) for t in taus], strict)
+        for t, p in enumerate(ref):
+            assert (int(got["n"][t]), int(got["accepted"][t]), int(got["false_accepts"][t])) == (n, p.accepted, p.false_accepts)
+            for k in ("coverage", "far", "cov_lo", "cov_hi", "far_lo", "far_hi"):
+                assert abs(float(got[k][t]) - getattr(p, k)) <= 1e-12, (k, t)
+        assert int(got["accepted"][0]) > 0 and int(got["accepted"][-1]) == 0
+        srt = sorted(range(len(taus)), key=lambda t: taus[t])
+        assert all(int(got["accepted"][a]) >= int(got["accepted"][b]) for a, b in zip(srt, srt[1:]))   # Eq. 13 monotone
+    # decisions of prepos_gate_serve agree with the sweep's count at the same tau
+    dec = torch.zeros(n, dtype=torch.int32, device="cuda")
+    tok = torch.zeros(n, dtype=torch.int32, device="cuda")
+    ctx.gate_serve(sid, recs, ver, bm, 3.0, dec, tok)
+    out = ctx.gate_sweep(recs, ver, bm, full.cuda(), torch.tensor([3.0], dtype=torch.float32, device="cuda"))
+    ctx.sync()
+    assert int((dec == 0).sum()) == int(prepos.unpack_sweep(out)["accepted"][0])
