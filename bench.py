@@ -371,6 +371,65 @@ def run_gate_serve(wl, prepos, reps=200):
     return res
 
 
+def run_co_schedule(wl, prepos, n_serves=300):
+    """SURVEY.md 8(f) NEXT-2 (the pass runs in the idle window and "yields to any request"):
+    wall latency of one gate serve (launch on a high-priority stream + D2H of the decisions + sync) while the
+    low-priority stream is kept full of pre-position steps, beside the same serve on an idle GPU.  The persistent
+    kernels leave room for one small CTA per SM, so the serve does not wait for a pre-position to finish."""
+    dev, s = wl.dev, wl.spec["shape"]
+    s_lo, s_hi = torch.cuda.Stream(priority=0), torch.cuda.Stream(priority=-1)
+    n = 64
+    ctx2 = prepos.Context(s.layers, s.Hq, s.Hkv, s.d, s.H, s.V, s.page, max_sessions=n)
+    sid = torch.arange(n, dtype=torch.int32, device=dev)
+    recs = prepos.new_records(n, dev)
+    ver = torch.zeros(n, dtype=torch.int64, device=dev)
+    hidden, _, _ = synth.make_hidden(s, n, wl.w, wl.fast, wl.spec["seed"] + 9)
+    ctx2.ready_dist(sid, hidden, wl.w, recs, ver)
+    torch.cuda.synchronize()
+    req = synth.serve_requests(n, n, wl.spec["seed"] + 3).to(dev)
+    dec = torch.zeros(n, dtype=torch.int32, device=dev)
+    tok = torch.zeros(n, dtype=torch.int32, device=dev)
+    dec_h = torch.empty(n, dtype=torch.int32).pin_memory()
+
+    def serve_once():
+        t0 = time.perf_counter()
+        with torch.cuda.stream(s_hi):
+            ctx2.gate_serve(req, recs, ver, wl.bitmap, s.tau, dec, tok)
+            dec_h.copy_(dec, non_blocking=True)
+        s_hi.synchronize()
+        return (time.perf_counter() - t0) * 1e6
+
+    for _ in range(20):
+        serve_once()
+    idle = sorted(serve_once() for _ in range(n_serves))
+    # the low-priority stream gets ~15 ms of pre-position steps in one go (no second host thread competing for the
+    # interpreter), and the serves are issued for as long as that work is running
+    t0 = time.perf_counter()
+    wl.step(0)
+    torch.cuda.synchronize()
+    per_step = max(time.perf_counter() - t0, 1e-4)
+    n_bg = max(4, min(400, int(0.015 / per_step)))
+    busy, i, rounds = [], 0, 0
+    while len(busy) < n_serves and rounds < 200:
+        rounds += 1
+        end = torch.cuda.Event()
+        with torch.cuda.stream(s_lo):
+            for _ in range(n_bg):
+                wl.step(i)
+                i += 1
+            end.record(s_lo)
+        while not end.query() and len(busy) < n_serves:
+            v = serve_once()
+            if not end.query():          # the pre-position was still running when the serve returned
+                busy.append(v)
+        torch.cuda.synchronize()
+    ctx2.close()
+    busy.sort()
+    q = lambda v, p: round(v[min(len(v) - 1, int(len(v) * p))], 1)
+    return {"requests_per_serve": n, "idle_wall_us": {"p50": q(idle, 0.5), "p99": q(idle, 0.99)},
+            "during_preposition_wall_us": {"p50": q(busy, 0.5), "p90": q(busy, 0.9), "p99": q(busy, 0.99)}}
+
+
 def run_fall_through(wl, reps=20):
     """SURVEY.md 8(f) NEXT-1, the step after a gate miss (Eq. 5): prepos_entry_attn with a delta of
     8 tokens, and with the single decode token, over the same cached sessions (all layers, one launch each).
@@ -634,6 +693,8 @@ def main():
         ft = run_fall_through(wl)
         if ft:
             line["fall_through"] = ft
+        if d.world == 1:
+            line["co_schedule"] = run_co_schedule(wl, prepos)
         if not args.no_cpu_baseline:
             osmp = OracleSample(spec)
             units, rows = osmp.plan(15.0)

@@ -36,8 +36,13 @@ constexpr int kThreads = 384;
 constexpr int kTile = kAttnTileTokens;  // 128 tokens
 constexpr int kNK = 3;                  // K ring slots
 constexpr float kRescaleThreshold = 8.f;  // log2 units: lazy rescale (P <= 2^8)
-constexpr int kServiceRegs = 72;          // 128 * 72 + 256 * 216 = 384 * 168
-constexpr int kSoftmaxRegs = 216;
+// Register budget: the kernel is launched with kLaunchRegs per thread, NOT the whole register file, and uses 1 KB less
+// than the shared-memory maximum, so that one small CTA of another kernel -- the gate serve of a request that
+// arrives while the idle-window pass is running (the pass "yields to any request") -- fits
+// beside it on every SM: 384 * 160 = 61440 registers leave 4096, a 128-thread gate_serve CTA takes 3072.
+constexpr int kLaunchRegs = 160;
+constexpr int kServiceRegs = 64;          // 128 * 64 + 256 * 208 = 384 * 160
+constexpr int kSoftmaxRegs = 208;
 
 struct UmmaParams {
     AttnArgs a;
@@ -210,7 +215,7 @@ __device__ __forceinline__ void append_entry(const UmmaParams &p, const Seg &s, 
 }
 
 template <int D>
-__global__ void __launch_bounds__(kThreads, 1)
+__global__ void __maxnreg__(kLaunchRegs)
 attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__ CUtensorMap tm_v,
                  const __grid_constant__ CUtensorMap tm_kn, const __grid_constant__ CUtensorMap tm_vn,
                  const __grid_constant__ CUtensorMap tm_q,
@@ -235,8 +240,8 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
     uint64_t *k_full = bars, *k_empty = bars + 3, *v_full = bars + 6, *v_empty = bars + 9;
     uint64_t *s_full = bars + 12, *p_ready = bars + 14, *o_done = bars + 16, *q_full = bars + 18;
     uint64_t *q_empty = bars + 19;    // the segment's last QK has read Q: the loader may overwrite it
-    float2 *ml_x = reinterpret_cast<float2 *>(bars + 20);  // [2][128] (m_used, l) exchange
-    uint32_t *tmem_slot = reinterpret_cast<uint32_t *>(ml_x + 256);
+    float2 *ml_x = reinterpret_cast<float2 *>(bars + 20);  // [128] (m, l) of stream 1 / the row factors back
+    uint32_t *tmem_slot = reinterpret_cast<uint32_t *>(ml_x + 128);
     int *merge_info = reinterpret_cast<int *>(tmem_slot + 1);  // [3]: c0 (or -1 = not last), c1, c0's slot
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -657,15 +662,28 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
             } else {
                 // both streams hold partial sums of the same rows: exchange (m, l), then WG w finishes columns
                 // [w * D/2, (w+1) * D/2) of the merged row
-                ml_x[w * 128 + row] = make_float2(m_used, l_sum);
-                ptx::bar_sync(1, 256);
-                const float2 a = ml_x[row], b = ml_x[128 + row];
+                // (one 1 KB array both ways: stream 1 hands (m, l) to stream 0, which hands back the two row factors)
                 const bool two = n_items > 1;
-                const float M = two ? fmaxf(a.x, b.x) : a.x;
-                const float wa = exp2f(a.x - M), wb = two ? exp2f(b.x - M) : 0.f;
-                const float L = wa * a.y + wb * b.y;
-                const float inv = 1.f / L;
-                const float fa = wa * inv, fb = wb * inv;
+                if (w == 1) ml_x[row] = make_float2(m_used, l_sum);
+                ptx::bar_sync(1, 256);
+                float fa, fb, lse2 = 0.f;
+                if (w == 0) {
+                    const float2 b = ml_x[row];
+                    const float M = two ? fmaxf(m_used, b.x) : m_used;
+                    const float wa = exp2f(m_used - M), wb = two ? exp2f(b.x - M) : 0.f;
+                    const float L = wa * l_sum + wb * b.y;
+                    const float inv = 1.f / L;
+                    fa = wa * inv;
+                    fb = wb * inv;
+                    lse2 = M + log2f(L);
+                    ml_x[row] = make_float2(fa, fb);
+                }
+                ptx::bar_sync(1, 256);
+                if (w == 1) {
+                    const float2 f2 = ml_x[row];
+                    fa = f2.x;
+                    fb = f2.y;
+                }
                 const bool live = row < rows;
                 constexpr int kHalfD = D / 2;
                 const uint32_t oa0 = tmem + lane_addr + kColO + w * kHalfD;
@@ -702,7 +720,7 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
                         }
                     }
                 }
-                if (live && !s.direct && w == 0) slot[kAttnMaxRows * D + row] = M + log2f(L);
+                if (live && !s.direct && w == 0) slot[kAttnMaxRows * D + row] = lse2;
                 ptx::bar_sync(1, 256);  // ml_x is reused by the next segment
             }
             // ---- the single cross-CTA pass: the last CTA to deliver its partial of a cut unit combines them
@@ -938,7 +956,7 @@ int launch(prepos_ctx *ctx, const AttnArgs &a, int tiles_per_lh, cudaStream_t st
     p.nv = two ? 2 : 3;
     if (D == 64) p.nv = 3;
     constexpr int kTileBytes = kTile * D * 2;
-    const size_t smem = static_cast<size_t>(p.q_tiles + kNK + p.nv) * kTileBytes + 20 * 8 + 256 * 8 + 16;
+    const size_t smem = static_cast<size_t>(p.q_tiles + kNK + p.nv) * kTileBytes + 20 * 8 + 128 * 8 + 16;
     // one CTA per SM; never more CTAs than tiles, never more than the partial slots provisioned
     long long grid = ctx->num_sms;
     if (grid > p.total_tiles) grid = p.total_tiles;

@@ -193,3 +193,38 @@ def test_gate_sweep_matches_oracle_risk_coverage(prepos, oracle):
     out = ctx.gate_sweep(recs, ver, bm, full.cuda(), torch.tensor([3.0], dtype=torch.float32, device="cuda"))
     ctx.sync()
     assert int((dec == 0).sum()) == int(prepos.unpack_sweep(out)["accepted"][0])
+
+
+def test_gate_serve_runs_beside_a_running_preposition(prepos):
+    """the idle-window pass "yields to any request".  The persistent
+    attention kernel leaves registers and shared memory for one small CTA per SM, so a gate serve issued on a
+    high-priority stream while a long pre-position (~1 ms of attention) runs on a low-priority stream completes
+    long before it: after the serve has synchronised, the pre-position's end event has not fired."""
+    shape = synth.Shape("cosched", layers=48, Hq=64, Hkv=8, d=128, H=256, V=1024, page=16)
+    sb = synth.make_sessions(shape, [16384], [32], seed=5, device="cuda")
+    ctx = prepos.Context(shape.layers, shape.Hq, shape.Hkv, shape.d, shape.H, shape.V, shape.page, max_sessions=1)
+    out = torch.empty_like(sb.q)
+    n = 64
+    ctx2 = prepos.Context(1, 4, 2, 64, 256, 1024, 16, max_sessions=n)
+    recs = prepos.new_records(n)
+    ver = torch.zeros(n, dtype=torch.int64, device="cuda")
+    sid = torch.arange(n, dtype=torch.int32, device="cuda")
+    bm = prepos.fastset_build(torch.arange(16), 1024).cuda()
+    dec = torch.zeros(n, dtype=torch.int32, device="cuda")
+    tok = torch.zeros(n, dtype=torch.int32, device="cuda")
+    lo, hi = torch.cuda.Stream(priority=0), torch.cuda.Stream(priority=-1)
+    done = torch.cuda.Event()
+    ahead = 0
+    for _ in range(5):
+        torch.cuda.synchronize()
+        with torch.cuda.stream(lo):
+            ctx.entry_attn(sb.q, sb.k_new, sb.v_new, sb.k_pool, sb.v_pool, sb.page_table, sb.n_s, sb.l_entry,
+                           sb.capacity, out)
+            done.record(lo)
+        with torch.cuda.stream(hi):
+            ctx2.gate_serve(sid, recs, ver, bm, 3.0, dec, tok)
+        hi.synchronize()
+        ahead += not done.query()
+        torch.cuda.synchronize()
+    assert ahead >= 4, f"the gate serve overtook the running pre-position only {ahead} of 5 times"
+    assert bool((dec == 3).all())        # fresh records were never pre-positioned: STALE_OR_INVALID
