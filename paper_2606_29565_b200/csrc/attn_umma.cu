@@ -10,14 +10,18 @@
 // (= its part of one unit).  A unit covered by one segment is written directly; otherwise every
 // covering CTA writes a normalised fp32 partial + log-sum-exp, bumps the unit's arrival counter, and the
 // last CTA to arrive combines the partials in CTA order (the single cross-CTA pass; deterministic for a
-// fixed plan whoever arrives last).
+// fixed plan whoever arrives last).  A CTA runs the cut head segment at the end of its range FIRST, so that both
+// partials of a cut unit are delivered early and no merge sits in the kernel's tail.
 //
 // Inside a CTA (384 threads):
 //   warp 0  K producer: TMA into a ring of K tiles -- cached tiles through a 5-D map over the pool (one
 //           4 KB box per page), entry-token tiles through a 5-D map over K_new (one box per 8 tokens)
 //   warp 3  V producer: same for V (plus a zero fill of the rows of an entry tile no box covers)
-//   warp 2  TMEM allocator and the Append(E) writer (Alg. 1 l.5): K_new/V_new -> the session's pages
-//   warp 1  MMA issuer: S = Q K^T (SS, K-major SW128) into TMEM, O += P V (A = P from TMEM, B = V MN-major)
+//   warp 2  TMEM allocator, Q loader (TMA, one box per 8-row group of the unit's (token, head) rows, issued as soon
+//           as the previous segment's last QK has retired) and the Append(E) writer (Alg. 1 l.5): K_new/V_new ->
+//           the session's pages
+//   warp 1  MMA issuer: S = Q K^T (SS, K-major SW128) into TMEM, O += P V (A = P from TMEM, B = V MN-major);
+//           warp-uniform descriptor words, only the tcgen05 instructions under elect.sync
 //   warps 4-7 / 8-11  two softmax warpgroups, one TMEM lane (= query row) per thread: online softmax
 //           with lazy rescaling, P written back to TMEM as bf16 over S.
 // The CTA always runs two independent streams (S_w, O_w, own running max/sum): with >128 rows stream w
@@ -286,7 +290,7 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
     const int page_bytes = p.page * D * 2;
     const int page_groups = p.page >> 3;
 
-    // register budget: launch gives 168 regs x 384 threads.  The four service warps (warpgroup 0) hand theirs
+    // register budget: launch gives kLaunchRegs x 384 threads.  The four service warps (warpgroup 0) hand theirs
     // down to kServiceRegs; each softmax thread, which holds a 128-wide score row, grows to kSoftmaxRegs.
     if (warp < 4) {
     ptx::setmaxnreg_dec<kServiceRegs>();
