@@ -285,44 +285,85 @@ def run_device_timed(wl, steps, warmup, dist_ctx):
 
 def run_e2e(wl, steps, warmup, dist_ctx):
     """Same step through the public binding with HOST inputs: every step copies that step's Q/K_new/V_new,
-    hidden and request ids from pinned host memory, and reads back the attention output, the records and the
-    decisions; one sync per step (a caller waits for the result)."""
-    st0 = wl.sets[0]
-    sb0 = st0["sb"]
-    host = {k: getattr(sb0, k).cpu().pin_memory() for k in ("q", "k_new", "v_new")}
-    host["hidden"] = st0["hidden"].cpu().pin_memory()
-    host["req"] = wl.req.cpu().pin_memory()
-    out_h = torch.empty(sb0.q.shape, dtype=torch.bfloat16).pin_memory()
-    rec_h = torch.empty(wl.records.shape, dtype=torch.uint8).pin_memory()
-    dec_h = torch.empty(wl.dec.shape, dtype=torch.int32).pin_memory()
-    tok_h = torch.empty(wl.tok.shape, dtype=torch.int32).pin_memory()
-    h2d = sum(t.numel() * t.element_size() for t in host.values())
-    d2h = sum(t.numel() * t.element_size() for t in (out_h, rec_h, dec_h, tok_h))
+    hidden and request ids from pinned host memory and reads back the attention output, the records and the
+    decisions.  The copies run on their own streams, chained to the step by events (H2D(i) -> step(i) -> D2H(i)),
+    so the transfers of neighbouring steps overlap the kernels as a serving loop would arrange it; the host waits
+    for the results of step i - 2 before it issues step i (at most two steps in flight)."""
+    R = len(wl.sets)
+    host = []
+    for st in wl.sets:
+        sb = st["sb"]
+        h = {k: getattr(sb, k).cpu().pin_memory() for k in ("q", "k_new", "v_new")}
+        h["hidden"] = st["hidden"].cpu().pin_memory()
+        h["out"] = torch.empty(sb.q.shape, dtype=torch.bfloat16).pin_memory()
+        h["rec"] = torch.empty(wl.records.shape, dtype=torch.uint8).pin_memory()
+        h["dec"] = torch.empty(wl.dec.shape, dtype=torch.int32).pin_memory()
+        h["tok"] = torch.empty(wl.tok.shape, dtype=torch.int32).pin_memory()
+        host.append(h)
+    req_h = wl.req.cpu().pin_memory()
+    h0 = host[0]
+    h2d = sum(h0[k].numel() * h0[k].element_size() for k in ("q", "k_new", "v_new", "hidden")) + req_h.numel() * 4
+    d2h = sum(h0[k].numel() * h0[k].element_size() for k in ("out", "rec", "dec", "tok"))
+    cur = torch.cuda.current_stream()
+    s_in, s_out = torch.cuda.Stream(), torch.cuda.Stream()
+    step_done = [None] * R      # per resident set: the step that last used its device buffers
+    out_read = [None] * R       # per resident set: its attention output has been copied out
+    small_read = [None]         # records / decisions of the previous step have been copied out
+    prev_step = [None]
+    results = []                # per step: the event after its last D2H
 
     def one(i):
-        st = wl.sets[i % len(wl.sets)]
+        k = i % R
+        st, h = wl.sets[k], host[k]
         sb = st["sb"]
-        sb.q.copy_(host["q"], non_blocking=True)
-        sb.k_new.copy_(host["k_new"], non_blocking=True)
-        sb.v_new.copy_(host["v_new"], non_blocking=True)
-        st["hidden"].copy_(host["hidden"], non_blocking=True)
-        wl.req.copy_(host["req"], non_blocking=True)
+        if len(results) >= 2:
+            results[-2].synchronize()           # the caller consumes the result of step i - 2
+        with torch.cuda.stream(s_in):
+            if step_done[k] is not None:
+                s_in.wait_event(step_done[k])   # the set's inputs are no longer being read
+            sb.q.copy_(h["q"], non_blocking=True)
+            sb.k_new.copy_(h["k_new"], non_blocking=True)
+            sb.v_new.copy_(h["v_new"], non_blocking=True)
+            st["hidden"].copy_(h["hidden"], non_blocking=True)
+            if prev_step[0] is not None:
+                s_in.wait_event(prev_step[0])   # the shared request buffer is free
+            wl.req.copy_(req_h, non_blocking=True)
+            e_in = torch.cuda.Event()
+            e_in.record(s_in)
+        cur.wait_event(e_in)
+        if out_read[k] is not None:
+            cur.wait_event(out_read[k])         # the set's output buffer has been read
+        if small_read[0] is not None:
+            cur.wait_event(small_read[0])       # the shared records / decisions have been read
         wl.step(i)
-        out_h.copy_(st["out"], non_blocking=True)
-        rec_h.copy_(wl.records, non_blocking=True)
-        dec_h.copy_(wl.dec, non_blocking=True)
-        tok_h.copy_(wl.tok, non_blocking=True)
-        torch.cuda.synchronize()
+        e_step = torch.cuda.Event()
+        e_step.record(cur)
+        step_done[k] = e_step
+        prev_step[0] = e_step
+        with torch.cuda.stream(s_out):
+            s_out.wait_event(e_step)
+            h["rec"].copy_(wl.records, non_blocking=True)
+            h["dec"].copy_(wl.dec, non_blocking=True)
+            h["tok"].copy_(wl.tok, non_blocking=True)
+            e_small = torch.cuda.Event()
+            e_small.record(s_out)
+            small_read[0] = e_small
+            h["out"].copy_(st["out"], non_blocking=True)
+            e_out = torch.cuda.Event()
+            e_out.record(s_out)
+            out_read[k] = e_out
+        results.append(e_out)
 
     for i in range(warmup):
         one(i)
-    dist_ctx.barrier()
     torch.cuda.synchronize()
+    dist_ctx.barrier()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    e0.record()
+    e0.record(cur)
     for i in range(steps):
         one(warmup + i)
-    e1.record()
+    cur.wait_event(results[-1])     # the last step's results are on the host
+    e1.record(cur)
     torch.cuda.synchronize()
     dist_ctx.barrier()
     return dict(ms_per_step=e0.elapsed_time(e1) / steps, h2d=h2d, d2h=d2h)
@@ -425,9 +466,11 @@ def run_co_schedule(wl, prepos, n_serves=300):
         torch.cuda.synchronize()
     ctx2.close()
     busy.sort()
-    q = lambda v, p: round(v[min(len(v) - 1, int(len(v) * p))], 1)
+    q = lambda v, p: round(v[min(len(v) - 1, int(len(v) * p))], 1) if v else None
+    # (a launch-bound workload such as c1 never gets ahead of the host: no serve falls inside a running step)
     return {"requests_per_serve": n, "idle_wall_us": {"p50": q(idle, 0.5), "p99": q(idle, 0.99)},
-            "during_preposition_wall_us": {"p50": q(busy, 0.5), "p90": q(busy, 0.9), "p99": q(busy, 0.99)}}
+            "during_preposition_wall_us": {"p50": q(busy, 0.5), "p90": q(busy, 0.9), "p99": q(busy, 0.99),
+                                           "samples": len(busy)}}
 
 
 def run_fall_through(wl, reps=20):
@@ -634,7 +677,8 @@ def main():
     if not args.no_e2e:
         e = run_e2e(wl, max(3, min(args.steps, 50)), 3, d)
         e_ms = d.max(e["ms_per_step"], dev)
-        e2e = {"value": e_ms * 1e3 / (n_sess * d.world), "unit": UNIT, "h2d_bytes_per_step": e["h2d"], "d2h_bytes_per_step": e["d2h"]}
+        e2e = {"value": e_ms * 1e3 / (n_sess * d.world), "unit": UNIT, "h2d_bytes_per_step": e["h2d"], "d2h_bytes_per_step": e["d2h"],
+               "timing": "CUDA events from before the first H2D to after the last D2H; copies on their own streams, two steps in flight"}
 
     if d.rank == 0:
         pk = peaks()
