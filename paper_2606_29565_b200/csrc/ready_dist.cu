@@ -146,9 +146,15 @@ __device__ __forceinline__ void write_record_fields(prepos_record *rec, const To
 __device__ __forceinline__ Top2Lse merge_partials_warp(const RdPartial *partials, int row, int n_parts, int lane)
 {
     Top2Lse acc = t2_init();
-    for (int c = lane; c < n_parts; c += 32) {
-        const Top2Lse p = t2_load(partials + static_cast<size_t>(row) * kMaxRdPartials + c);
-        t2_merge(acc, p);
+    constexpr int kBatch = 5;  // 148 CTAs = 5 partials per lane: loaded together, merged in CTA order
+    for (int c0 = lane; c0 < n_parts; c0 += 32 * kBatch) {
+        Top2Lse part[kBatch];
+#pragma unroll
+        for (int j = 0; j < kBatch; ++j)
+            if (c0 + 32 * j < n_parts) part[j] = t2_load(partials + static_cast<size_t>(row) * kMaxRdPartials + c0 + 32 * j);
+#pragma unroll
+        for (int j = 0; j < kBatch; ++j)
+            if (c0 + 32 * j < n_parts) t2_merge(acc, part[j]);
     }
 #pragma unroll
     for (int mask = 1; mask < 32; mask <<= 1) {
@@ -524,7 +530,27 @@ ready_dist_batch_kernel(const __grid_constant__ CUtensorMap tm_w, const __grid_c
     ptx::tc_fence_before();
     __syncthreads();
     if (warp == 1) ptx::tmem_dealloc<256>(tmem);
-    finalize_records(p, warp, lane, kBThreads / 32);
+}
+
+// The single cross-CTA pass of the batched kernel, as its own launch: one warp per hidden row merges that row's
+// per-CTA partials in CTA order and writes the record.  (Done by the last-arriving CTA inside the kernel, the merge
+// of 64 rows x 148 partials by six warps was a 60 us serial tail behind a 160 us stream of W.)
+__global__ void __launch_bounds__(32) rd_finalize_kernel(const RdParams p, int n_parts)
+{
+    ptx::griddep_wait();
+    ptx::griddep_launch();
+    const int row = blockIdx.x, lane = threadIdx.x;
+    const Top2Lse t = merge_partials_warp(p.partials, row, n_parts, lane);
+    if (lane == 0 && !(p.skip_mask && p.skip_mask[row])) {
+        const int sid = p.session_ids[row];
+        prepos_record *rec = p.records + sid;
+        write_record_fields(rec, t);
+        rec->entry_hash = p.entry_hash ? p.entry_hash[row] : 0ull;
+        rec->position = p.position_p ? p.position_p[row] : 0ll;
+        rec->version = p.session_version[sid];
+        __threadfence();  // payload before the valid bit
+        rec->flags = PREPOS_FLAG_VALID | (t.nonfinite ? PREPOS_FLAG_NONFINITE : 0u);
+    }
 }
 
 // ---- a4': scan of stored fp32 logits ---------------------------------------------------------------
@@ -647,7 +673,8 @@ int prepos_launch_ready_dist(prepos_ctx *ctx, int n, const int32_t *session_ids,
             PREPOS_CUDA_TRY(cudaFuncSetAttribute(ready_dist_batch_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                                  static_cast<int>(smem)));
             PREPOS_CUDA_TRY(prepos_launch_pdl(ready_dist_batch_kernel, dim3(grid), dim3(kBThreads), smem, stream, tm, tmx, p));
-            ctx->launches += 1;
+            PREPOS_CUDA_TRY(prepos_launch_pdl(rd_finalize_kernel, dim3(p.n), dim3(32), 0, stream, p, grid));
+            ctx->launches += 2;
         }
         return PREPOS_OK;
     }
