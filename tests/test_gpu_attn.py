@@ -97,6 +97,10 @@ SHAPES = {
     "d128_g8": synth.Shape("b", layers=1, Hq=16, Hkv=2, d=128, H=128, V=64, page=16),
     "d64_g2": synth.Shape("c", layers=2, Hq=4, Hkv=2, d=64, H=128, V=64, page=16),
     "d128_g1": synth.Shape("d", layers=1, Hq=2, Hkv=2, d=128, H=128, V=64, page=16),
+    "d128_g16": synth.Shape("e", layers=1, Hq=16, Hkv=1, d=128, H=128, V=64, page=16),   # G > 8: two Q boxes per token
+    "d128_g3": synth.Shape("f", layers=2, Hq=6, Hkv=2, d=128, H=128, V=64, page=16),      # G not a power of two
+    "d128_p32": synth.Shape("g", layers=1, Hq=8, Hkv=2, d=128, H=128, V=64, page=32),     # another page size
+    "d96_g2": synth.Shape("h", layers=1, Hq=4, Hkv=2, d=96, H=128, V=64, page=16),        # head_dim the tcgen05 path skips
 }
 
 
@@ -112,6 +116,10 @@ SHAPES = {
     ("d128_g1", [260], [3]),
     ("d128_g4", [2500], [24]),                    # long enough to be split over many CTAs
     ("d128_g4", [300, 100], [0, 7]),              # an empty entry next to a real one
+    ("d128_g16", [200, 77], [9, 20]),             # 144 / 320 rows with 16 heads per kv head
+    ("d128_g3", [150], [11]),                     # CUDA-core kernel only (the tcgen05 path wants G = 2^k)
+    ("d128_p32", [333], [24]),
+    ("d96_g2", [140], [6]),
 ])
 def test_shapes_vs_oracle(prepos, oracle, path, shape_key, n_s, l_entry):
     shape = SHAPES[shape_key]
