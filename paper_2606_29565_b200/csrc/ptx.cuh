@@ -341,6 +341,40 @@ __device__ __forceinline__ void cp_async_wait_all()
     asm volatile("cp.async.wait_all;" ::: "memory");
 }
 
+// 2^x on the FMA pipe (Cody-Waite split + degree-3 minimax polynomial on [0, 1), relative error ~1e-4: far below
+// the bf16 rounding the result goes through): takes exp2 work off the 4-lane XU, which is a co-limit of the softmax.
+// x <= 127; anything below -126 returns 2^-126.
+__device__ __forceinline__ float ex2_poly(float x)
+{
+    x = fmaxf(x, -126.f);
+    float r;
+    asm("add.rm.ftz.f32 %0, %1, %2;" : "=f"(r) : "f"(x), "f"(12582912.f));   // low mantissa bits = floor(x)
+    const float f = x - (r - 12582912.f);                                    // in [0, 1)
+    const float q = fmaf(fmaf(fmaf(0.077119089663028717f, f, 0.227564394474029541f), f, 0.695146143436431885f), f, 1.0f);
+    return __int_as_float(__float_as_int(q) + (__float_as_int(r) << 23));
+}
+
+// the same for a pair, with the subtraction and the polynomial on packed fp32 pairs
+__device__ __forceinline__ void ex2_poly2(float x0, float x1, float &y0, float &y1)
+{
+    x0 = fmaxf(x0, -126.f);
+    x1 = fmaxf(x1, -126.f);
+    float r0, r1;
+    asm("add.rm.ftz.f32 %0, %1, %2;" : "=f"(r0) : "f"(x0), "f"(12582912.f));
+    asm("add.rm.ftz.f32 %0, %1, %2;" : "=f"(r1) : "f"(x1), "f"(12582912.f));
+    const uint64_t one2 = pack_f32x2(1.0f, 1.0f);
+    const uint64_t xf2 = add_f32x2(pack_f32x2(r0, r1), pack_f32x2(-12582912.f, -12582912.f));
+    const uint64_t f2 = fma_f32x2(xf2, pack_f32x2(-1.0f, -1.0f), pack_f32x2(x0, x1));
+    uint64_t q2 = fma_f32x2(pack_f32x2(0.077119089663028717f, 0.077119089663028717f), f2,
+                            pack_f32x2(0.227564394474029541f, 0.227564394474029541f));
+    q2 = fma_f32x2(q2, f2, pack_f32x2(0.695146143436431885f, 0.695146143436431885f));
+    q2 = fma_f32x2(q2, f2, one2);
+    float q0, q1;
+    unpack_f32x2(q2, q0, q1);
+    y0 = __int_as_float(__float_as_int(q0) + (__float_as_int(r0) << 23));
+    y1 = __int_as_float(__float_as_int(q1) + (__float_as_int(r1) << 23));
+}
+
 // named barrier among a subset of the CTA's warps
 __device__ __forceinline__ void bar_sync(int id, int threads)
 {
