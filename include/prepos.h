@@ -23,6 +23,16 @@
  *   - Launches are asynchronous on `stream` (a cudaStream_t passed as void*; NULL = the legacy default
  *     stream) and stream-ordered with each other.  An asynchronous CUDA fault surfaces as PREPOS_E_CUDA
  *     on a later call or on prepos_ctx_sync().
+ *   - Kernels are launched with programmatic dependent launch: a kernel's prologue may overlap the tail of the
+ *     previous libprepos kernel in the stream, and prepos_ready_dist starts fetching w_vocab before its
+ *     predecessor has finished.  Everything a libprepos call can write (pools, out, records, versions,
+ *     decisions) is read only after the predecessor has completed; w_vocab, fast_set_bitmap and page_table are
+ *     inputs no libprepos call writes, and must not be written by a caller's kernel that itself triggers
+ *     dependent launches early and is still running when the call is issued.  After any ordinary kernel, copy
+ *     or event the calls behave as plain stream-ordered launches.
+ *   - The persistent kernels leave registers and shared memory for one small block per SM, so that a
+ *     prepos_gate_serve issued on a higher-priority stream runs beside a pre-position pass instead of behind it
+ *     (PAPER.md:132, 144).
  *   - bf16 tensors are raw 16-bit patterns (void*).  All accumulation and every record field is fp32.
  *   - A ctx is not thread-safe; use one ctx per host thread / stream.
  */
