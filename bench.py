@@ -269,7 +269,9 @@ def run_device_timed(wl, steps, warmup, dist_ctx):
     dist_ctx.barrier()
     wall = time.perf_counter() - t_wall0
     launches = wl.ctx.launch_count() - launches0
-    # pass B: per-call events
+    # pass B: per-call events (after half a second of idle: the long HBM- and tensor-bound steps of pass A leave the
+    # board at its power cap, and a kernel timed between two events is meant to be the kernel alone)
+    time.sleep(0.5)
     evs = [[torch.cuda.Event(enable_timing=True) for _ in range(5)] for _ in range(steps)]
     with ClockSampler(torch.cuda.current_device()) as clk_b:
         for i in range(steps):
