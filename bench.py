@@ -475,6 +475,55 @@ def run_co_schedule(wl, prepos, n_serves=300):
                                            "samples": len(busy)}}
 
 
+def run_layer_sequential(wl, reps=10):
+    """SURVEY.md 8(d) schedule (S): the attention of the step as one launch PER LAYER (what an engine whose layer
+    l + 1 queries depend on layer l must issue; the timed step uses schedule (F), all layers in one launch, valid
+    for the synthetic where per-layer Q/K/V are pre-drawn).  Same kernel, `layer_begin = l, layer_end = l + 1`.
+    Timed twice: the calls issued one by one from Python (host-bound: ~19 us per call), and the same launches
+    captured once into a CUDA graph and replayed (what the device needs: programmatic dependent launch overlaps
+    the prologues, units spread over many CTAs take the cooperative merge)."""
+    s = wl.spec["shape"]
+    ab = algorithmic_bytes(wl.spec)["entry_attn"]
+
+    def issue(st):
+        sb = st["sb"]
+        for l in range(s.layers):
+            wl.ctx.entry_attn(sb.q, sb.k_new, sb.v_new, sb.k_pool, sb.v_pool, sb.page_table, wl.n_s_h, wl.l_h, wl.cap_h,
+                              st["out"], layer_begin=l, layer_end=l + 1)
+
+    def timed(fn):
+        ev = []
+        for i in range(reps + 2):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            fn(i)
+            e1.record()
+            ev.append((e0, e1))
+        torch.cuda.synchronize()
+        return statistics.fmean(a.elapsed_time(b) for a, b in ev[2:])
+
+    ms = timed(lambda i: issue(wl.sets[i % len(wl.sets)]))
+    out = {"launches": s.layers, "attn_ms": round(ms, 5), "achieved_gbs": round(ab / (ms * 1e-3) / 1e9, 1),
+           "frac_of_measured_hbm": round(ab / (ms * 1e-3) / 1e9 / peaks()["hbm"], 4)}
+    try:
+        graphs = []
+        side = torch.cuda.Stream()
+        for st in wl.sets:
+            g = torch.cuda.CUDAGraph()
+            side.wait_stream(torch.cuda.current_stream())
+            with torch.cuda.graph(g, stream=side):
+                issue(st)
+            graphs.append(g)
+        torch.cuda.current_stream().wait_stream(side)
+        gms = timed(lambda i: graphs[i % len(graphs)].replay())
+        out["graph_replay"] = {"attn_ms": round(gms, 5), "achieved_gbs": round(ab / (gms * 1e-3) / 1e9, 1),
+                               "frac_of_measured_hbm": round(ab / (gms * 1e-3) / 1e9 / peaks()["hbm"], 4)}
+    except Exception as e:  # capture is a convenience of this measurement, not part of the path
+        out["graph_replay"] = {"unavailable": str(e)[:120]}
+        torch.cuda.synchronize()
+    return out
+
+
 def run_fall_through(wl, reps=20):
     """SURVEY.md 8(f) NEXT-1, the step after a gate miss (Eq. 5): prepos_entry_attn with a delta of
     8 tokens, and with the single decode token, over the same cached sessions (all layers, one launch each).
@@ -736,6 +785,7 @@ def main():
         if e2e:
             line["e2e"] = e2e
         line["gate_serve"] = run_gate_serve(wl, prepos)
+        line["attn_layer_sequential"] = run_layer_sequential(wl)
         ft = run_fall_through(wl)
         if ft:
             line["fall_through"] = ft

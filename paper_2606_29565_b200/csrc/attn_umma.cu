@@ -39,6 +39,7 @@ namespace {
 constexpr int kThreads = 384;
 constexpr int kTile = kAttnTileTokens;  // 128 tokens
 constexpr int kNK = 3;                  // K ring slots
+constexpr int kLastArriverMax = 2;        // partials of a cut unit that the last-arriving CTA combines on the spot
 constexpr float kRescaleThreshold = 8.f;  // log2 units: lazy rescale (P <= 2^8)
 // Register budget: the kernel is launched with kLaunchRegs per thread, NOT the whole register file, and uses 1 KB less
 // than the shared-memory maximum, so that one small CTA of another kernel -- the gate serve of a request that
@@ -520,6 +521,13 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
         const uint32_t lane_addr = static_cast<uint32_t>((warp & 3) << 5) << 16;
         const int st = threadIdx.x - 128;                      // 0..255 among softmax threads
         uint32_t sph = 0, oph = 0;
+#ifdef PREPOS_CTA_TIMES
+        long long tz[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+#define PREPOS_TZ(i) if (st == 0 && tz[i] == 0) asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(tz[i]))
+        PREPOS_TZ(0);
+#else
+#define PREPOS_TZ(i)
+#endif
         SegIter it(p, t0, t1);
         Seg s;
         while (it.next(p, s)) {
@@ -547,6 +555,7 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
                 ptx::mbar_wait(ptx::smem_u32(&s_full[w]), sph);
                 sph ^= 1;
                 ptx::tc_fence_after();
+                PREPOS_TZ(1);
                 // The tile body exists twice (all columns visible / masked at `limit`): one body with a branch
                 // around the masking makes the compiler copy the whole 128-register score row at the join.
                 auto tile_body = [&](auto masked_tag) {
@@ -643,6 +652,7 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
                 have = true;
             }
             // ---- epilogue
+            PREPOS_TZ(2);
             ptx::mbar_wait(ptx::smem_u32(&o_done[w]), oph);
             oph ^= 1;
             ptx::tc_fence_after();
@@ -745,25 +755,35 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
                 ptx::bar_sync(1, 256);  // ml_x is reused by the next segment
             }
             // ---- the single cross-CTA pass: the last CTA to deliver its partial of a cut unit combines them
+            PREPOS_TZ(3);
             if (!s.direct) {
                 // the barrier orders every thread's partial stores before thread 0's release fence + ticket
                 ptx::bar_sync(1, 256);
+                const long long U0s = static_cast<long long>(s.lh) * p.tiles_per_lh + s.u.tile_prefix;
+                const int c0s = cta_of(p.total_tiles, gridDim.x, U0s);
+                const int c1s = cta_of(p.total_tiles, gridDim.x, U0s + s.u.n_tiles - 1);
+                // up to kLastArriverMax partials: the last CTA to arrive combines them right here.  More (a unit spread
+                // over many CTAs, e.g. one launch per layer): every covering CTA combines its share of the rows after
+                // its last segment (cooperative pass below); the ticket is fire-and-forget and nobody waits for it.
+                const bool coop = (c1s - c0s >= kLastArriverMax);
                 if (st == 0) {
-                    const long long U0 = static_cast<long long>(s.lh) * p.tiles_per_lh + s.u.tile_prefix;
-                    const int c0 = cta_of(p.total_tiles, gridDim.x, U0);
-                    const int c1 = cta_of(p.total_tiles, gridDim.x, U0 + s.u.n_tiles - 1);
                     unsigned int *cnt = p.counters + static_cast<size_t>(s.lh) * p.a.n_units + s.unit_idx;
                     ptx::fence_acq_rel_gpu();
-                    const unsigned int prev = atomicAdd(cnt, 1u);
-                    const bool last = (prev == static_cast<unsigned int>(c1 - c0));
-                    if (last) {
-                        *cnt = 0u;  // self-reset for the next launch
-                        ptx::fence_acq_rel_gpu();
+                    if (coop) {
+                        atomicAdd(cnt, 1u);
+                    } else {
+                        const unsigned int prev = atomicAdd(cnt, 1u);
+                        const bool last = (prev == static_cast<unsigned int>(c1s - c0s));
+                        if (last) {
+                            *cnt = 0u;  // self-reset for the next launch
+                            ptx::fence_acq_rel_gpu();
+                        }
+                        merge_info[0] = last ? c0s : -1;
+                        merge_info[1] = c1s;
+                        merge_info[2] = (cta_begin(p.total_tiles, gridDim.x, c0s) < U0s) ? 1 : 0;  // c0's slot for this unit
                     }
-                    merge_info[0] = last ? c0 : -1;
-                    merge_info[1] = c1;
-                    merge_info[2] = (cta_begin(p.total_tiles, gridDim.x, c0) < U0) ? 1 : 0;  // c0's slot for this unit
                 }
+                if (coop) continue;
                 ptx::bar_sync(1, 256);
                 const int c0 = merge_info[0], c1 = merge_info[1], c0_slot = merge_info[2];
                 if (c0 >= 0) {
@@ -857,6 +877,97 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
                 ptx::bar_sync(1, 256);  // merge_info is reused by the next segment
             }
         }
+        PREPOS_TZ(4);
+        // ---- cooperative cross-CTA pass for units spread over more than kLastArriverMax CTAs: this CTA has delivered
+        // all its partials (so no CTA ever waits for one that is itself waiting), now for each such unit it waits
+        // until every covering CTA has delivered, combines ITS share of the unit's rows from all partials in CTA
+        // order, and checks out; the last CTA to check out resets the counter.  All CTAs of the grid are resident
+        // (grid <= SM count, one CTA per SM), so the wait is for CTAs that are running.
+        {
+            SegIter it2(p, t0, t1);
+            Seg s2;
+            while (it2.next(p, s2)) {
+                if (s2.direct) continue;
+                const long long U0 = static_cast<long long>(s2.lh) * p.tiles_per_lh + s2.u.tile_prefix;
+                const int c0 = cta_of(p.total_tiles, gridDim.x, U0);
+                const int c1 = cta_of(p.total_tiles, gridDim.x, U0 + s2.u.n_tiles - 1);
+                const int nc = c1 - c0 + 1;
+                if (nc <= kLastArriverMax) continue;
+                unsigned int *cnt = p.counters + static_cast<size_t>(s2.lh) * p.a.n_units + s2.unit_idx;
+                if (st == 0) {
+                    while (ptx::ld_acquire_gpu(cnt) < static_cast<unsigned int>(nc)) __nanosleep(64);
+                }
+                ptx::bar_sync(1, 256);
+                PREPOS_TZ(5);
+                constexpr int kVec = D / 4;
+                constexpr int kCB = 20;  // partials loaded together: one round trip for a unit spread over <= 20 CTAs
+                constexpr size_t kSlotFloats = static_cast<size_t>(kAttnMaxRows) * (D + 2);
+                const int c0_slot = (cta_begin(p.total_tiles, gridDim.x, c0) < U0) ? 1 : 0;
+                const int rows = s2.u.ntok * G;
+                const int j = static_cast<int>(blockIdx.x) - c0;
+                const int r_lo = static_cast<int>(static_cast<long long>(rows) * j / nc);
+                const int r_hi = static_cast<int>(static_cast<long long>(rows) * (j + 1) / nc);
+                __nv_bfloat16 *ob = p.a.out + static_cast<size_t>(s2.layer) * p.a.out_layer_stride;
+                for (int idx = r_lo * kVec + st; idx < r_hi * kVec; idx += 256) {
+                    const int r = idx / kVec, v = idx - r * kVec;
+                    float M = -CUDART_INF_F, wsum = 0.f;
+                    float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
+                    for (int cb = 0; cb < nc; cb += kCB) {
+                        float lse[kCB];
+                        float4 o[kCB];
+#pragma unroll
+                        for (int q = 0; q < kCB; ++q) {
+                            const int c = c0 + cb + q;
+                            lse[q] = -CUDART_INF_F;
+                            o[q] = make_float4(0.f, 0.f, 0.f, 0.f);
+                            if (cb + q < nc) {
+                                const float *sl = p.partials + (2 * static_cast<size_t>(c) + (c == c0 ? c0_slot : 0)) * kSlotFloats;
+                                lse[q] = __ldcg(sl + kAttnMaxRows * D + r);
+                                o[q] = __ldcg(reinterpret_cast<const float4 *>(sl + static_cast<size_t>(r) * D) + v);
+                            }
+                        }
+                        float mc = lse[0];
+#pragma unroll
+                        for (int q = 1; q < kCB; ++q) mc = fmaxf(mc, lse[q]);
+                        const float Mn = fmaxf(M, mc);
+                        const float resc = (M == -CUDART_INF_F) ? 0.f : exp2f(M - Mn);
+                        acc.x *= resc;
+                        acc.y *= resc;
+                        acc.z *= resc;
+                        acc.w *= resc;
+                        wsum *= resc;
+                        M = Mn;
+#pragma unroll
+                        for (int q = 0; q < kCB; ++q) {  // CTA order
+                            const float wgt = (cb + q < nc) ? exp2f(lse[q] - M) : 0.f;
+                            acc.x = fmaf(wgt, o[q].x, acc.x);
+                            acc.y = fmaf(wgt, o[q].y, acc.y);
+                            acc.z = fmaf(wgt, o[q].z, acc.z);
+                            acc.w = fmaf(wgt, o[q].w, acc.w);
+                            wsum += wgt;
+                        }
+                    }
+                    const float inv = 1.f / wsum;
+                    const int tok = s2.u.tok0 + r / G, h = s2.kvh * G + r % G;
+                    uint2 pk;
+                    pk.x = pack_bf16(acc.x * inv, acc.y * inv);
+                    pk.y = pack_bf16(acc.z * inv, acc.w * inv);
+                    *reinterpret_cast<uint2 *>(ob + (static_cast<size_t>(s2.u.row0 + tok) * p.Hq + h) * D + v * 4) = pk;
+                }
+                ptx::bar_sync(1, 256);
+                if (st == 0) {
+                    ptx::fence_acq_rel_gpu();
+                    const unsigned int prev = atomicAdd(cnt, 1u);
+                    if (prev == static_cast<unsigned int>(2 * nc - 1)) *cnt = 0u;  // everyone has checked out
+                }
+                PREPOS_TZ(6);
+            }
+        }
+#ifdef PREPOS_CTA_TIMES
+        if (st == 0)
+            printf("TZ cta %d first_s %lld items %lld wait_o+epi %lld ticket %lld spin %lld merge %lld\n", blockIdx.x, tz[1] - tz[0],
+                   tz[2] - tz[1], tz[3] - tz[2], tz[4] - tz[3], tz[5] - tz[4], tz[6] - tz[5]);
+#endif
     }
 
     ptx::tc_fence_before();
