@@ -325,3 +325,27 @@ def test_fall_through_delta_resume_full_size(prepos, oracle):
                  v_new=synth.randn_bf16((shape.layers, 1, shape.Hkv, shape.d), g))
     o3 = run(v3, (sb.k_pool, sb.v_pool))
     assert sample(v3, o3, rng, layers) <= ATTN_ATOL
+
+
+def test_one_launch_per_layer_cooperative_merge(prepos, oracle):
+    """Schedule (S): one prepos_entry_attn call per layer.  With 2 kv heads x 25 tiles over 148 persistent CTAs every
+    unit is spread over ~25 CTAs, which takes the cooperative cross-CTA pass (each covering CTA merges its share of
+    the rows); 256 query rows per kv head (config 5's row geometry) and a ragged last tile.  Oracle on every row,
+    Append(E) on every layer, and a second round of launches on the same context (the self-resetting counters)."""
+    shape = synth.Shape("s_sched", layers=3, Hq=16, Hkv=2, d=128, H=128, V=64, page=16)
+    sb = synth.make_sessions(shape, [3100], [32], seed=77)
+    dev = "cuda"
+    ctx = prepos.Context(shape.layers, shape.Hq, shape.Hkv, shape.d, shape.H, shape.V, shape.page, max_sessions=1)
+    ctx.set_attn_path(2)
+    outs, _, _, _ = oracle_attn_batch(oracle, sb)
+    for rnd in range(2):
+        kp, vp = sb.k_pool.to(dev).clone(), sb.v_pool.to(dev).clone()
+        before = (kp.clone(), vp.clone())
+        out = torch.full(sb.q.shape, float("nan"), dtype=torch.bfloat16, device=dev)
+        q, kn, vn, pt = sb.q.to(dev), sb.k_new.to(dev), sb.v_new.to(dev), sb.page_table.to(dev)
+        for l in range(shape.layers):
+            st = ctx.entry_attn(q, kn, vn, kp, vp, pt, sb.n_s, sb.l_entry, sb.capacity, out, layer_begin=l, layer_end=l + 1)
+            assert st == [0]
+        ctx.sync()
+        check_attn(out, outs, sb)
+        _check_append(sb, kp, vp, before, [0], range(shape.layers))
