@@ -39,7 +39,7 @@ namespace {
 constexpr int kThreads = 384;
 constexpr int kTile = kAttnTileTokens;  // 128 tokens
 constexpr int kNK = 3;                  // K ring slots
-constexpr int kLastArriverMax = 2;        // partials of a cut unit that the last-arriving CTA combines on the spot
+constexpr int kLastArriverMax = 4;        // partials of a cut unit that the last-arriving CTA combines on the spot
 constexpr float kRescaleThreshold = 8.f;  // log2 units: lazy rescale (P <= 2^8)
 // Register budget: the kernel is launched with kLaunchRegs per thread, NOT the whole register file, and uses 1 KB less
 // than the shared-memory maximum, so that one small CTA of another kernel -- the gate serve of a request that
