@@ -51,7 +51,7 @@ constexpr int kMaxRdPartials = 1024;  // CTAs of a ready-dist launch (upper boun
 constexpr int kRdMaxRows = 128;       // hidden rows reduced by one ready-dist launch
 constexpr int kAttnTileTokens = 128;  // KV tokens per tile of the tcgen05 attention kernel
 constexpr int kAttnMaxRows = 256;     // query rows (G * entry tokens) per attention unit
-constexpr int kAttnMaxCtas = 1024;    // upper bound on the persistent attention grid
+constexpr int kAttnMaxCtas = 256;     // upper bound on the persistent attention grid (one CTA per SM: 148 on B200)
 
 // per-CTA partial of the vocabulary reduction (a4): merged under the order (logit desc, id asc)
 struct RdPartial {
