@@ -385,9 +385,11 @@ def run_gate_serve(wl, prepos, reps=200):
     res = {}
     for B in (1, 64, 4096):
         req = synth.serve_requests(B, n_sess, wl.spec["seed"] + B).to(dev)
-        dec = torch.zeros(B, dtype=torch.int32, device=dev)
-        tok = torch.zeros(B, dtype=torch.int32, device=dev)
-        dec_h, tok_h = torch.empty(B, dtype=torch.int32).pin_memory(), torch.empty(B, dtype=torch.int32).pin_memory()
+        # decisions and tokens in one device buffer and one pinned host buffer: a serve is answered with ONE D2H copy
+        both = torch.zeros((2, B), dtype=torch.int32, device=dev)
+        dec, tok = both[0], both[1]
+        both_h = torch.empty((2, B), dtype=torch.int32).pin_memory()
+        dec_h = both_h[0]
         for _ in range(10):
             ctx.gate_serve(req, recs, ver, wl.bitmap, s.tau, dec, tok)
         torch.cuda.synchronize()
@@ -402,8 +404,7 @@ def run_gate_serve(wl, prepos, reps=200):
         for _ in range(reps):
             t0 = time.perf_counter()
             ctx.gate_serve(req, recs, ver, wl.bitmap, s.tau, dec, tok)
-            dec_h.copy_(dec, non_blocking=True)
-            tok_h.copy_(tok, non_blocking=True)
+            both_h.copy_(both, non_blocking=True)
             torch.cuda.synchronize()
             walls.append((time.perf_counter() - t0) * 1e6)
         res[f"B{B}"] = {"device_us_per_call": round(dev_us, 3), "device_us_per_serve": round(dev_us / B, 5),
