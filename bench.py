@@ -470,10 +470,62 @@ def run_co_schedule(wl, prepos, n_serves=300):
     ctx2.close()
     busy.sort()
     q = lambda v, p: round(v[min(len(v) - 1, int(len(v) * p))], 1) if v else None
+    # A request that needs whole SMs -- the fall-through decode step of one session (L = 1, all layers) -- has to wait
+    # for pre-position CTAs to retire.  The caller bounds that wait by issuing the pre-position in layer chunks
+    # (`layer_begin/layer_end`): measured for one launch per step and for chunks of layers / 8.
+    decode = {}
+    if wl.n_s_h.numel() >= 1 and s.layers >= 8:
+        sb0 = wl.sets[0]["sb"]
+        ctx3 = prepos.Context(s.layers, s.Hq, s.Hkv, s.d, s.H, s.V, s.page, max_sessions=1)
+        q1 = sb0.q[:, :1].contiguous()
+        k1, v1 = sb0.k_new[:, :1].contiguous(), sb0.v_new[:, :1].contiguous()
+        o1 = torch.empty_like(q1)
+        ns1, l1, cap1 = wl.n_s_h[:1].clone(), torch.ones(1, dtype=torch.int32), wl.cap_h[:1].clone()
+
+        def decode_once():
+            t0 = time.perf_counter()
+            with torch.cuda.stream(s_hi):
+                ctx3.entry_attn(q1, k1, v1, sb0.k_pool, sb0.v_pool, sb0.page_table[:1], ns1, l1, cap1, o1)
+            s_hi.synchronize()
+            return (time.perf_counter() - t0) * 1e6
+
+        def step_chunked(i, chunk):
+            st = wl.sets[i % len(wl.sets)]
+            sb = st["sb"]
+            wl.ctx.invalidate(wl.sid, wl.version, wl.records)
+            for l0 in range(0, s.layers, chunk):
+                wl.ctx.entry_attn(sb.q, sb.k_new, sb.v_new, sb.k_pool, sb.v_pool, sb.page_table, wl.n_s_h, wl.l_h, wl.cap_h,
+                                  st["out"], layer_begin=l0, layer_end=min(s.layers, l0 + chunk))
+            wl.ctx.ready_dist(wl.sid, st["hidden"], wl.w, wl.records, wl.version, position_p=wl.position)
+            wl.ctx.gate_serve(wl.req, wl.records, wl.version, wl.bitmap, s.tau, wl.dec, wl.tok)
+
+        for _ in range(5):
+            decode_once()
+        d_idle = sorted(decode_once() for _ in range(40))
+        decode["idle_wall_us_p50"] = q(d_idle, 0.5)
+        for label, chunk in (("one_launch", s.layers), ("layer_chunks_of_%d" % (s.layers // 8), s.layers // 8)):
+            got, i, rounds = [], 0, 0
+            while len(got) < 40 and rounds < 100:
+                rounds += 1
+                end = torch.cuda.Event()
+                with torch.cuda.stream(s_lo):
+                    for _ in range(n_bg):
+                        step_chunked(i, chunk)
+                        i += 1
+                    end.record(s_lo)
+                while not end.query() and len(got) < 40:
+                    v = decode_once()
+                    if not end.query():
+                        got.append(v)
+                torch.cuda.synchronize()
+            got.sort()
+            decode["during_preposition_" + label] = {"p50": q(got, 0.5), "p90": q(got, 0.9), "samples": len(got)}
+        ctx3.close()
     # (a launch-bound workload such as c1 never gets ahead of the host: no serve falls inside a running step)
     return {"requests_per_serve": n, "idle_wall_us": {"p50": q(idle, 0.5), "p99": q(idle, 0.99)},
             "during_preposition_wall_us": {"p50": q(busy, 0.5), "p90": q(busy, 0.9), "p99": q(busy, 0.99),
-                                           "samples": len(busy)}}
+                                           "samples": len(busy)},
+            "decode_step_wall_us": decode}
 
 
 def run_layer_sequential(wl, reps=10):
