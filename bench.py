@@ -93,9 +93,9 @@ def attention_flops(spec):
 # DRAM bytes (dram__bytes_read.sum + dram__bytes_write.sum) of ONE launch of the dominant kernel, from the committed
 # `ncu --set full` captures (profiles/r01_ncu_full_final.md); None where no capture of that workload exists.
 NCU_TRAFFIC = {
-    ("c2", "entry_attn"): 546458000 + 10491904,
-    ("c2", "ready_dist"): 1050730000 + 4182528,
-    ("c3", "ready_dist"): 1050730000 + 4182528,   # same launch (V, H) as c2
+    ("c2", "entry_attn"): 546446000 + 7390976,
+    ("c2", "ready_dist"): 1050731000 + 3634432,
+    ("c3", "ready_dist"): 1050731000 + 3634432,   # same launch (V, H) as c2
     ("c4", "entry_attn"): 71075900000 + 1660029000,
     ("c4", "ready_dist"): 1051261000 + 3196000,
     ("c5", "entry_attn"): 5424376000 + 56912384,
