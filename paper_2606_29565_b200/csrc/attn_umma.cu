@@ -788,7 +788,7 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
                 const int c0 = merge_info[0], c1 = merge_info[1], c0_slot = merge_info[2];
                 if (c0 >= 0) {
                     constexpr int kVec = D / 4;  // float4 per row
-                    constexpr int kMaxC = 4;     // partials combined with all loads in flight; more take the loop
+                    constexpr int kMaxC = kLastArriverMax;  // partials combined with all loads in flight
                     constexpr size_t kSlotFloats = static_cast<size_t>(kAttnMaxRows) * (D + 2);
                     const float *base0 = p.partials + (2 * static_cast<size_t>(c0) + c0_slot) * kSlotFloats;
                     const int nc = c1 - c0 + 1;
@@ -850,28 +850,8 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
                     };
                     if (nc <= 2) {
                         merge_pass(std::integral_constant<int, 12>{}, std::integral_constant<int, 2>{});
-                    } else if (nc <= kMaxC) {
+                    } else {  // nc <= kLastArriverMax == kMaxC: more partials take the cooperative pass below
                         merge_pass(std::integral_constant<int, kU>{}, std::integral_constant<int, kMaxC>{});
-                    } else {
-                        for (int idx = st; idx < total; idx += 256) {
-                            const int r = idx / kVec, v = idx - r * kVec;
-                            float M = __ldcg(base0 + kAttnMaxRows * D + r);
-                            for (int c = c0 + 1; c <= c1; ++c)
-                                M = fmaxf(M, __ldcg(p.partials + 2 * static_cast<size_t>(c) * kSlotFloats + kAttnMaxRows * D + r));
-                            float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
-                            float wsum = 0.f;
-                            for (int c = c0; c <= c1; ++c) {
-                                const float *sl = (c == c0) ? base0 : p.partials + 2 * static_cast<size_t>(c) * kSlotFloats;
-                                const float wgt = exp2f(__ldcg(sl + kAttnMaxRows * D + r) - M);
-                                const float4 o = __ldcg(reinterpret_cast<const float4 *>(sl + static_cast<size_t>(r) * D) + v);
-                                acc.x = fmaf(wgt, o.x, acc.x);
-                                acc.y = fmaf(wgt, o.y, acc.y);
-                                acc.z = fmaf(wgt, o.z, acc.z);
-                                acc.w = fmaf(wgt, o.w, acc.w);
-                                wsum += wgt;
-                            }
-                            store_row(idx, acc, wsum);
-                        }
                     }
                 }
                 ptx::bar_sync(1, 256);  // merge_info is reused by the next segment
