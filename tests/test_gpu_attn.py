@@ -349,3 +349,41 @@ def test_one_launch_per_layer_cooperative_merge(prepos, oracle):
         ctx.sync()
         check_attn(out, outs, sb)
         _check_append(sb, kp, vp, before, [0], range(shape.layers))
+
+
+@pytest.mark.parametrize("path", PATHS)
+def test_random_geometries_vs_oracle(prepos, oracle, path):
+    """24 seeded random geometries (head_dim, group size, kv heads, layers, page size, 1-4 sessions with n_s in
+    [0, 700] and L in [0, 70], some sessions over budget): every output row and the Append(E) post-condition
+    against the oracle, on both GPU paths."""
+    rng = np.random.default_rng(20260629)
+    ran = 0
+    for case in range(24):
+        d = int(rng.choice([64, 128]))
+        G = int(rng.choice([1, 2, 4, 8]))
+        Hkv = int(rng.choice([1, 2, 3]))
+        layers = int(rng.integers(1, 4))
+        page = int(rng.choice([8, 16, 32, 64]))
+        n_sess = int(rng.integers(1, 5))
+        n_s = [int(rng.integers(0, 701)) for _ in range(n_sess)]
+        l_e = [int(rng.integers(0, 71)) for _ in range(n_sess)]
+        if sum(l_e) == 0:
+            l_e[0] = 5
+        shape = synth.Shape(f"rnd{case}", layers=layers, Hq=G * Hkv, Hkv=Hkv, d=d, H=128, V=64, page=page)
+        tight = [None] * n_sess
+        if n_sess > 1 and case % 3 == 0:
+            tight[1] = n_s[1] + max(0, l_e[1] - 1)      # one token short of the budget: skipped (Alg. 1 l.2-3)
+        sb = synth.make_sessions(shape, n_s, l_e, seed=9000 + case, tight_capacity=tight)
+        try:
+            out, kp, vp, before, status, _ = _gpu_run(prepos, sb, path)
+        except pytest.skip.Exception:
+            continue
+        ran += 1
+        outs, st, _, _ = oracle_attn_batch(oracle, sb)
+        assert status == [st[s] for s in range(n_sess)], (case, status, st)
+        for s in range(n_sess):
+            if status[s] != 0:          # skipped: its output rows are untouched
+                outs = {k: v for k, v in outs.items() if k[1] != s}
+        check_attn(out, outs, sb)
+        _check_append(sb, kp, vp, before, status, range(layers))
+    assert ran >= 12
