@@ -59,7 +59,8 @@ struct UmmaParams {
     int q_tiles;        // resident Q M-tiles (1 or 2)
     int nv;             // V ring slots
     float scale_log2;
-    float *partials;    // [2 * grid] slots of kAttnMaxRows * (D + 2) floats: O [256][D], lse2 [256], pad [256]
+    float *partials;    // [2 * grid] slots of kAttnMaxRows * (D + 2) floats: O as float4 [D / 4][256 rows] (a warp's
+                        // 32 rows of one float4 column are 512 contiguous bytes), lse2 [256], pad [256]
     unsigned int *counters;  // [n_lh][n_units] arrival counters of the cross-CTA pass (self-resetting)
 };
 
@@ -683,7 +684,7 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
                         } else {
 #pragma unroll
                             for (int c = 0; c < 32; c += 4)
-                                *reinterpret_cast<float4 *>(slot + static_cast<size_t>(urow) * D + cb + c) =
+                                reinterpret_cast<float4 *>(slot)[static_cast<size_t>((cb + c) >> 2) * kAttnMaxRows + urow] =
                                     make_float4(__uint_as_float(o[c]) * inv, __uint_as_float(o[c + 1]) * inv,
                                                 __uint_as_float(o[c + 2]) * inv, __uint_as_float(o[c + 3]) * inv);
                         }
@@ -746,7 +747,7 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
                         } else {
 #pragma unroll
                             for (int c = 0; c < 32; c += 4)
-                                *reinterpret_cast<float4 *>(slot + static_cast<size_t>(row) * D + w * kHalfD + cb + c) =
+                                reinterpret_cast<float4 *>(slot)[static_cast<size_t>((w * kHalfD + cb + c) >> 2) * kAttnMaxRows + row] =
                                     make_float4(f[c], f[c + 1], f[c + 2], f[c + 3]);
                         }
                     }
@@ -795,7 +796,7 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
                     constexpr int kU = 4;  // rows x float4 columns per thread and pass: kU * 2 * nc loads in flight
                     const int total = rows * kVec;
                     auto store_row = [&](int idx, const float4 &acc, float wsum) {
-                        const int r = idx / kVec, v = idx - r * kVec;
+                        const int v = idx / rows, r = idx - v * rows;
                         const float inv = 1.f / wsum;
                         const int tok = s.u.tok0 + r / G, h = s.kvh * G + r % G;
                         uint2 pk;
@@ -814,7 +815,7 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
 #pragma unroll
                             for (int u = 0; u < kU_; ++u) {
                                 const int idx = idx0 + u * 256;
-                                const int r = idx / kVec, v = idx - r * kVec;
+                                const int v = idx / rows, r = idx - v * rows;   // lanes run along the rows
 #pragma unroll
                                 for (int j = 0; j < kC_; ++j) {
                                     const float *sl = (j == 0) ? base0 : p.partials + 2 * static_cast<size_t>(c0 + j) * kSlotFloats;
@@ -822,7 +823,7 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
                                     o[u][j] = make_float4(0.f, 0.f, 0.f, 0.f);
                                     if (j < nc && idx < total) {
                                         lse[u][j] = __ldcg(sl + kAttnMaxRows * D + r);
-                                        o[u][j] = __ldcg(reinterpret_cast<const float4 *>(sl + static_cast<size_t>(r) * D) + v);
+                                        o[u][j] = __ldcg(reinterpret_cast<const float4 *>(sl) + static_cast<size_t>(v) * kAttnMaxRows + r);
                                     }
                                 }
                             }
@@ -888,8 +889,9 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
                 const int r_lo = static_cast<int>(static_cast<long long>(rows) * j / nc);
                 const int r_hi = static_cast<int>(static_cast<long long>(rows) * (j + 1) / nc);
                 __nv_bfloat16 *ob = p.a.out + static_cast<size_t>(s2.layer) * p.a.out_layer_stride;
-                for (int idx = r_lo * kVec + st; idx < r_hi * kVec; idx += 256) {
-                    const int r = idx / kVec, v = idx - r * kVec;
+                const int n_r = r_hi - r_lo;
+                for (int idx = st; idx < n_r * kVec; idx += 256) {
+                    const int v = idx / n_r, r = r_lo + (idx - v * n_r);   // lanes run along the rows
                     float M = -CUDART_INF_F, wsum = 0.f;
                     float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
                     for (int cb = 0; cb < nc; cb += kCB) {
@@ -903,7 +905,7 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
                             if (cb + q < nc) {
                                 const float *sl = p.partials + (2 * static_cast<size_t>(c) + (c == c0 ? c0_slot : 0)) * kSlotFloats;
                                 lse[q] = __ldcg(sl + kAttnMaxRows * D + r);
-                                o[q] = __ldcg(reinterpret_cast<const float4 *>(sl + static_cast<size_t>(r) * D) + v);
+                                o[q] = __ldcg(reinterpret_cast<const float4 *>(sl) + static_cast<size_t>(v) * kAttnMaxRows + r);
                             }
                         }
                         float mc = lse[0];
