@@ -59,6 +59,8 @@ struct UmmaParams {
     int q_tiles;        // resident Q M-tiles (1 or 2)
     int nv;             // V ring slots
     float scale_log2;
+    int use_bnd;        // 1: CTA c's range is [bnd[c], bnd[c + 1]) (units fewer than CTAs: whole CTAs per unit)
+    int bnd[kAttnMaxCtas + 1];
     float *partials;    // [2 * grid] slots of kAttnMaxRows * (D + 2) floats: O as float4 [D / 4][256 rows] (a warp's
                         // 32 rows of one float4 column are 512 contiguous bytes), lse2 [256], pad [256]
     unsigned int *counters;  // [n_lh][n_units] arrival counters of the cross-CTA pass (self-resetting)
@@ -141,14 +143,26 @@ struct SegIter {
     }
 };
 
-__device__ __forceinline__ long long cta_begin(long long total, int grid, int c)
+// CTA c's range of the global tile space is [cta_begin(c), cta_begin(c + 1)): equal shares of the tile space
+// (stream-K), or the host's table when the launch has fewer units than CTAs (then every unit gets whole CTAs).
+__device__ __forceinline__ long long cta_begin(const UmmaParams &p, int grid, int c)
 {
-    return total * c / grid;
+    if (p.use_bnd) return p.bnd[c];
+    return p.total_tiles * c / grid;
 }
-// the CTA whose range [cta_begin(c), cta_begin(c + 1)) holds tile t
-__device__ __forceinline__ int cta_of(long long total, int grid, long long t)
+// the CTA whose range holds tile t
+__device__ __forceinline__ int cta_of(const UmmaParams &p, int grid, long long t)
 {
-    return static_cast<int>(((t + 1) * grid + total - 1) / total) - 1;
+    if (p.use_bnd) {
+        int lo = 0, hi = grid - 1;   // the last c with bnd[c] <= t
+        while (lo < hi) {
+            const int mid = (lo + hi + 1) >> 1;
+            if (p.bnd[mid] <= t) lo = mid;
+            else hi = mid - 1;
+        }
+        return lo;
+    }
+    return static_cast<int>(((t + 1) * grid + p.total_tiles - 1) / p.total_tiles) - 1;
 }
 
 // 64-bit UMMA shared-memory descriptor, SWIZZLE_128B, version 1 (sm_100), as two words: low = start address and
@@ -285,8 +299,8 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
     if (threadIdx.x == 0) asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(dbg_t0));
 #endif
 
-    const long long t0 = cta_begin(p.total_tiles, gridDim.x, blockIdx.x);
-    const long long t1 = cta_begin(p.total_tiles, gridDim.x, blockIdx.x + 1);
+    const long long t0 = cta_begin(p, gridDim.x, blockIdx.x);
+    const long long t1 = cta_begin(p, gridDim.x, blockIdx.x + 1);
     const int G = p.Hq / p.Hkv;
     const int pages_per_tile = kTile >> p.page_shift;
     const int page_bytes = p.page * D * 2;
@@ -761,8 +775,8 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
                 // the barrier orders every thread's partial stores before thread 0's release fence + ticket
                 ptx::bar_sync(1, 256);
                 const long long U0s = static_cast<long long>(s.lh) * p.tiles_per_lh + s.u.tile_prefix;
-                const int c0s = cta_of(p.total_tiles, gridDim.x, U0s);
-                const int c1s = cta_of(p.total_tiles, gridDim.x, U0s + s.u.n_tiles - 1);
+                const int c0s = cta_of(p, gridDim.x, U0s);
+                const int c1s = cta_of(p, gridDim.x, U0s + s.u.n_tiles - 1);
                 // up to kLastArriverMax partials: the last CTA to arrive combines them right here.  More (a unit spread
                 // over many CTAs, e.g. one launch per layer): every covering CTA combines its share of the rows after
                 // its last segment (cooperative pass below); the ticket is fire-and-forget and nobody waits for it.
@@ -781,7 +795,7 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
                         }
                         merge_info[0] = last ? c0s : -1;
                         merge_info[1] = c1s;
-                        merge_info[2] = (cta_begin(p.total_tiles, gridDim.x, c0s) < U0s) ? 1 : 0;  // c0's slot for this unit
+                        merge_info[2] = (cta_begin(p, gridDim.x, c0s) < U0s) ? 1 : 0;  // c0's slot for this unit
                     }
                 }
                 if (coop) continue;
@@ -870,8 +884,8 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
             while (it2.next(p, s2)) {
                 if (s2.direct) continue;
                 const long long U0 = static_cast<long long>(s2.lh) * p.tiles_per_lh + s2.u.tile_prefix;
-                const int c0 = cta_of(p.total_tiles, gridDim.x, U0);
-                const int c1 = cta_of(p.total_tiles, gridDim.x, U0 + s2.u.n_tiles - 1);
+                const int c0 = cta_of(p, gridDim.x, U0);
+                const int c1 = cta_of(p, gridDim.x, U0 + s2.u.n_tiles - 1);
                 const int nc = c1 - c0 + 1;
                 if (nc <= kLastArriverMax) continue;
                 unsigned int *cnt = p.counters + static_cast<size_t>(s2.lh) * p.a.n_units + s2.unit_idx;
@@ -883,7 +897,7 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
                 constexpr int kVec = D / 4;
                 constexpr int kCB = 20;  // partials loaded together: one round trip for a unit spread over <= 20 CTAs
                 constexpr size_t kSlotFloats = static_cast<size_t>(kAttnMaxRows) * (D + 2);
-                const int c0_slot = (cta_begin(p.total_tiles, gridDim.x, c0) < U0) ? 1 : 0;
+                const int c0_slot = (cta_begin(p, gridDim.x, c0) < U0) ? 1 : 0;
                 const int rows = s2.u.ntok * G;
                 const int j = static_cast<int>(blockIdx.x) - c0;
                 const int r_lo = static_cast<int>(static_cast<long long>(rows) * j / nc);
@@ -1090,6 +1104,45 @@ int launch(prepos_ctx *ctx, const AttnArgs &a, int tiles_per_lh, cudaStream_t st
                     grid = g;
                     break;
                 }
+    }
+    // Fewer units than CTAs (one launch per layer: 8 kv heads for 148 CTAs): give every unit a whole number of CTAs,
+    // in proportion to its tiles, and cut it evenly among them.  No CTA then straddles two units (one segment, one
+    // epilogue per CTA) and the CTAs of a unit finish together, which is what its cooperative merge waits for.
+    p.use_bnd = 0;
+    {
+        const long long n_units_total = static_cast<long long>(p.n_lh) * a.n_units;
+        if (n_units_total < grid && p.total_tiles < (1ll << 30)) {
+            std::vector<long long> start, tiles;
+            for (int lh = 0; lh < p.n_lh; ++lh)
+                for (const AttnUnit &u : ctx->plan_units) {
+                    start.push_back(static_cast<long long>(lh) * tiles_per_lh + u.tile_prefix);
+                    tiles.push_back(u.n_tiles);
+                }
+            const int n = static_cast<int>(tiles.size());
+            std::vector<int> k(n);
+            long long used = 0;
+            for (int i = 0; i < n; ++i) {
+                long long ki = tiles[i] * grid / p.total_tiles;
+                ki = ki < 1 ? 1 : (ki > tiles[i] ? tiles[i] : ki);
+                k[i] = static_cast<int>(ki);
+                used += ki;
+            }
+            while (used < grid) {   // hand the remaining CTAs to the units with the most tiles per CTA
+                int best = -1;
+                for (int i = 0; i < n; ++i)
+                    if (k[i] < tiles[i] && (best < 0 || tiles[i] * k[best] > tiles[best] * k[i])) best = i;
+                if (best < 0) break;
+                ++k[best];
+                ++used;
+            }
+            if (used == grid) {
+                int c = 0;
+                for (int i = 0; i < n; ++i)
+                    for (int j = 0; j < k[i]; ++j) p.bnd[c++] = static_cast<int>(start[i] + tiles[i] * j / k[i]);
+                p.bnd[c] = static_cast<int>(p.total_tiles);
+                p.use_bnd = 1;
+            }
+        }
     }
     if (ctx->tm_k_ptr != a.k_pool || ctx->tm_v_ptr != a.v_pool || ctx->tm_layer_stride != a.pool_layer_stride ||
         ctx->tm_n_pages != a.n_pages) {
