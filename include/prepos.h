@@ -33,6 +33,17 @@
  *   - The persistent kernels leave registers and shared memory for one small block per SM, so that a
  *     prepos_gate_serve issued on a higher-priority stream runs beside a pre-position pass instead of behind it
  *     (PAPER.md:132, 144).
+ *   - Record publication (Sec. 3.6: a cached distribution is never served after the state
+ *     changed).  A record may be re-published (prepos_ready_dist) or invalidated (prepos_invalidate) on one stream
+ *     while prepos_gate_serve reads it on another.  Writer: flags <- next sequence number with VALID clear; fence;
+ *     payload incl. the version stamp; fence; flags <- sequence | VALID.  Reader: word 1 (gap, flags, version); fence;
+ *     words 0 and 2; fence; word 1 again -- any difference means a publication was in progress and the request falls
+ *     through (PREPOS_STALE_OR_INVALID); then the live session version is read and compared with the stamp.  A serve
+ *     therefore returns top1 and gap of ONE publication, stamped with the version that was live when the serve read
+ *     it.  One writer per record at a time: two prepos_ready_dist calls for the same session must be stream-ordered.
+ *     Pass expected_version to prepos_ready_dist whenever a mutation can commit (on any stream) while the
+ *     pre-position is running: the record is stamped with the version its inputs were computed at, never with a
+ *     later one.
  *   - bf16 tensors are raw 16-bit patterns (void*).  All accumulation and every record field is fp32.
  *   - A ctx is not thread-safe; use one ctx per host thread / stream.
  */
@@ -69,9 +80,10 @@ enum {
     PREPOS_INELIGIBLE = 4        /* l.1-2: realised entry != pre-positioned entry */
 };
 
-/* record flag bits */
+/* record flag bits; bits 2..31 of `flags` hold the publication sequence number (see "Record publication") */
 #define PREPOS_FLAG_VALID 1u     /* Alg. 1 l.12 decoded/valid */
 #define PREPOS_FLAG_NONFINITE 2u /* a logit was NaN/Inf: never served */
+#define PREPOS_FLAG_MASK 3u
 
 typedef struct prepos_ctx prepos_ctx;
 
@@ -80,7 +92,7 @@ typedef struct {
     int32_t n_q_heads;  /* Hq */
     int32_t n_kv_heads; /* Hkv, divides Hq; query head h reads kv head h / (Hq/Hkv) */
     int32_t head_dim;   /* d: multiple of 8, <= 256.  d in {64,128} with page_size 16 takes the tcgen05 path */
-    int32_t hidden;     /* H: multiple of 256 */
+    int32_t hidden;     /* H: multiple of 128 */
     int32_t vocab;      /* V >= 2 */
     int32_t page_size;  /* tokens per KV page (power of two, <= 128) */
 } prepos_model_shape;
@@ -95,7 +107,7 @@ typedef struct {
     int32_t top1;        /* argmax(l_ready): ties -> lowest id */
     int32_t top2;        /* id of l^(2) under the order (logit desc, id asc) */
     float gap;           /* gamma = l^(1) - l^(2), Eq. 11 */
-    uint32_t flags;      /* PREPOS_FLAG_* */
+    uint32_t flags;      /* PREPOS_FLAG_* in bits 0-1, publication sequence number in bits 2-31 */
     uint64_t version;    /* session state version the record was computed at */
     uint64_t entry_hash; /* caller's hash of the pre-positioned entry tokens; 0 = relaxed match */
     int64_t position;    /* decision point p = n_s + L_entry, Eq. 1 */
@@ -157,21 +169,26 @@ int prepos_entry_attn(prepos_ctx *ctx, int layer_begin, int layer_end, int n_ses
  * Alg. 1 l.6 (LM head) + l.10-12 and Alg. 2 l.3-4 (Eq. 11):
  * logits l_v = sum_k W[v][k] x_r[k] for each of n hidden rows, reduced in the same pass to the
  * record {max, lse, top1, top2, gap} under the order (logit desc, id asc).  records[session_ids[r]]
- * is overwritten: version = session_version[session_ids[r]] (the live version at pre-position
- * time), flags = VALID (| NONFINITE), position = position_p[r] (0 if NULL), entry_hash likewise.
+ * is overwritten: version = expected_version[r], the state version the caller computed hidden row r at,
+ * and the record is VALID only if that still equals session_version[session_ids[r]] when the pass ends (a
+ * mutation that committed meanwhile, on any stream, leaves it invalid: Sec. 3.6).  With expected_version
+ * NULL the live version at the end of the pass is stamped, which is right only when every mutation of the
+ * session is stream-ordered with this call.  flags = VALID (| NONFINITE) plus the publication sequence,
+ * position = position_p[r] (0 if NULL), entry_hash likewise.
  * skip_mask (DEVICE int32 [n], nullable): rows with a non-zero entry are left untouched (sessions
  * whose pre-position was skipped on budget; their record is NOT made valid).
  *
  * hidden DEVICE bf16 [n][H]; w_vocab DEVICE bf16 [V][H] row-major; session_ids DEVICE int32 [n];
  * position_p DEVICE int64 [n] nullable; entry_hash DEVICE uint64 [n] nullable;
  * records DEVICE (indexed by session id); session_version DEVICE uint64 (indexed by session id);
+ * expected_version DEVICE uint64 [n] nullable;
  * logits_out DEVICE fp32 [n][V] nullable (the full ready distribution).
  */
 int prepos_ready_dist(prepos_ctx *ctx, int n, const int32_t *session_ids,
                       const void *hidden, const void *w_vocab,
                       const int64_t *position_p, const uint64_t *entry_hash, const int32_t *skip_mask,
                       prepos_record *records, const uint64_t *session_version,
-                      float *logits_out, void *stream);
+                      const uint64_t *expected_version, float *logits_out, void *stream);
 
 /*
  * Alg. 2 l.3-4 on stored logits (the paper's serve-time vocabulary scan, Eq. 3):

@@ -51,6 +51,19 @@ def lib():
         L.oracle_entry_attn.restype = C.c_int
         L.oracle_entry_attn.argtypes = [p, p, p, p, p, p, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int,
                                         C.c_int, C.c_int, C.c_double, p, p, p]
+        L.oracle_entry_attn_ranged.restype = C.c_int
+        L.oracle_entry_attn_ranged.argtypes = [p, p, p, p, p, p, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int,
+                                               C.c_int, C.c_int, C.c_double, C.c_int, C.c_int, C.c_int, C.c_int,
+                                               p, p, p]
+        L.oracle_entry_attn_fp8.restype = C.c_int
+        L.oracle_entry_attn_fp8.argtypes = [p, p, p, p, p, p, p, p, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int,
+                                            C.c_int, C.c_int, C.c_double, C.c_int, C.c_int, C.c_int, C.c_int, p, p]
+        L.oracle_logits_w4.restype = None
+        L.oracle_logits_w4.argtypes = [p, p, p, C.c_int, C.c_int, C.c_int, p]
+        L.oracle_e4m3_decode.restype = C.c_double
+        L.oracle_e4m3_decode.argtypes = [C.c_uint8]
+        L.oracle_e4m3_encode.restype = C.c_uint8
+        L.oracle_e4m3_encode.argtypes = [C.c_float]
         L.oracle_logits.restype = None
         L.oracle_logits.argtypes = [p, p, C.c_int, C.c_int, p]
         L.oracle_record.restype = None
@@ -88,9 +101,11 @@ def _ptr(a: np.ndarray):
 
 
 def entry_attn(q, k_new, v_new, k_pool, v_pool, page_table, n_s, capacity_tokens, scale=None,
-               want_rowsum=False):
+               want_rowsum=False, heads=None, rows=None):
     """O1 for one session, one layer.  q [L,Hq,d], k_new/v_new [L,Hkv,d], pools [n_pages,Hkv,page,d]
-    (uint16 ndarrays; pools are modified in place by the append).  Returns dict(status, out, rowsum, position)."""
+    (uint16 ndarrays; pools are modified in place by the append).  Returns dict(status, out, rowsum, position).
+    heads=(lo, hi) / rows=(lo, hi) restrict the OUTPUTS computed to those query heads / entry rows (the others stay
+    NaN); the append is always complete."""
     L, Hq, d = q.shape
     Hkv = k_new.shape[1]
     page = k_pool.shape[2]
@@ -104,12 +119,77 @@ def entry_attn(q, k_new, v_new, k_pool, v_pool, page_table, n_s, capacity_tokens
     pos = np.zeros(1, dtype=np.int64)
     if scale is None:
         scale = 1.0 / float(np.sqrt(d))
-    st = lib().oracle_entry_attn(_ptr(q), _ptr(k_new), _ptr(v_new), _ptr(k_pool), _ptr(v_pool), _ptr(pt),
-                                 int(n_s), int(L), int(capacity_tokens), int(Hq), int(Hkv), int(d), int(page),
-                                 float(scale), _ptr(out), _ptr(rowsum) if want_rowsum else None, _ptr(pos))
+    if heads is None and rows is None:
+        st = lib().oracle_entry_attn(_ptr(q), _ptr(k_new), _ptr(v_new), _ptr(k_pool), _ptr(v_pool), _ptr(pt),
+                                     int(n_s), int(L), int(capacity_tokens), int(Hq), int(Hkv), int(d), int(page),
+                                     float(scale), _ptr(out), _ptr(rowsum) if want_rowsum else None, _ptr(pos))
+    else:
+        h_lo, h_hi = (0, Hq) if heads is None else heads
+        i_lo, i_hi = (0, L) if rows is None else rows
+        st = lib().oracle_entry_attn_ranged(_ptr(q), _ptr(k_new), _ptr(v_new), _ptr(k_pool), _ptr(v_pool), _ptr(pt),
+                                            int(n_s), int(L), int(capacity_tokens), int(Hq), int(Hkv), int(d),
+                                            int(page), float(scale), int(h_lo), int(h_hi), int(i_lo), int(i_hi),
+                                            _ptr(out), _ptr(rowsum) if want_rowsum else None, _ptr(pos))
     if st < 0:
         raise ValueError("oracle_entry_attn: bad argument")
     return {"status": st, "out": out, "rowsum": rowsum, "position": int(pos[0]) if st == 0 else None}
+
+
+def e4m3_decode(codes) -> np.ndarray:
+    """e4m3 codes (uint8 array) -> fp64 values, through the oracle's decoder."""
+    c = np.asarray(codes, dtype=np.uint8)
+    L = lib()
+    return np.array([L.oracle_e4m3_decode(int(b)) for b in c.ravel()], dtype=np.float64).reshape(c.shape)
+
+
+def e4m3_encode(values) -> np.ndarray:
+    """fp32 values -> e4m3 codes (round to nearest even, saturating), through the oracle's encoder."""
+    v = np.asarray(values, dtype=np.float32)
+    L = lib()
+    return np.array([L.oracle_e4m3_encode(float(y)) for y in v.ravel()], dtype=np.uint8).reshape(v.shape)
+
+
+def entry_attn_fp8(q, k_new, v_new, k_pool8, v_pool8, k_scale, v_scale, page_table, n_s, capacity_tokens,
+                   scale=None, heads=None, rows=None):
+    """O7: O1 over an e4m3 KV cache (reading Q20).  Pools [n_pages,Hkv,page,d] uint8 (modified in place
+    by the append), scales [n_pages,Hkv] float32.  Returns dict(status, out, position)."""
+    L, Hq, d = q.shape
+    Hkv = k_new.shape[1]
+    page = k_pool8.shape[2]
+    assert k_pool8.dtype == np.uint8 and k_pool8.flags.c_contiguous and v_pool8.flags.c_contiguous
+    q = np.ascontiguousarray(q)
+    k_new = np.ascontiguousarray(k_new)
+    v_new = np.ascontiguousarray(v_new)
+    ks = np.ascontiguousarray(k_scale, dtype=np.float32)
+    vs = np.ascontiguousarray(v_scale, dtype=np.float32)
+    pt = np.ascontiguousarray(page_table, dtype=np.int32)
+    out = np.full((L, Hq, d), np.nan, dtype=np.float64)
+    pos = np.zeros(1, dtype=np.int64)
+    if scale is None:
+        scale = 1.0 / float(np.sqrt(d))
+    h_lo, h_hi = (0, Hq) if heads is None else heads
+    i_lo, i_hi = (0, L) if rows is None else rows
+    st = lib().oracle_entry_attn_fp8(_ptr(q), _ptr(k_new), _ptr(v_new), _ptr(k_pool8), _ptr(v_pool8), _ptr(ks), _ptr(vs),
+                                     _ptr(pt), int(n_s), int(L), int(capacity_tokens), int(Hq), int(Hkv), int(d),
+                                     int(page), float(scale), int(h_lo), int(h_hi), int(i_lo), int(i_hi), _ptr(out),
+                                     _ptr(pos))
+    if st < 0:
+        raise ValueError("oracle_entry_attn_fp8: bad argument")
+    return {"status": st, "out": out, "position": int(pos[0]) if st == 0 else None}
+
+
+def logits_w4(w4, w_scale, x, group=128) -> np.ndarray:
+    """O8: O2 over a 4-bit W_vocab (reading Q21).  w4 [V,H/2] uint8, w_scale [V,H/group] bf16 bits,
+    x [H] bf16 bits -> fp64 [V]."""
+    V, H2 = w4.shape
+    H = 2 * H2
+    w4 = np.ascontiguousarray(w4, dtype=np.uint8)
+    w_scale = np.ascontiguousarray(w_scale, dtype=np.uint16)
+    x = np.ascontiguousarray(x, dtype=np.uint16)
+    assert x.shape == (H,) and w_scale.shape == (V, H // group) and H % group == 0
+    out = np.empty(V, dtype=np.float64)
+    lib().oracle_logits_w4(_ptr(w4), _ptr(w_scale), _ptr(x), V, H, int(group), _ptr(out))
+    return out
 
 
 def logits(w, x) -> np.ndarray:

@@ -16,9 +16,15 @@
  *   O3 oracle_record       Eq. 11, Alg. 2 l.3-4
  *   O4 oracle_gate         Eq. 12, Alg. 2
  *   O5 oracle_invalidate / oracle_stamp   Sec. 3.6, Fig. 3
+ *   O7 oracle_entry_attn_fp8  O1 over an FP8 (e4m3) KV cache   } the quantised variants of SURVEY.md 8(f) NEXT-4
+ *   O8 oracle_logits_w4       O2 over a 4-bit W_vocab          } (the paper's headline model "runs at 4-bit
+ *                             precision").  The paper gives no storage format: the rules are
+ *                             this build's reading, Q20 / Q21; each dequantises exactly and then IS O1 / O2.
  *
  * Pins (tests/test_oracle_*.py, all `-m "not gpu"`): every function here is pinned by
  * closed forms, invariants, library cross-checks and brute force; none is "parity unpinned".
+ * O7 / O8: the e4m3 codec against a library's e4m3 on all 256 codes and a dense grid of values, and
+ * equality with O1 / O2 wherever code * scale is exactly representable (tests/test_oracle_quant.py).
  *
  * OpenMP is used only over independent outputs (query rows, vocabulary rows); each
  * output is still computed by the serial definition.
@@ -68,13 +74,19 @@ static size_t pool_offset(const int32_t *page_table, int j, int g, int Hkv, int 
  * rowsum [L][Hq]      fp64   sum_j p_j of every row (for the "softmax sums to 1" pin); may be NULL
  * returns 0 = done, 1 = skipped on budget, -1 = bad argument
  */
-int oracle_entry_attn(const uint16_t *q, const uint16_t *k_new, const uint16_t *v_new,
-                      uint16_t *k_pool, uint16_t *v_pool, const int32_t *page_table,
-                      int n_s, int L, int capacity_tokens,
-                      int Hq, int Hkv, int d, int page, double scale,
-                      double *out, double *rowsum, int64_t *position_out)
+/* The same pass, producing only the outputs (h, i) with h_lo <= h < h_hi, i_lo <= i < i_hi (the other rows of `out`
+ * and `rowsum` are left untouched; the append is always done in full).  oracle_entry_attn below IS this function
+ * over the full ranges, so every pin of O1 exercises this code; the sampled full-size parity tests use the ranges. */
+int oracle_entry_attn_ranged(const uint16_t *q, const uint16_t *k_new, const uint16_t *v_new,
+                             uint16_t *k_pool, uint16_t *v_pool, const int32_t *page_table,
+                             int n_s, int L, int capacity_tokens,
+                             int Hq, int Hkv, int d, int page, double scale,
+                             int h_lo, int h_hi, int i_lo, int i_hi,
+                             double *out, double *rowsum, int64_t *position_out)
 {
     if (n_s < 0 || L < 0 || Hq <= 0 || Hkv <= 0 || d <= 0 || page <= 0 || Hq % Hkv != 0)
+        return -1;
+    if (h_lo < 0 || h_hi > Hq || i_lo < 0 || i_hi > L)
         return -1;
     /* Alg. 1 l.2-3: cell-budget headroom B = capacity - n_s */
     if (L > capacity_tokens - n_s)
@@ -93,8 +105,8 @@ int oracle_entry_attn(const uint16_t *q, const uint16_t *k_new, const uint16_t *
     /* Alg. 1 l.6: attention of each entry row over cache positions 0..n_s+i */
     int bad = 0;
 #pragma omp parallel for collapse(2) schedule(dynamic, 1)
-    for (int h = 0; h < Hq; ++h)
-        for (int i = 0; i < L; ++i) {
+    for (int h = h_lo; h < h_hi; ++h)
+        for (int i = i_lo; i < i_hi; ++i) {
             const int g = h / G;
             const int n_keys = n_s + i + 1;
             double *s = (double *)malloc((size_t)n_keys * sizeof(double));
@@ -140,6 +152,16 @@ int oracle_entry_attn(const uint16_t *q, const uint16_t *k_new, const uint16_t *
     return 0;
 }
 
+int oracle_entry_attn(const uint16_t *q, const uint16_t *k_new, const uint16_t *v_new,
+                      uint16_t *k_pool, uint16_t *v_pool, const int32_t *page_table,
+                      int n_s, int L, int capacity_tokens,
+                      int Hq, int Hkv, int d, int page, double scale,
+                      double *out, double *rowsum, int64_t *position_out)
+{
+    return oracle_entry_attn_ranged(q, k_new, v_new, k_pool, v_pool, page_table, n_s, L, capacity_tokens, Hq, Hkv, d,
+                                    page, scale, 0, Hq, 0, L < 0 ? 0 : L, out, rowsum, position_out);
+}
+
 /*
  * O2.  Ready-distribution logits: l_v = sum_k W[v][k] * x[k].
  * w [V][H] bf16 bits row-major, x [H] bf16 bits (reading Q7: the caller's final hidden
@@ -153,6 +175,166 @@ void oracle_logits(const uint16_t *w, const uint16_t *x, int V, int H, double *l
         double acc = 0.0;
         for (int k = 0; k < H; ++k)
             acc += bf16_to_double(wv[k]) * bf16_to_double(x[k]);
+        logits[v] = acc;
+    }
+}
+
+/* ------------------------------------------------------------------------------------------------------------------
+ * Quantised variants ("4-bit precision").  The paper states no format, so
+ * these follow DESIGN.md readings Q20 (FP8 KV) and Q21 (4-bit W_vocab).  Both dequantise EXACTLY (every code times
+ * its scale is formed in fp64) and then apply the fp64 definitions O1 / O2 unchanged.
+ * ---------------------------------------------------------------------------------------------------------------- */
+
+/* OCP FP8 E4M3 ("e4m3fn"): 1 sign, 4 exponent (bias 7), 3 mantissa bits; no infinities; S.1111.111 is NaN;
+ * exponent field 0 is subnormal: (m/8) * 2^-6.  Largest finite value 448 = 1.75 * 2^8. */
+double oracle_e4m3_decode(uint8_t b)
+{
+    const int sign = b >> 7, e = (b >> 3) & 15, m = b & 7;
+    double v;
+    if (e == 15 && m == 7)
+        return NAN;
+    if (e == 0)
+        v = ldexp((double)m / 8.0, -6);
+    else
+        v = ldexp(1.0 + (double)m / 8.0, e - 7);
+    return sign ? -v : v;
+}
+
+/* fp32 -> e4m3, round to nearest, ties to the even code, saturating to +-448 (NaN -> 0x7f).  Written as a search
+ * over the 127 finite magnitudes (codes 0x00..0x7e are monotone in value), not as bit manipulation. */
+uint8_t oracle_e4m3_encode(float y)
+{
+    if (isnan(y))
+        return 0x7f;
+    const uint8_t sign = signbit(y) ? 0x80 : 0x00;
+    const double a = fabs((double)y);
+    if (a >= 448.0)
+        return (uint8_t)(sign | 0x7e);
+    int lo = 0; /* largest code with value <= a */
+    for (int c = 0; c <= 0x7e; ++c)
+        if (oracle_e4m3_decode((uint8_t)c) <= a)
+            lo = c;
+    if (lo == 0x7e)
+        return (uint8_t)(sign | 0x7e);
+    const double vlo = oracle_e4m3_decode((uint8_t)lo), vhi = oracle_e4m3_decode((uint8_t)(lo + 1));
+    int pick;
+    if (a - vlo < vhi - a)
+        pick = lo;
+    else if (a - vlo > vhi - a)
+        pick = lo + 1;
+    else
+        pick = (lo & 1) ? lo + 1 : lo; /* tie: even mantissa */
+    return (uint8_t)(sign | pick);
+}
+
+/* scale of logical cache token j, kv head g: scales are [n_pages][Hkv] fp32, one per (page, kv head) (Q20) */
+static double page_scale(const float *scale, const int32_t *page_table, int j, int g, int Hkv, int page)
+{
+    return (double)scale[(size_t)page_table[j / page] * (size_t)Hkv + (size_t)g];
+}
+
+/*
+ * O7.  O1 over an FP8 KV cache (reading Q20).  k_pool8 / v_pool8 [n_pages][Hkv][page][d] are e4m3 codes;
+ * k_scale / v_scale [n_pages][Hkv] fp32 are caller-owned, one per (page, kv head), for every page of the session
+ * including the ones the entry is appended to.  Cached value = decode(code) * scale.
+ *   l.5  Append(E): code = e4m3(fp32(x) / scale) with the fp32 division and the conversion rounded to nearest even,
+ *        saturating (both sides take this decision in fp32, the kernel's precision)
+ *   l.6  Forward(E) runs after the append (Alg. 1 order), so entry row i sees the entry tokens j' <= i through
+ *        their STORED codes -- which makes a pre-position of L1 then L2 tokens identical to one of L1 + L2.
+ * Everything else (budget skip, scale, GQA map, two-pass softmax in fp64) is O1 word for word.
+ */
+int oracle_entry_attn_fp8(const uint16_t *q, const uint16_t *k_new, const uint16_t *v_new,
+                          uint8_t *k_pool8, uint8_t *v_pool8, const float *k_scale, const float *v_scale,
+                          const int32_t *page_table, int n_s, int L, int capacity_tokens,
+                          int Hq, int Hkv, int d, int page, double scale,
+                          int h_lo, int h_hi, int i_lo, int i_hi,
+                          double *out, int64_t *position_out)
+{
+    if (n_s < 0 || L < 0 || Hq <= 0 || Hkv <= 0 || d <= 0 || page <= 0 || Hq % Hkv != 0)
+        return -1;
+    if (h_lo < 0 || h_hi > Hq || i_lo < 0 || i_hi > L)
+        return -1;
+    if (L > capacity_tokens - n_s)
+        return 1;
+    const int G = Hq / Hkv;
+
+    for (int jp = 0; jp < L; ++jp)
+        for (int g = 0; g < Hkv; ++g) {
+            const size_t dst = pool_offset(page_table, n_s + jp, g, Hkv, page, d);
+            const size_t src = ((size_t)jp * (size_t)Hkv + (size_t)g) * (size_t)d;
+            const float ks = k_scale[(size_t)page_table[(n_s + jp) / page] * (size_t)Hkv + (size_t)g];
+            const float vs = v_scale[(size_t)page_table[(n_s + jp) / page] * (size_t)Hkv + (size_t)g];
+            for (int c = 0; c < d; ++c) {
+                k_pool8[dst + c] = oracle_e4m3_encode((float)bf16_to_double(k_new[src + c]) / ks);
+                v_pool8[dst + c] = oracle_e4m3_encode((float)bf16_to_double(v_new[src + c]) / vs);
+            }
+        }
+
+    int bad = 0;
+#pragma omp parallel for collapse(2) schedule(dynamic, 1)
+    for (int h = h_lo; h < h_hi; ++h)
+        for (int i = i_lo; i < i_hi; ++i) {
+            const int g = h / G;
+            const int n_keys = n_s + i + 1;
+            double *s = (double *)malloc((size_t)n_keys * sizeof(double));
+            if (!s) {
+                bad = 1;
+                continue;
+            }
+            const uint16_t *qi = q + ((size_t)i * (size_t)Hq + (size_t)h) * (size_t)d;
+            double m = -INFINITY;
+            for (int j = 0; j < n_keys; ++j) {
+                const uint8_t *kj = k_pool8 + pool_offset(page_table, j, g, Hkv, page, d);
+                const double ks = page_scale(k_scale, page_table, j, g, Hkv, page);
+                double acc = 0.0;
+                for (int c = 0; c < d; ++c)
+                    acc += bf16_to_double(qi[c]) * (oracle_e4m3_decode(kj[c]) * ks);
+                s[j] = acc * scale;
+                if (s[j] > m)
+                    m = s[j];
+            }
+            double denom = 0.0;
+            for (int j = 0; j < n_keys; ++j) {
+                s[j] = exp(s[j] - m);
+                denom += s[j];
+            }
+            double *oi = out + ((size_t)i * (size_t)Hq + (size_t)h) * (size_t)d;
+            for (int c = 0; c < d; ++c)
+                oi[c] = 0.0;
+            for (int j = 0; j < n_keys; ++j) {
+                const double p = s[j] / denom;
+                const uint8_t *vj = v_pool8 + pool_offset(page_table, j, g, Hkv, page, d);
+                const double vs = page_scale(v_scale, page_table, j, g, Hkv, page);
+                for (int c = 0; c < d; ++c)
+                    oi[c] += p * (oracle_e4m3_decode(vj[c]) * vs);
+            }
+            free(s);
+        }
+    if (bad)
+        return -1;
+    if (position_out)
+        *position_out = (int64_t)n_s + (int64_t)L;
+    return 0;
+}
+
+/*
+ * O8.  O2 over a 4-bit W_vocab (reading Q21).  w4 [V][H/2]: two codes per byte, the element with even k in the low
+ * nibble; a code is a two's-complement int4 in -8..7.  w_scale [V][H/group] bf16 bits, one per (row, group of `group`
+ * consecutive k).  W[v][k] = code * scale[v][k / group]; then l_v = sum_k W[v][k] x[k] exactly as O2.
+ */
+void oracle_logits_w4(const uint8_t *w4, const uint16_t *w_scale, const uint16_t *x, int V, int H, int group,
+                      double *logits)
+{
+#pragma omp parallel for schedule(static)
+    for (int v = 0; v < V; ++v) {
+        const uint8_t *wv = w4 + (size_t)v * (size_t)(H / 2);
+        const uint16_t *sv = w_scale + (size_t)v * (size_t)(H / group);
+        double acc = 0.0;
+        for (int k = 0; k < H; ++k) {
+            const int nib = (k & 1) ? (wv[k >> 1] >> 4) : (wv[k >> 1] & 15);
+            const int code = nib >= 8 ? nib - 16 : nib;
+            acc += ((double)code * bf16_to_double(sv[k / group])) * bf16_to_double(x[k]);
+        }
         logits[v] = acc;
     }
 }

@@ -228,9 +228,10 @@ int prepos_entry_attn(prepos_ctx *ctx, int layer_begin, int layer_end, int n_ses
 
     // ---- plan key: reuse the device copy of the plan when the batch geometry is unchanged
     std::vector<int32_t> key;
-    key.reserve(3 * n_sessions + 2);
+    key.reserve(3 * n_sessions + 3);
     key.push_back(use_umma ? 2 : 1);
     key.push_back(n_sessions);
+    key.push_back(page_table_stride);   // the plan was checked against this stride
     for (int i = 0; i < n_sessions; ++i) {
         if (n_s[i] < 0 || l_entry[i] < 0 || capacity_tokens[i] < 0) return PREPOS_E_INVALID_ARG;
         key.push_back(n_s[i]);
@@ -315,7 +316,8 @@ int prepos_entry_attn(prepos_ctx *ctx, int layer_begin, int layer_end, int n_ses
 
 int prepos_ready_dist(prepos_ctx *ctx, int n, const int32_t *session_ids, const void *hidden, const void *w_vocab,
                       const int64_t *position_p, const uint64_t *entry_hash, const int32_t *skip_mask,
-                      prepos_record *records, const uint64_t *session_version, float *logits_out, void *stream)
+                      prepos_record *records, const uint64_t *session_version, const uint64_t *expected_version,
+                      float *logits_out, void *stream)
 {
     if (!ctx || n < 0) return PREPOS_E_INVALID_ARG;
     if (n == 0) return PREPOS_OK;
@@ -323,7 +325,8 @@ int prepos_ready_dist(prepos_ctx *ctx, int n, const int32_t *session_ids, const 
     if (!aligned16(hidden) || !aligned16(w_vocab) || !aligned16(records)) return PREPOS_E_ALIGN;
     return prepos_launch_ready_dist(ctx, n, session_ids, static_cast<const __nv_bfloat16 *>(hidden),
                                     static_cast<const __nv_bfloat16 *>(w_vocab), position_p, entry_hash, skip_mask,
-                                    records, session_version, logits_out, static_cast<cudaStream_t>(stream));
+                                    records, session_version, expected_version, logits_out,
+                                    static_cast<cudaStream_t>(stream));
 }
 
 int prepos_scan_logits(prepos_ctx *ctx, int n, const float *logits, prepos_record *out, void *stream)

@@ -294,10 +294,6 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
     // kernels in the stream wrote (the plan, the pools, Q)
     ptx::griddep_wait();
     ptx::griddep_launch();
-#ifdef PREPOS_CTA_TIMES
-    long long dbg_t0 = 0;
-    if (threadIdx.x == 0) asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(dbg_t0));
-#endif
 
     const long long t0 = cta_begin(p, gridDim.x, blockIdx.x);
     const long long t1 = cta_begin(p, gridDim.x, blockIdx.x + 1);
@@ -483,19 +479,27 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
                 const bool last_use = (n_mt == 1) || w == 1;
                 if (first_use) {
                     ptx::mbar_wait(ptx::smem_u32(&v_full[vslot]), vph);
-                    // rows past the valid tokens of a ragged cached tile hold whatever the pool / the ring held:
-                    // P is exactly 0 there, but 0 * NaN would poison O, so zero them before the MMA reads them.
+                    // rows past the valid tokens of a ragged cached tile hold whatever the pool / the ring held, and the
+                    // last 8-token box of an entry tile reaches into rows of later tokens or of the NEXT session (which
+                    // the caller may never have initialised, e.g. a budget-skipped neighbour): P is exactly 0 there,
+                    // but 0 * NaN would poison O, so zero them before the MMA reads them.
+                    int valid, zero_to;
                     if (t < s.u.n_cached_tiles) {
-                        const int valid = s.u.n_s - t * kTile;
-                        if (valid < kTile) {
-                            uint8_t *vb = v_s + vslot * kTileBytes;
-                            for (int idx = valid * (D / 8) + lane; idx < kTile * (D / 8); idx += 32) {
-                                const int r = idx / (D / 8), c = idx - r * (D / 8);
-                                *reinterpret_cast<uint4 *>(vb + tile_offset<D>(r, c)) = make_uint4(0, 0, 0, 0);
-                            }
-                            ptx::fence_proxy_async_smem();
-                            __syncwarp();
+                        valid = s.u.n_s - t * kTile;
+                        zero_to = kTile;
+                    } else {
+                        valid = s.u.tok0 + s.u.ntok - (t - s.u.n_cached_tiles) * kTile;
+                        zero_to = ((valid + 7) >> 3) << 3;   // the producer zeroed every row no box covers
+                    }
+                    zero_to = zero_to < kTile ? zero_to : kTile;
+                    if (valid < zero_to) {
+                        uint8_t *vb = v_s + vslot * kTileBytes;
+                        for (int idx = valid * (D / 8) + lane; idx < zero_to * (D / 8); idx += 32) {
+                            const int r = idx / (D / 8), c = idx - r * (D / 8);
+                            *reinterpret_cast<uint4 *>(vb + tile_offset<D>(r, c)) = make_uint4(0, 0, 0, 0);
                         }
+                        ptx::fence_proxy_async_smem();
+                        __syncwarp();
                     }
                 }
                 ptx::mbar_wait(ptx::smem_u32(&p_ready[w]), (pph >> w) & 1u);
@@ -536,13 +540,6 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
         const uint32_t lane_addr = static_cast<uint32_t>((warp & 3) << 5) << 16;
         const int st = threadIdx.x - 128;                      // 0..255 among softmax threads
         uint32_t sph = 0, oph = 0;
-#ifdef PREPOS_CTA_TIMES
-        long long tz[8] = {0, 0, 0, 0, 0, 0, 0, 0};
-#define PREPOS_TZ(i) if (st == 0 && tz[i] == 0) asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(tz[i]))
-        PREPOS_TZ(0);
-#else
-#define PREPOS_TZ(i)
-#endif
         SegIter it(p, t0, t1);
         Seg s;
         while (it.next(p, s)) {
@@ -570,7 +567,6 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
                 ptx::mbar_wait(ptx::smem_u32(&s_full[w]), sph);
                 sph ^= 1;
                 ptx::tc_fence_after();
-                PREPOS_TZ(1);
                 // The tile body exists twice (all columns visible / masked at `limit`): one body with a branch
                 // around the masking makes the compiler copy the whole 128-register score row at the join.
                 auto tile_body = [&](auto masked_tag) {
@@ -667,15 +663,17 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
                 have = true;
             }
             // ---- epilogue
-            PREPOS_TZ(2);
             ptx::mbar_wait(ptx::smem_u32(&o_done[w]), oph);
             oph ^= 1;
             ptx::tc_fence_after();
             __nv_bfloat16 *ob = p.a.out + static_cast<size_t>(s.layer) * p.a.out_layer_stride;
             float *slot = p.partials + static_cast<size_t>(2 * blockIdx.x + s.slot) * (kAttnMaxRows * (D + 2));
             if (n_mt == 2) {
-                // stream w owns M-tile w: rows urow, all D columns
-                const float inv = 1.f / l_sum;
+                // stream w owns M-tile w: rows urow, all D columns.  A row that saw no column in this segment (a cut
+                // segment made only of a later entry tile: G = 1 units span two entry tiles) contributes a zero partial
+                // with log-sum-exp -inf, which the merges weigh with 0.
+                const bool seen = l_sum > 0.f;
+                const float inv = seen ? 1.f / l_sum : 0.f;
                 const bool live = urow < rows;
                 const uint32_t oa = tmem + lane_addr + kColO + w * D;
                 __nv_bfloat16 *orow = ob + (static_cast<size_t>(s.u.row0 + my_tok) * p.Hq + s.kvh * G + urow % G) * D;
@@ -684,6 +682,10 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
                     uint32_t o[32];
                     ptx::tmem_ld_32x32b_x32(oa + cb, o);
                     ptx::tmem_ld_wait();
+                    if (!seen) {
+#pragma unroll
+                        for (int c = 0; c < 32; ++c) o[c] = 0u;
+                    }
                     if (live) {
                         if (s.direct) {
 #pragma unroll
@@ -704,7 +706,7 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
                         }
                     }
                 }
-                if (live && !s.direct) slot[kAttnMaxRows * D + urow] = m_used + log2f(l_sum);
+                if (live && !s.direct) slot[kAttnMaxRows * D + urow] = seen ? m_used + log2f(l_sum) : -CUDART_INF_F;
             } else {
                 // both streams hold partial sums of the same rows: exchange (m, l), then WG w finishes columns
                 // [w * D/2, (w+1) * D/2) of the merged row
@@ -716,12 +718,17 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
                 if (w == 0) {
                     const float2 b = ml_x[row];
                     const float M = two ? fmaxf(m_used, b.x) : m_used;
-                    const float wa = exp2f(m_used - M), wb = two ? exp2f(b.x - M) : 0.f;
-                    const float L = wa * l_sum + wb * b.y;
-                    const float inv = 1.f / L;
-                    fa = wa * inv;
-                    fb = wb * inv;
-                    lse2 = M + log2f(L);
+                    if (M == -CUDART_INF_F) {   // the row saw no column in this segment: zero partial, lse -inf
+                        fa = fb = 0.f;
+                        lse2 = -CUDART_INF_F;
+                    } else {
+                        const float wa = exp2f(m_used - M), wb = two ? exp2f(b.x - M) : 0.f;
+                        const float L = wa * l_sum + wb * b.y;
+                        const float inv = 1.f / L;
+                        fa = wa * inv;
+                        fb = wb * inv;
+                        lse2 = M + log2f(L);
+                    }
                     ml_x[row] = make_float2(fa, fb);
                 }
                 ptx::bar_sync(1, 256);
@@ -770,35 +777,30 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
                 ptx::bar_sync(1, 256);  // ml_x is reused by the next segment
             }
             // ---- the single cross-CTA pass: the last CTA to deliver its partial of a cut unit combines them
-            PREPOS_TZ(3);
             if (!s.direct) {
-                // the barrier orders every thread's partial stores before thread 0's release fence + ticket
-                ptx::bar_sync(1, 256);
                 const long long U0s = static_cast<long long>(s.lh) * p.tiles_per_lh + s.u.tile_prefix;
                 const int c0s = cta_of(p, gridDim.x, U0s);
                 const int c1s = cta_of(p, gridDim.x, U0s + s.u.n_tiles - 1);
                 // up to kLastArriverMax partials: the last CTA to arrive combines them right here.  More (a unit spread
-                // over many CTAs, e.g. one launch per layer): every covering CTA combines its share of the rows after
-                // its last segment (cooperative pass below); the ticket is fire-and-forget and nobody waits for it.
-                const bool coop = (c1s - c0s >= kLastArriverMax);
+                // over many CTAs, e.g. one launch per layer): the partials are complete when this kernel ends and
+                // attn_merge_kernel, launched right behind it, combines them -- no ticket, and no CTA ever waits for
+                // another one.
+                if (c1s - c0s >= kLastArriverMax) continue;
+                // the barrier orders every thread's partial stores before thread 0's release fence + ticket
+                ptx::bar_sync(1, 256);
                 if (st == 0) {
                     unsigned int *cnt = p.counters + static_cast<size_t>(s.lh) * p.a.n_units + s.unit_idx;
                     ptx::fence_acq_rel_gpu();
-                    if (coop) {
-                        atomicAdd(cnt, 1u);
-                    } else {
-                        const unsigned int prev = atomicAdd(cnt, 1u);
-                        const bool last = (prev == static_cast<unsigned int>(c1s - c0s));
-                        if (last) {
-                            *cnt = 0u;  // self-reset for the next launch
-                            ptx::fence_acq_rel_gpu();
-                        }
-                        merge_info[0] = last ? c0s : -1;
-                        merge_info[1] = c1s;
-                        merge_info[2] = (cta_begin(p, gridDim.x, c0s) < U0s) ? 1 : 0;  // c0's slot for this unit
+                    const unsigned int prev = atomicAdd(cnt, 1u);
+                    const bool last = (prev == static_cast<unsigned int>(c1s - c0s));
+                    if (last) {
+                        *cnt = 0u;  // self-reset for the next launch
+                        ptx::fence_acq_rel_gpu();
                     }
+                    merge_info[0] = last ? c0s : -1;
+                    merge_info[1] = c1s;
+                    merge_info[2] = (cta_begin(p, gridDim.x, c0s) < U0s) ? 1 : 0;  // c0's slot for this unit
                 }
-                if (coop) continue;
                 ptx::bar_sync(1, 256);
                 const int c0 = merge_info[0], c1 = merge_info[1], c0_slot = merge_info[2];
                 if (c0 >= 0) {
@@ -852,7 +854,7 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
                                 float wsum = 0.f;
 #pragma unroll
                                 for (int j = 0; j < kC_; ++j) {  // CTA order
-                                    const float wgt = (j < nc) ? exp2f(lse[u][j] - M) : 0.f;
+                                    const float wgt = (j < nc && lse[u][j] != -CUDART_INF_F) ? exp2f(lse[u][j] - M) : 0.f;
                                     acc.x = fmaf(wgt, o[u][j].x, acc.x);
                                     acc.y = fmaf(wgt, o[u][j].y, acc.y);
                                     acc.z = fmaf(wgt, o[u][j].z, acc.z);
@@ -865,124 +867,100 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
                     };
                     if (nc <= 2) {
                         merge_pass(std::integral_constant<int, 12>{}, std::integral_constant<int, 2>{});
-                    } else {  // nc <= kLastArriverMax == kMaxC: more partials take the cooperative pass below
+                    } else {  // nc <= kLastArriverMax == kMaxC: more partials are combined by attn_merge_kernel
                         merge_pass(std::integral_constant<int, kU>{}, std::integral_constant<int, kMaxC>{});
                     }
                 }
                 ptx::bar_sync(1, 256);  // merge_info is reused by the next segment
             }
         }
-        PREPOS_TZ(4);
-        // ---- cooperative cross-CTA pass for units spread over more than kLastArriverMax CTAs: this CTA has delivered
-        // all its partials (so no CTA ever waits for one that is itself waiting), now for each such unit it waits
-        // until every covering CTA has delivered, combines ITS share of the unit's rows from all partials in CTA
-        // order, and checks out; the last CTA to check out resets the counter.  All CTAs of the grid are resident
-        // (grid <= SM count, one CTA per SM), so the wait is for CTAs that are running.
-        {
-            SegIter it2(p, t0, t1);
-            Seg s2;
-            while (it2.next(p, s2)) {
-                if (s2.direct) continue;
-                const long long U0 = static_cast<long long>(s2.lh) * p.tiles_per_lh + s2.u.tile_prefix;
-                const int c0 = cta_of(p, gridDim.x, U0);
-                const int c1 = cta_of(p, gridDim.x, U0 + s2.u.n_tiles - 1);
-                const int nc = c1 - c0 + 1;
-                if (nc <= kLastArriverMax) continue;
-                unsigned int *cnt = p.counters + static_cast<size_t>(s2.lh) * p.a.n_units + s2.unit_idx;
-                if (st == 0) {
-                    while (ptx::ld_acquire_gpu(cnt) < static_cast<unsigned int>(nc)) __nanosleep(64);
-                }
-                ptx::bar_sync(1, 256);
-                PREPOS_TZ(5);
-                constexpr int kVec = D / 4;
-                constexpr int kCB = 20;  // partials loaded together: one round trip for a unit spread over <= 20 CTAs
-                constexpr size_t kSlotFloats = static_cast<size_t>(kAttnMaxRows) * (D + 2);
-                const int c0_slot = (cta_begin(p, gridDim.x, c0) < U0) ? 1 : 0;
-                const int rows = s2.u.ntok * G;
-                const int j = static_cast<int>(blockIdx.x) - c0;
-                const int r_lo = static_cast<int>(static_cast<long long>(rows) * j / nc);
-                const int r_hi = static_cast<int>(static_cast<long long>(rows) * (j + 1) / nc);
-                __nv_bfloat16 *ob = p.a.out + static_cast<size_t>(s2.layer) * p.a.out_layer_stride;
-                const int n_r = r_hi - r_lo;
-                for (int idx = st; idx < n_r * kVec; idx += 256) {
-                    const int v = idx / n_r, r = r_lo + (idx - v * n_r);   // lanes run along the rows
-                    float M = -CUDART_INF_F, wsum = 0.f;
-                    float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
-                    for (int cb = 0; cb < nc; cb += kCB) {
-                        float lse[kCB];
-                        float4 o[kCB];
-#pragma unroll
-                        for (int q = 0; q < kCB; ++q) {
-                            const int c = c0 + cb + q;
-                            lse[q] = -CUDART_INF_F;
-                            o[q] = make_float4(0.f, 0.f, 0.f, 0.f);
-                            if (cb + q < nc) {
-                                const float *sl = p.partials + (2 * static_cast<size_t>(c) + (c == c0 ? c0_slot : 0)) * kSlotFloats;
-                                lse[q] = __ldcg(sl + kAttnMaxRows * D + r);
-                                o[q] = __ldcg(reinterpret_cast<const float4 *>(sl) + static_cast<size_t>(v) * kAttnMaxRows + r);
-                            }
-                        }
-                        float mc = lse[0];
-#pragma unroll
-                        for (int q = 1; q < kCB; ++q) mc = fmaxf(mc, lse[q]);
-                        const float Mn = fmaxf(M, mc);
-                        const float resc = (M == -CUDART_INF_F) ? 0.f : exp2f(M - Mn);
-                        acc.x *= resc;
-                        acc.y *= resc;
-                        acc.z *= resc;
-                        acc.w *= resc;
-                        wsum *= resc;
-                        M = Mn;
-#pragma unroll
-                        for (int q = 0; q < kCB; ++q) {  // CTA order
-                            const float wgt = (cb + q < nc) ? exp2f(lse[q] - M) : 0.f;
-                            acc.x = fmaf(wgt, o[q].x, acc.x);
-                            acc.y = fmaf(wgt, o[q].y, acc.y);
-                            acc.z = fmaf(wgt, o[q].z, acc.z);
-                            acc.w = fmaf(wgt, o[q].w, acc.w);
-                            wsum += wgt;
-                        }
-                    }
-                    const float inv = 1.f / wsum;
-                    const int tok = s2.u.tok0 + r / G, h = s2.kvh * G + r % G;
-                    uint2 pk;
-                    pk.x = pack_bf16(acc.x * inv, acc.y * inv);
-                    pk.y = pack_bf16(acc.z * inv, acc.w * inv);
-                    *reinterpret_cast<uint2 *>(ob + (static_cast<size_t>(s2.u.row0 + tok) * p.Hq + h) * D + v * 4) = pk;
-                }
-                ptx::bar_sync(1, 256);
-                if (st == 0) {
-                    ptx::fence_acq_rel_gpu();
-                    const unsigned int prev = atomicAdd(cnt, 1u);
-                    if (prev == static_cast<unsigned int>(2 * nc - 1)) *cnt = 0u;  // everyone has checked out
-                }
-                PREPOS_TZ(6);
-            }
-        }
-#ifdef PREPOS_CTA_TIMES
-        if (st == 0)
-            printf("TZ cta %d first_s %lld items %lld wait_o+epi %lld ticket %lld spin %lld merge %lld\n", blockIdx.x, tz[1] - tz[0],
-                   tz[2] - tz[1], tz[3] - tz[2], tz[4] - tz[3], tz[5] - tz[4], tz[6] - tz[5]);
-#endif
     }
 
     ptx::tc_fence_before();
     __syncthreads();
     if (warp == 2) ptx::tmem_dealloc<512>(tmem);
-#ifdef PREPOS_CTA_TIMES
-    if (threadIdx.x == 0) {
-        long long dbg_t1;
-        asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(dbg_t1));
-        int nseg = 0, ncut = 0;
-        SegIter it(p, t0, t1);
-        Seg s;
-        while (it.next(p, s)) {
-            ++nseg;
-            ncut += !s.direct;
+}
+
+// The cross-CTA pass of units spread over more than kLastArriverMax CTAs (a launch with few units and many CTAs: one
+// launch per layer, a single long session), as its own launch right behind the attention kernel.  Its
+// griddepcontrol.wait returns when that kernel has ended, so every partial is complete: no ticket, no CTA waiting for
+// another one (the in-kernel form of this pass spun on co-residency that an ordinary launch does not guarantee).  One
+// CTA = 32 rows x 4 float4 columns of one unit: a warp's lanes run along the rows of one float4 column (512
+// contiguous bytes of a partial), partials are combined in CTA order with kCB loads in flight per thread.
+template <int D>
+__global__ void __launch_bounds__(128) attn_merge_kernel(const UmmaParams p, int attn_grid)
+{
+    ptx::griddep_launch();
+    ptx::griddep_wait();
+    constexpr int kVec = D / 4;
+    constexpr int kRowBlks = kAttnMaxRows / 32, kColBlks = kVec / 4;
+    constexpr int kCB = 8;
+    constexpr size_t kSlotFloats = static_cast<size_t>(kAttnMaxRows) * (D + 2);
+    const int G = p.Hq / p.Hkv;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const long long n_items = static_cast<long long>(p.n_lh) * p.a.n_units * (kRowBlks * kColBlks);
+    for (long long item = blockIdx.x; item < n_items; item += gridDim.x) {
+        const int sub = static_cast<int>(item % (kRowBlks * kColBlks));
+        const long long lu = item / (kRowBlks * kColBlks);
+        const int ui = static_cast<int>(lu % p.a.n_units), lh = static_cast<int>(lu / p.a.n_units);
+        const int rb = sub / kColBlks, v = (sub % kColBlks) * 4 + warp;
+        const AttnUnit u = p.units[ui];
+        const int rows = u.ntok * G;
+        if (rb * 32 >= rows) continue;
+        const long long U0 = static_cast<long long>(lh) * p.tiles_per_lh + u.tile_prefix;
+        const int c0 = cta_of(p, attn_grid, U0), c1 = cta_of(p, attn_grid, U0 + u.n_tiles - 1);
+        const int nc = c1 - c0 + 1;
+        if (nc <= kLastArriverMax) continue;   // combined inside the attention kernel
+        const int r = rb * 32 + lane;
+        if (r >= rows) continue;
+        const int c0_slot = (cta_begin(p, attn_grid, c0) < U0) ? 1 : 0;
+        float M = -CUDART_INF_F, wsum = 0.f;
+        float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
+        for (int cb = 0; cb < nc; cb += kCB) {
+            float lse[kCB];
+            float4 o[kCB];
+#pragma unroll
+            for (int q = 0; q < kCB; ++q) {
+                lse[q] = -CUDART_INF_F;
+                o[q] = make_float4(0.f, 0.f, 0.f, 0.f);
+                if (cb + q < nc) {
+                    const int c = c0 + cb + q;
+                    const float *sl = p.partials + (2 * static_cast<size_t>(c) + (c == c0 ? c0_slot : 0)) * kSlotFloats;
+                    lse[q] = __ldcg(sl + kAttnMaxRows * D + r);
+                    o[q] = __ldcg(reinterpret_cast<const float4 *>(sl) + static_cast<size_t>(v) * kAttnMaxRows + r);
+                }
+            }
+            float mc = lse[0];
+#pragma unroll
+            for (int q = 1; q < kCB; ++q) mc = fmaxf(mc, lse[q]);
+            const float Mn = fmaxf(M, mc);
+            if (Mn == -CUDART_INF_F) continue;   // nothing seen so far
+            const float resc = (M == -CUDART_INF_F) ? 0.f : exp2f(M - Mn);
+            acc.x *= resc;
+            acc.y *= resc;
+            acc.z *= resc;
+            acc.w *= resc;
+            wsum *= resc;
+            M = Mn;
+#pragma unroll
+            for (int q = 0; q < kCB; ++q) {  // CTA order
+                const float wgt = (lse[q] == -CUDART_INF_F) ? 0.f : exp2f(lse[q] - M);
+                acc.x = fmaf(wgt, o[q].x, acc.x);
+                acc.y = fmaf(wgt, o[q].y, acc.y);
+                acc.z = fmaf(wgt, o[q].z, acc.z);
+                acc.w = fmaf(wgt, o[q].w, acc.w);
+                wsum += wgt;
+            }
         }
-        printf("CTA %d start %lld dur %lld tiles %lld nseg %d ncut %d\n", blockIdx.x, dbg_t0, dbg_t1 - dbg_t0, t1 - t0, nseg, ncut);
+        const float inv = 1.f / wsum;
+        const int layer = p.a.layer_begin + lh / p.Hkv, kvh = lh % p.Hkv;
+        const int tok = u.tok0 + r / G, h = kvh * G + r % G;
+        __nv_bfloat16 *ob = p.a.out + static_cast<size_t>(layer) * p.a.out_layer_stride;
+        uint2 pk;
+        pk.x = pack_bf16(acc.x * inv, acc.y * inv);
+        pk.y = pack_bf16(acc.z * inv, acc.w * inv);
+        *reinterpret_cast<uint2 *>(ob + (static_cast<size_t>(u.row0 + tok) * p.Hq + h) * D + v * 4) = pk;
     }
-#endif
 }
 
 typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
@@ -1107,8 +1085,9 @@ int launch(prepos_ctx *ctx, const AttnArgs &a, int tiles_per_lh, cudaStream_t st
     }
     // Fewer units than CTAs (one launch per layer: 8 kv heads for 148 CTAs): give every unit a whole number of CTAs,
     // in proportion to its tiles, and cut it evenly among them.  No CTA then straddles two units (one segment, one
-    // epilogue per CTA) and the CTAs of a unit finish together, which is what its cooperative merge waits for.
+    // epilogue per CTA) and the CTAs of a unit finish together.
     p.use_bnd = 0;
+    long long n_wide_bnd = 0;   // units given more than kLastArriverMax CTAs by the table below
     {
         const long long n_units_total = static_cast<long long>(p.n_lh) * a.n_units;
         if (n_units_total < grid && p.total_tiles < (1ll << 30)) {
@@ -1137,8 +1116,10 @@ int launch(prepos_ctx *ctx, const AttnArgs &a, int tiles_per_lh, cudaStream_t st
             }
             if (used == grid) {
                 int c = 0;
-                for (int i = 0; i < n; ++i)
+                for (int i = 0; i < n; ++i) {
                     for (int j = 0; j < k[i]; ++j) p.bnd[c++] = static_cast<int>(start[i] + tiles[i] * j / k[i]);
+                    n_wide_bnd += (k[i] > kLastArriverMax);
+                }
                 p.bnd[c] = static_cast<int>(p.total_tiles);
                 p.use_bnd = 1;
             }
@@ -1174,11 +1155,36 @@ int launch(prepos_ctx *ctx, const AttnArgs &a, int tiles_per_lh, cudaStream_t st
     }
     if (static_cast<size_t>(p.n_lh) * a.n_units > ctx->attn_counters_n) return PREPOS_E_WORKSPACE;
     p.counters = ctx->attn_counters;
+    // units spread over more than kLastArriverMax CTAs are combined by attn_merge_kernel behind the attention kernel
+    long long merge_units = 0;
+    if (p.use_bnd) {
+        merge_units = n_wide_bnd;
+    } else {
+        const long long m = p.total_tiles / grid;   // shortest CTA range
+        long long max_n = 0;
+        for (const AttnUnit &u : ctx->plan_units) max_n = u.n_tiles > max_n ? u.n_tiles : max_n;
+        if ((max_n - 1 + m - 1) / m + 1 > kLastArriverMax) {
+            auto cta_of_h = [&](long long t) { return ((t + 1) * grid + p.total_tiles - 1) / p.total_tiles - 1; };
+            for (int lh = 0; lh < p.n_lh; ++lh)
+                for (const AttnUnit &u : ctx->plan_units) {
+                    const long long U0 = static_cast<long long>(lh) * tiles_per_lh + u.tile_prefix;
+                    merge_units += (cta_of_h(U0 + u.n_tiles - 1) - cta_of_h(U0) >= kLastArriverMax);
+                }
+        }
+    }
     PREPOS_CUDA_TRY(cudaFuncSetAttribute(attn_umma_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                          static_cast<int>(smem)));
     PREPOS_CUDA_TRY(prepos_launch_pdl(attn_umma_kernel<D>, dim3(static_cast<unsigned>(grid)), dim3(kThreads), smem, stream,
                                       ctx->tm_k, ctx->tm_v, ctx->tm_kn, ctx->tm_vn, ctx->tm_q, p));
     ctx->launches += 1;
+    if (merge_units > 0) {
+        long long mg = merge_units * (kAttnMaxRows / 32) * (D / 16);
+        const long long cap = static_cast<long long>(ctx->num_sms) * 4;
+        mg = mg > cap ? cap : mg;
+        PREPOS_CUDA_TRY(prepos_launch_pdl(attn_merge_kernel<D>, dim3(static_cast<unsigned>(mg)), dim3(128), 0, stream, p,
+                                          static_cast<int>(grid)));
+        ctx->launches += 1;
+    }
     return PREPOS_OK;
 }
 

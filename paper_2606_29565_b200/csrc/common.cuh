@@ -123,7 +123,7 @@ struct prepos_ctx {
 int prepos_launch_ready_dist(prepos_ctx *ctx, int n, const int32_t *session_ids, const __nv_bfloat16 *hidden,
                              const __nv_bfloat16 *w, const int64_t *position_p, const uint64_t *entry_hash,
                              const int32_t *skip_mask, prepos_record *records, const uint64_t *session_version,
-                             float *logits_out, cudaStream_t stream);
+                             const uint64_t *expected_version, float *logits_out, cudaStream_t stream);
 int prepos_launch_scan_logits(prepos_ctx *ctx, int n, const float *logits, prepos_record *out, cudaStream_t stream);
 int prepos_launch_gate_serve(prepos_ctx *ctx, int n, const int32_t *session_ids, const uint64_t *req_hash,
                              const prepos_record *records, const uint64_t *session_version,

@@ -6,12 +6,19 @@
 
 namespace {
 
-// Alg. 2 for one request.  The record is read as three 16-byte words; the version compare is the
-// authority for staleness (reading Q11), the VALID bit is redundant with it.
+__device__ __forceinline__ uint4 ld_relaxed_v4(const uint4 *p)
+{
+    uint4 v;
+    asm volatile("ld.relaxed.gpu.global.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "l"(p) : "memory");
+    return v;
+}
+
+// Alg. 2 for one request.  The version compare is the authority for staleness (reading Q11), the VALID
+// bit is redundant with it.
 __global__ void __launch_bounds__(128) gate_serve_kernel(int n, const int32_t *__restrict__ session_ids,
                                                          const uint64_t *__restrict__ req_hash,
-                                                         const prepos_record *__restrict__ records,
-                                                         const uint64_t *__restrict__ session_version,
+                                                         const prepos_record *records,
+                                                         const uint64_t *session_version,
                                                          const uint32_t *__restrict__ bitmap, int vocab, float tau,
                                                          int strict_gt, int32_t *__restrict__ decision,
                                                          int32_t *__restrict__ token)
@@ -21,20 +28,29 @@ __global__ void __launch_bounds__(128) gate_serve_kernel(int n, const int32_t *_
     const int r = blockIdx.x * blockDim.x + threadIdx.x;
     if (r >= n) return;
     const int sid = session_ids[r];
+    // Reader side of the publication protocol (include/prepos.h "Record publication"): the record may be re-published
+    // or invalidated on another stream while this serve runs.  Word 1 (gap, flags + sequence, version) is read before
+    // and after the payload words; if the two reads differ a publication was in progress and the request falls
+    // through.  The live version is read last: a record is served only if it was computed at the version that is
+    // live after its fields were read (Sec. 3.6).
     const uint4 *p = reinterpret_cast<const uint4 *>(records + sid);
-    const uint4 w0 = p[0];  // max_logit, lse, top1, top2
-    const uint4 w1 = p[1];  // gap, flags, version
-    const uint4 w2 = p[2];  // entry_hash, position
+    const uint4 w1a = ld_relaxed_v4(p + 1);  // gap, flags, version
+    ptx::fence_acq_rel_gpu();
+    const uint4 w0 = ld_relaxed_v4(p);       // max_logit, lse, top1, top2
+    const uint4 w2 = ld_relaxed_v4(p + 2);   // entry_hash, position
+    ptx::fence_acq_rel_gpu();
+    const uint4 w1 = ld_relaxed_v4(p + 1);
+    const bool torn = (w1a.x != w1.x) | (w1a.y != w1.y) | (w1a.z != w1.z) | (w1a.w != w1.w);
     const int32_t top1 = static_cast<int32_t>(w0.z);
     const float gap = __uint_as_float(w1.x);
     const uint32_t flags = w1.y;
     const uint64_t rec_version = (static_cast<uint64_t>(w1.w) << 32) | w1.z;
     const uint64_t rec_hash = (static_cast<uint64_t>(w2.y) << 32) | w2.x;
-    const uint64_t live = session_version[sid];
+    const uint64_t live = *reinterpret_cast<const volatile uint64_t *>(session_version + sid);
     const uint64_t rh = req_hash ? req_hash[r] : 0ull;
 
     int dec;
-    if (!(flags & PREPOS_FLAG_VALID) || (flags & PREPOS_FLAG_NONFINITE) || rec_version != live) {
+    if (torn || !(flags & PREPOS_FLAG_VALID) || (flags & PREPOS_FLAG_NONFINITE) || rec_version != live) {
         dec = PREPOS_STALE_OR_INVALID;  // Alg. 2 l.1-2
     } else if (rec_hash != 0ull && rh != 0ull && rec_hash != rh) {
         dec = PREPOS_INELIGIBLE;  // Alg. 2 l.1-2, realised entry != pre-positioned entry

@@ -141,6 +141,48 @@ __device__ __forceinline__ void write_record_fields(prepos_record *rec, const To
     rec->gap = (t.i2 == 0x7fffffff) ? CUDART_INF_F : t.v1 - t.v2;
 }
 
+struct RdParams {
+    int n;  // hidden rows in this pass (<= kNB)
+    int H, V;
+    int n_stages;
+    int x_rows;  // rows of the smem hidden block (n+1 with a trailing zero row, or 8)
+    const __nv_bfloat16 *hidden;  // [n][H]
+    const int32_t *session_ids;   // [n]
+    const int64_t *position_p;
+    const uint64_t *entry_hash;
+    const int32_t *skip_mask;
+    prepos_record *records;
+    const uint64_t *session_version;
+    const uint64_t *expected_version;  // [n] or null
+    float *logits_out;  // [n][V] or null
+    RdPartial *partials;
+    unsigned int *counter;
+};
+
+// Alg. 1 l.10-12 for one session: publishes the record so that a gate serve on ANOTHER stream never pairs fields of
+// two different publications (protocol in include/prepos.h "Record publication"): the upper 30 bits of `flags` are a
+// sequence number.  (1) flags <- new sequence, VALID clear; fence; (2) payload incl. the version stamp; fence;
+// (3) flags <- sequence | VALID.  The stamp is the version the caller computed the hidden row at (`expected`), and
+// the record is made VALID only if that still is the live version (Sec. 3.6: a state mutation that commits while the
+// pre-position is running must win); without `expected` the live version at this moment is stamped (same-stream use).
+__device__ __forceinline__ void publish_record(const RdParams &p, int row, const Top2Lse &t)
+{
+    const int sid = p.session_ids[row];
+    prepos_record *rec = p.records + sid;
+    volatile uint32_t *fl = &rec->flags;
+    const uint32_t seq = ((*fl >> 2) + 1u) << 2;
+    *fl = seq;
+    __threadfence();
+    const uint64_t live = *reinterpret_cast<const volatile uint64_t *>(p.session_version + sid);
+    const uint64_t stamp = p.expected_version ? p.expected_version[row] : live;
+    write_record_fields(rec, t);
+    rec->entry_hash = p.entry_hash ? p.entry_hash[row] : 0ull;
+    rec->position = p.position_p ? p.position_p[row] : 0ll;
+    rec->version = stamp;
+    __threadfence();
+    *fl = seq | (stamp == live ? PREPOS_FLAG_VALID : 0u) | (t.nonfinite ? PREPOS_FLAG_NONFINITE : 0u);
+}
+
 // Merge `n_parts` per-CTA partials of row `row` (partials[row * kMaxRdPartials + c]) in CTA order with one
 // warp; result valid in lane 0.
 __device__ __forceinline__ Top2Lse merge_partials_warp(const RdPartial *partials, int row, int n_parts, int lane)
@@ -164,22 +206,6 @@ __device__ __forceinline__ Top2Lse merge_partials_warp(const RdPartial *partials
     return acc;
 }
 
-struct RdParams {
-    int n;  // hidden rows in this pass (<= kNB)
-    int H, V;
-    int n_stages;
-    int x_rows;  // rows of the smem hidden block (n+1 with a trailing zero row, or 8)
-    const __nv_bfloat16 *hidden;  // [n][H]
-    const int32_t *session_ids;   // [n]
-    const int64_t *position_p;
-    const uint64_t *entry_hash;
-    const int32_t *skip_mask;
-    prepos_record *records;
-    const uint64_t *session_version;
-    float *logits_out;  // [n][V] or null
-    RdPartial *partials;
-    unsigned int *counter;
-};
 
 // The single cross-CTA pass: the last CTA to arrive merges the per-CTA partials of every hidden row in CTA order
 // and writes the records (Alg. 1 l.10-12: position, dist (here: argmax, gamma, max, lse), decoded/valid).
@@ -196,16 +222,7 @@ __device__ __forceinline__ void finalize_records(const RdParams &p, int warp, in
     __threadfence();
     for (int row = warp; row < p.n; row += n_warps) {
         const Top2Lse t = merge_partials_warp(p.partials, row, gridDim.x, lane);
-        if (lane == 0 && !(p.skip_mask && p.skip_mask[row])) {
-            const int sid = p.session_ids[row];
-            prepos_record *rec = p.records + sid;
-            write_record_fields(rec, t);
-            rec->entry_hash = p.entry_hash ? p.entry_hash[row] : 0ull;
-            rec->position = p.position_p ? p.position_p[row] : 0ll;
-            rec->version = p.session_version[sid];
-            __threadfence();  // payload before the valid bit
-            rec->flags = PREPOS_FLAG_VALID | (t.nonfinite ? PREPOS_FLAG_NONFINITE : 0u);
-        }
+        if (lane == 0 && !(p.skip_mask && p.skip_mask[row])) publish_record(p, row, t);
     }
     if (threadIdx.x == 0) *p.counter = 0u;  // self-reset for the next launch on this stream
 }
@@ -541,16 +558,7 @@ __global__ void __launch_bounds__(32) rd_finalize_kernel(const RdParams p, int n
     ptx::griddep_launch();
     const int row = blockIdx.x, lane = threadIdx.x;
     const Top2Lse t = merge_partials_warp(p.partials, row, n_parts, lane);
-    if (lane == 0 && !(p.skip_mask && p.skip_mask[row])) {
-        const int sid = p.session_ids[row];
-        prepos_record *rec = p.records + sid;
-        write_record_fields(rec, t);
-        rec->entry_hash = p.entry_hash ? p.entry_hash[row] : 0ull;
-        rec->position = p.position_p ? p.position_p[row] : 0ll;
-        rec->version = p.session_version[sid];
-        __threadfence();  // payload before the valid bit
-        rec->flags = PREPOS_FLAG_VALID | (t.nonfinite ? PREPOS_FLAG_NONFINITE : 0u);
-    }
+    if (lane == 0 && !(p.skip_mask && p.skip_mask[row])) publish_record(p, row, t);
 }
 
 // ---- a4': scan of stored fp32 logits ---------------------------------------------------------------
@@ -622,7 +630,7 @@ typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t
 int prepos_launch_ready_dist(prepos_ctx *ctx, int n, const int32_t *session_ids, const __nv_bfloat16 *hidden,
                              const __nv_bfloat16 *w, const int64_t *position_p, const uint64_t *entry_hash,
                              const int32_t *skip_mask, prepos_record *records, const uint64_t *session_version,
-                             float *logits_out, cudaStream_t stream)
+                             const uint64_t *expected_version, float *logits_out, cudaStream_t stream)
 {
     const int H = ctx->shape.hidden, V = ctx->shape.vocab;
     EncodeTiledFn encode = reinterpret_cast<EncodeTiledFn>(prepos_get_encode_tiled());
@@ -666,6 +674,7 @@ int prepos_launch_ready_dist(prepos_ctx *ctx, int n, const int32_t *session_ids,
             p.skip_mask = skip_mask ? skip_mask + r0 : nullptr;
             p.records = records;
             p.session_version = session_version;
+            p.expected_version = expected_version ? expected_version + r0 : nullptr;
             p.logits_out = logits_out ? logits_out + static_cast<size_t>(r0) * V : nullptr;
             p.partials = ctx->rd_partials;
             p.counter = ctx->rd_counter;
@@ -697,6 +706,7 @@ int prepos_launch_ready_dist(prepos_ctx *ctx, int n, const int32_t *session_ids,
         p.skip_mask = skip_mask ? skip_mask + r0 : nullptr;
         p.records = records;
         p.session_version = session_version;
+        p.expected_version = expected_version ? expected_version + r0 : nullptr;
         p.logits_out = logits_out ? logits_out + static_cast<size_t>(r0) * V : nullptr;
         p.partials = ctx->rd_partials;
         p.counter = ctx->rd_counter;

@@ -18,7 +18,7 @@ _SO = os.path.join(_HERE, "libprepos.so")
 OK, SKIPPED_BUDGET = 0, 1
 E_INVALID_ARG, E_SHAPE, E_ALIGN, E_CUDA, E_WORKSPACE, E_NO_DEVICE = -1, -2, -3, -4, -5, -6
 SERVED, GAP_BELOW_TAU, NOT_IN_FAST_SET, STALE_OR_INVALID, INELIGIBLE = 0, 1, 2, 3, 4
-FLAG_VALID, FLAG_NONFINITE = 1, 2
+FLAG_VALID, FLAG_NONFINITE, FLAG_MASK = 1, 2, 3
 RECORD_BYTES = 48
 
 EXPORTS = [
@@ -71,7 +71,7 @@ def lib() -> C.CDLL:
         L.prepos_entry_attn.argtypes = [vp, i32, i32, i32, vp, i64, vp, vp, i64, vp, vp, i64, i64, vp, i32, vp, vp, vp,
                                         vp, i64, vp, f32, vp]
         L.prepos_ready_dist.restype = i32
-        L.prepos_ready_dist.argtypes = [vp, i32, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp]
+        L.prepos_ready_dist.argtypes = [vp, i32, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp]
         L.prepos_scan_logits.restype = i32
         L.prepos_scan_logits.argtypes = [vp, i32, vp, vp, vp]
         L.prepos_gate_serve.restype = i32
@@ -134,7 +134,8 @@ def unpack_records(records: torch.Tensor) -> dict:
     i = r.view(torch.int32).view(-1, 12)
     q = r.view(torch.int64).view(-1, 6)
     return {"max_logit": f[:, 0].clone(), "lse": f[:, 1].clone(), "top1": i[:, 2].clone(), "top2": i[:, 3].clone(),
-            "gap": f[:, 4].clone(), "flags": i[:, 5].clone(), "version": q[:, 3].clone(),
+            "gap": f[:, 4].clone(), "flags": i[:, 5] & FLAG_MASK, "seq": (i[:, 5] >> 2) & 0x3FFFFFFF,
+            "version": q[:, 3].clone(),
             "entry_hash": q[:, 4].clone(), "position": q[:, 5].clone()}
 
 
@@ -217,14 +218,14 @@ class Context:
         return status.tolist()
 
     def ready_dist(self, session_ids, hidden, w_vocab, records, session_version, position_p=None, entry_hash=None,
-                   skip_mask=None, logits_out=None):
+                   skip_mask=None, logits_out=None, expected_version=None):
         """prepos_ready_dist.  All tensors on the device."""
         assert hidden.dtype == torch.bfloat16 and w_vocab.dtype == torch.bfloat16
         assert session_ids.dtype == torch.int32 and session_version.dtype == torch.int64
         n = session_ids.numel()
         _check(lib().prepos_ready_dist(self._h, n, _p(session_ids), _p(hidden), _p(w_vocab), _p(position_p),
                                        _p(entry_hash), _p(skip_mask), _p(records), _p(session_version),
-                                       _p(logits_out), _stream()), "prepos_ready_dist")
+                                       _p(expected_version), _p(logits_out), _stream()), "prepos_ready_dist")
 
     def scan_logits(self, logits, records_out):
         assert logits.dtype == torch.float32 and logits.is_contiguous()

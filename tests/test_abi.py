@@ -78,7 +78,7 @@ def test_fails_loudly_without_device(lib):
     assert st == prepos.E_NO_DEVICE and not h.value
     # compute entry points reject a null ctx instead of computing anything
     assert lib.prepos_gate_serve(None, 1, None, None, None, None, None, 3.0, 0, None, None, None) == prepos.E_INVALID_ARG
-    assert lib.prepos_ready_dist(None, 1, None, None, None, None, None, None, None, None, None, None) == prepos.E_INVALID_ARG
+    assert lib.prepos_ready_dist(None, 1, None, None, None, None, None, None, None, None, None, None, None) == prepos.E_INVALID_ARG
 
 
 def test_product_never_imports_oracle():
