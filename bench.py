@@ -11,10 +11,11 @@ sessions, every stage through the C ABI of libprepos (ctypes binding, paper_2606
     prepos_ready_dist   LM head at the last entry position fused with the vocabulary reduction (a3-a4)
     prepos_gate_serve   the request(s) that arrive next are answered from the cached record (a5)
 
-The default workload is BASELINE.json configs[1] (Llama-3-8B-shaped single streaming session:
-32 layers, 32/8 heads, d=128, page 16, n_s=4096, L_entry=24, H=4096, V=128256).  It prints ONE JSON
-line; see DESIGN.md "Measurement" for every field.  `--impl reference` times the CPU oracle (oracle/)
-on a bounded sample of the same workload instead.
+Without --config it runs ALL FIVE BASELINE.json configs and prints ONE JSON line: the top-level fields are
+those of the headline workload, configs[4] (70B-shaped: the paper's measured model class, and the
+largest per-session pass: 7.56 GB), and `per_config` carries the same fields for c1..c4.  --config cN runs that one
+config alone (what the ncu captures under profiles/ use).  See DESIGN.md "Measurement" for every field.
+`--impl reference` times the CPU oracle (oracle/) on a bounded sample of the headline workload instead.
 """
 from __future__ import annotations
 
@@ -39,6 +40,9 @@ from paper_2606_29565_b200 import synth
 METRIC = "prepos_entry_us_per_session"
 UNIT = "us/session"
 L2_BYTES = 126 << 20
+HEADLINE = "c5"
+ALL_CONFIGS = ["c1", "c2", "c3", "c4", "c5"]
+DEFAULT_STEPS = {"c1": (200, 20), "c2": (100, 10), "c3": (40, 5), "c4": (10, 3), "c5": (40, 5)}
 
 
 # ----------------------------------------------------------------------------------------------------
@@ -90,16 +94,25 @@ def attention_flops(spec):
     return f * s.layers
 
 
-# DRAM bytes (dram__bytes_read.sum + dram__bytes_write.sum) of ONE launch of the dominant kernel, from the committed
-# `ncu --set full` captures (profiles/r01_ncu_full_final.md); None where no capture of that workload exists.
-NCU_TRAFFIC = {
-    ("c2", "entry_attn"): 546446000 + 7390976,
-    ("c2", "ready_dist"): 1050731000 + 3634432,
-    ("c3", "ready_dist"): 1050731000 + 3634432,   # same launch (V, H) as c2
-    ("c4", "entry_attn"): 71075900000 + 1660029000,
-    ("c4", "ready_dist"): 1051261000 + 3196000,
-    ("c5", "entry_attn"): 5424376000 + 56912384,
-}
+def ncu_traffic(config, kernel):
+    """DRAM bytes (dram__bytes_read.sum + dram__bytes_write.sum) of ONE launch of `kernel` on `config`, from the
+    committed summary of the `ncu --set full` captures, profiles/ncu_traffic.csv (columns: config, kernel,
+    dram_read_bytes, dram_write_bytes, capture = the .md under profiles/ that documents the command, commit).  It is a
+    measurement of THAT capture, not of this run: the source is returned with it.  (None, None) without a row."""
+    path = os.path.join(ROOT, "profiles", "ncu_traffic.csv")
+    if not os.path.exists(path):
+        return None, None
+    best = None
+    with open(path) as f:
+        for ln in f:
+            parts = [x.strip() for x in ln.split(",")]
+            if len(parts) < 6 or parts[0].startswith("#") or parts[0] == "config":
+                continue
+            if parts[0] == config and parts[1] == kernel:
+                best = parts            # the last row wins (newest capture)
+    if best is None:
+        return None, None
+    return int(float(best[2])) + int(float(best[3])), f"profiles/{best[4]}@{best[5]}"
 
 
 def peaks():
@@ -279,10 +292,12 @@ def run_device_timed(wl, steps, warmup, dist_ctx):
                 flush.fill_(i & 0xFF)
             wl.step(warmup + steps + i, evs[i])
         torch.cuda.synchronize()
-    calls = {name: statistics.fmean(e[a].elapsed_time(e[b]) for e in evs)
-             for name, a, b in (("invalidate", 0, 1), ("entry_attn", 1, 2), ("ready_dist", 2, 3), ("gate_serve", 3, 4))}
-    return dict(total_ms=total_ms, per_step=per_step, calls=calls, launches=launches, wall_s=wall, clocks=clk.summary(),
-                clocks_per_call_pass=clk_b.summary())
+    spans = (("invalidate", 0, 1), ("entry_attn", 1, 2), ("ready_dist", 2, 3), ("gate_serve", 3, 4))
+    calls = {name: statistics.fmean(e[a].elapsed_time(e[b]) for e in evs) for name, a, b in spans}
+    calls_median = {name: statistics.median(e[a].elapsed_time(e[b]) for e in evs) for name, a, b in spans}
+    calls_min = {name: min(e[a].elapsed_time(e[b]) for e in evs) for name, a, b in spans}
+    return dict(total_ms=total_ms, per_step=per_step, calls=calls, calls_median=calls_median, calls_min=calls_min,
+                launches=launches, wall_s=wall, clocks=clk.summary(), clocks_per_call_pass=clk_b.summary())
 
 
 def run_e2e(wl, steps, warmup, dist_ctx):
@@ -708,26 +723,211 @@ class Dist:
             self.dist.destroy_process_group()
 
 
+def run_graph_replay(wl, replays=24):
+    """SURVEY.md 8(d) timing protocol: the whole per-session pass (the four calls of a step) captured once per resident
+    set into a CUDA graph and replayed, CUDA events around every replay: median and min over `replays` (>= 20).
+    c1 flushes L2 before every replay."""
+    flush = torch.empty(2 * L2_BYTES, dtype=torch.uint8, device=wl.dev) if wl.spec["flush_l2"] else None
+    try:
+        graphs = []
+        side = torch.cuda.Stream()
+        for k in range(len(wl.sets)):
+            g = torch.cuda.CUDAGraph()
+            side.wait_stream(torch.cuda.current_stream())
+            with torch.cuda.graph(g, stream=side):
+                wl.step(k)
+            graphs.append(g)
+        torch.cuda.current_stream().wait_stream(side)
+        ev = []
+        for i in range(replays + 3):
+            if flush is not None:
+                flush.fill_(i & 0xFF)
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            graphs[i % len(graphs)].replay()
+            e1.record()
+            ev.append((e0, e1))
+        torch.cuda.synchronize()
+        us = sorted(a.elapsed_time(b) * 1e3 / wl.n for a, b in ev[3:])
+        return {"replays": replays, "median_us_per_session": round(statistics.median(us), 3),
+                "min_us_per_session": round(us[0], 3), "max_us_per_session": round(us[-1], 3)}
+    except Exception as e:  # noqa: BLE001  (capture is a convenience of this measurement, not part of the path)
+        torch.cuda.synchronize()
+        return {"unavailable": str(e)[:160]}
+
+
+def run_scan_logits(wl, prepos, reps=50):
+    """a4' -- the paper's serve-time vocabulary scan T_scan(V) (Eq. 3; 0.664 ms derived on its host,
+    PAPER.md:276): prepos_scan_logits over stored fp32 logits, n = 1 and n = 64 rows.  Device time per call with
+    the logits L2-resident (back-to-back calls) and after an L2 flush (the logits come from HBM), and wall time of
+    call + D2H of the record(s) into pinned memory + sync."""
+    dev, s = wl.dev, wl.spec["shape"]
+    res = {}
+    flush = torch.empty(2 * L2_BYTES, dtype=torch.uint8, device=dev)
+    for n in (1, 64):
+        ctx = prepos.Context(s.layers, s.Hq, s.Hkv, s.d, s.H, s.V, s.page, max_sessions=n)
+        lg = torch.randn((n, s.V), generator=synth.gen(wl.spec["seed"] + 31 + n, dev), device=dev, dtype=torch.float32)
+        recs = prepos.new_records(n, dev)
+        rec_h = torch.empty(recs.shape, dtype=torch.uint8).pin_memory()
+        for _ in range(5):
+            ctx.scan_logits(lg, recs)
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(reps):
+            ctx.scan_logits(lg, recs)
+        e1.record()
+        torch.cuda.synchronize()
+        warm = e0.elapsed_time(e1) * 1e3 / reps
+        cold = []
+        for i in range(10):
+            flush.fill_(i)
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record()
+            ctx.scan_logits(lg, recs)
+            b.record()
+            torch.cuda.synchronize()
+            cold.append(a.elapsed_time(b) * 1e3)
+        walls = []
+        for _ in range(reps):
+            t0 = time.perf_counter()
+            ctx.scan_logits(lg, recs)
+            rec_h.copy_(recs, non_blocking=True)
+            torch.cuda.synchronize()
+            walls.append((time.perf_counter() - t0) * 1e6)
+        nbytes = n * s.V * 4
+        res[f"n{n}"] = {"logit_bytes": nbytes, "device_us_l2_resident": round(warm, 2),
+                        "device_us_from_hbm_median": round(statistics.median(cold), 2),
+                        "hbm_gbs_from_hbm": round(nbytes / (statistics.median(cold) * 1e-6) / 1e9, 1),
+                        "wall_us_call_d2h_sync_p50": round(statistics.median(walls), 2)}
+        ctx.close()
+    return res
+
+
+def run_update_trace(wl, prepos, n_steps=1000):
+    """BASELINE configs[2]'s trace at the config's real vocabulary shape (reading Q16; "triggered after a
+    data update"): per update, with probability 0.3 the state version is bumped (prepos_invalidate); then one gate
+    serve; if that serve was refused as stale, the session is re-pre-positioned with the next of 16 hidden rows
+    (prepos_ready_dist only: the attention of the update is the step timed above).  Wall time of the whole trace, the
+    decisions' counts, and two invariants checked on the spot: every serve right after a bump is STALE, no other is."""
+    dev, s = wl.dev, wl.spec["shape"]
+    seed = wl.spec["seed"]
+    bumps = synth.bump_trace(n_steps, seed)
+    pool, _, _ = synth.make_hidden(s, 16, wl.w, wl.fast, seed + 17)
+    ctx = prepos.Context(s.layers, s.Hq, s.Hkv, s.d, s.H, s.V, s.page, max_sessions=1)
+    recs = prepos.new_records(1, dev)
+    ver = torch.zeros(1, dtype=torch.int64, device=dev)
+    sid = torch.zeros(1, dtype=torch.int32, device=dev)
+    decs = torch.full((n_steps,), -9, dtype=torch.int32, device=dev)
+    toks = torch.full((n_steps,), -9, dtype=torch.int32, device=dev)
+    exp = torch.arange(0, n_steps + 1, dtype=torch.int64, device=dev)
+    ctx.ready_dist(sid, pool[0:1], wl.w, recs, ver, expected_version=exp[0:1])
+    torch.cuda.synchronize()
+    cur, nb = 0, 0
+    t0 = time.perf_counter()
+    for t, b in enumerate(bumps):
+        if b:
+            ctx.invalidate(sid, ver, recs)
+            nb += 1
+        ctx.gate_serve(sid, recs, ver, wl.bitmap, s.tau, decs[t:t + 1], toks[t:t + 1])
+        if b:   # the serve above was refused (stale): pre-position again on the new state
+            cur = (cur + 1) % 16
+            ctx.ready_dist(sid, pool[cur:cur + 1], wl.w, recs, ver, expected_version=exp[nb:nb + 1])
+    torch.cuda.synchronize()
+    wall = time.perf_counter() - t0
+    d = decs.cpu().tolist()
+    stale_ok = all((d[t] == prepos.STALE_OR_INVALID) == bool(b) for t, b in enumerate(bumps))
+    ctx.close()
+    counts = {name: sum(1 for x in d if x == code) for name, code in
+              (("served", 0), ("gap_below_tau", 1), ("not_in_fast_set", 2), ("stale_or_invalid", 3), ("ineligible", 4))}
+    return {"updates": n_steps, "bumps": nb, "wall_us_per_update": round(wall * 1e6 / n_steps, 2),
+            "ready_dist_calls": nb + 1, "decisions": counts, "stale_iff_bumped": stale_ok,
+            "final_version": int(ver[0])}
+
+
+def run_c2_variants(spec, dev, prepos, steps=40):
+    """What the steady-state step of config 2 does not show: (a) a session whose n_s advances by L after every
+    pre-position, as a real one does (the host rebuilds and uploads the attention plan on every call); (b) n_s = 4100,
+    where the units do not divide evenly over the CTAs and the general stream-K grid runs (cut segments + merges)
+    instead of the whole-unit grid of n_s = 4096."""
+    s = spec["shape"]
+    res = {}
+    L = spec["l_entry"][0]
+    # (a)
+    n0 = spec["n_s"][0]
+    sb = synth.make_sessions(s, [n0], [L], spec["seed"] + 5, dev, extra_pages=(steps + 12) * L // s.page + 2)
+    ctx = prepos.Context(s.layers, s.Hq, s.Hkv, s.d, s.H, s.V, s.page, max_sessions=1)
+    out = torch.empty_like(sb.q)
+    for i in range(10):
+        ctx.entry_attn(sb.q, sb.k_new, sb.v_new, sb.k_pool, sb.v_pool, sb.page_table, [n0 + i * L], [L], sb.capacity, out)
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    t0 = time.perf_counter()
+    e0.record()
+    for i in range(steps):
+        ctx.entry_attn(sb.q, sb.k_new, sb.v_new, sb.k_pool, sb.v_pool, sb.page_table, [n0 + (10 + i) * L], [L],
+                       sb.capacity, out)
+    e1.record()
+    torch.cuda.synchronize()
+    res["advancing_n_s"] = {"attn_ms_per_call_device": round(e0.elapsed_time(e1) / steps, 5),
+                            "attn_ms_per_call_wall": round((time.perf_counter() - t0) * 1e3 / steps, 5),
+                            "n_s_from_to": [n0 + 10 * L, n0 + (10 + steps) * L]}
+    ctx.close()
+    del sb, out
+    # (b)
+    spec_b = dict(spec, n_s=[4100])
+    ab = algorithmic_bytes(spec_b)["entry_attn"]
+    sets = [synth.make_sessions(s, [4100], [L], spec["seed"] + 7 + r, dev) for r in range(3)]
+    ctx = prepos.Context(s.layers, s.Hq, s.Hkv, s.d, s.H, s.V, s.page, max_sessions=1)
+    outs = [torch.empty_like(x.q) for x in sets]
+    ev = []
+    for i in range(steps + 5):
+        sb = sets[i % 3]
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        ctx.entry_attn(sb.q, sb.k_new, sb.v_new, sb.k_pool, sb.v_pool, sb.page_table, sb.n_s, sb.l_entry, sb.capacity,
+                       outs[i % 3])
+        b.record()
+        ev.append((a, b))
+    torch.cuda.synchronize()
+    ms = statistics.median(a.elapsed_time(b) for a, b in ev[5:])
+    res["n_s_4100_general_grid"] = {"attn_ms_median": round(ms, 5), "achieved_gbs": round(ab / (ms * 1e-3) / 1e9, 1),
+                                    "frac_of_measured_hbm": round(ab / (ms * 1e-3) / 1e9 / peaks()["hbm"], 4)}
+    ctx.close()
+    return res
+
+
+def headline_config_dict(spec, world):
+    return {"workload": spec["text"], "sessions_per_step": len(spec["n_s"]), "gate_serves_per_step": spec["serves"],
+            "resident_sets": spec["resident"],
+            "l2": "flushed between timed steps" if spec["flush_l2"] else
+                  "inputs larger than L2 (rotating resident sets; W_vocab alone is 8x L2)",
+            "parallelism": f"session-sharded replicas x{world}, no collective"}
+
+
 def main_reference(args, d):
     """--impl reference: the CPU oracle on this arm's config/metric/unit, each step a bounded sample."""
     if d.rank != 0:
         return
-    spec = workload_spec(args.config)
+    name = args.config or HEADLINE
+    spec = workload_spec(name)
     os_ = OracleSample(spec)
-    budget = 120.0 / max(1, args.steps + args.warmup)
+    steps = args.steps if args.steps is not None else 3
+    warmup = args.warmup if args.warmup is not None else 1
+    budget = 120.0 / max(1, steps + warmup)
     units, rows = os_.plan(min(budget, 15.0))
-    for _ in range(args.warmup):
+    for _ in range(warmup):
         os_.run(units, rows)
     t0 = time.perf_counter()
-    fulls = [os_.run(units, rows)[0] for _ in range(args.steps)]
+    fulls = [os_.run(units, rows)[0] for _ in range(steps)]
     wall = time.perf_counter() - t0
     value = statistics.fmean(fulls) * 1e6
     line = {
-        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
-        "warmup": args.warmup, "ms_per_step": wall * 1e3 / args.steps, "higher_is_better": False, "scaling": "weak",
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": steps,
+        "warmup": warmup, "ms_per_step": wall * 1e3 / steps, "higher_is_better": False, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": spec["text"], "sessions_per_step": 1, "note": "ms_per_step is the sampled step's wall time; "
-                   "value is the per-session estimate from the sample"},
+        "config": headline_config_dict(spec, d.world),
+        "sampling": "ms_per_step is the sampled step's wall time; value is the per-session estimate from the sample",
         "cpu_baseline": {"value": value, "unit": UNIT, "cores": os_.cores, "kind": "oracle", "sample": os_.describe(units, rows)},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
@@ -735,23 +935,136 @@ def main_reference(args, d):
     print(json.dumps(line))
 
 
+def cpu_baseline_leg(spec, budget_s):
+    """The oracle as it stands on the box's host cores: all cores on a bounded sample, and one thread on a smaller one."""
+    osmp = OracleSample(spec)
+    units, rows = osmp.plan(budget_s)
+    full, spent = osmp.run(units, rows)
+    out = {"value": full * 1e6, "unit": UNIT, "cores": osmp.cores, "kind": "oracle",
+           "sample": osmp.describe(units, rows), "sample_seconds": round(spent, 2)}
+    try:
+        osmp.o.set_num_threads(1)
+        u1 = max(1, min(units, max(1, units // osmp.cores)))
+        r1 = max(min(1024, spec["shape"].V), rows // osmp.cores)
+        full1, spent1 = osmp.run(u1, r1)
+        out["one_thread"] = {"value": full1 * 1e6, "unit": UNIT, "cores": 1, "sample": osmp.describe(u1, r1),
+                             "sample_seconds": round(spent1, 2)}
+    finally:
+        osmp.o.set_num_threads(osmp.cores)
+    return out
+
+
+def run_config(name, args, d, dev, prepos):
+    """One BASELINE config -> the dict of its JSON fields (rank 0; other ranks return None)."""
+    spec = workload_spec(name)
+    steps = args.steps if args.steps is not None else DEFAULT_STEPS[name][0]
+    warmup = max(args.warmup if args.warmup is not None else DEFAULT_STEPS[name][1], 3)
+    wl = Workload(spec, dev, prepos)
+    if args.attn_path:
+        wl.ctx.set_attn_path(args.attn_path)
+    n_sess = wl.n
+    res = run_device_timed(wl, steps, warmup, d)
+    total_ms = d.max(res["total_ms"], dev)
+    ms_per_step = total_ms / steps
+    # weak scaling: every rank pre-positions its own sessions; whole-job us/session = time / (N * sessions)
+    value = ms_per_step * 1e3 / (n_sess * d.world)
+
+    e2e = None
+    if not args.no_e2e:
+        e = run_e2e(wl, max(3, min(steps, 30)), 3, d)
+        e_ms = d.max(e["ms_per_step"], dev)
+        e2e = {"value": e_ms * 1e3 / (n_sess * d.world), "unit": UNIT, "h2d_bytes_per_step": e["h2d"], "d2h_bytes_per_step": e["d2h"],
+               "timing": "CUDA events from before the first H2D to after the last D2H; copies on their own streams, two steps in flight"}
+    if d.rank != 0:
+        del wl
+        torch.cuda.empty_cache()
+        return None
+
+    pk = peaks()
+    ab = algorithmic_bytes(spec)
+    calls = res["calls"]
+    kern = {}
+    for kname_ in ("entry_attn", "ready_dist"):
+        gbs = ab[kname_] / (calls[kname_] * 1e-3) / 1e9
+        kern[kname_] = {"ms": round(calls[kname_], 5), "ms_median": round(res["calls_median"][kname_], 5),
+                        "ms_min": round(res["calls_min"][kname_], 5), "algorithmic_bytes": ab[kname_],
+                        "achieved_gbs": round(gbs, 1), "frac_of_measured_hbm": round(gbs / pk["hbm"], 4)}
+    fl = attention_flops(spec)
+    kern["entry_attn"]["tflops"] = round(fl / (calls["entry_attn"] * 1e-3) / 1e12, 1)
+    kern["entry_attn"]["frac_of_measured_bf16"] = round(kern["entry_attn"]["tflops"] / pk["bf16"], 4)
+    kern["invalidate"] = {"ms": round(calls["invalidate"], 5)}
+    kern["gate_serve"] = {"ms": round(calls["gate_serve"], 5), "requests": spec["serves"]}
+    dom = max(("entry_attn", "ready_dist"), key=lambda k: calls[k])
+    intensity = fl / max(1, ab["entry_attn"])   # flop per algorithmic byte of the attention call
+    ridge = pk["bf16"] * 1e12 / (pk["hbm"] * 1e9)
+    kname = ("attn_generic_kernel" if name == "c1" else "attn_umma_kernel") if dom == "entry_attn" else (
+        "ready_dist_batch_kernel" if n_sess > 8 else "ready_dist_kernel")
+    if dom == "entry_attn" and intensity >= 0.9 * ridge:
+        # G * L_entry at or above the ridge: the attention is a tensor-bound dense contraction (DESIGN.md 6.1);
+        # the kernel is timed alone between events: burst peak
+        roofline = {"kernel": kname, "bound": "tensor", "achieved": kern[dom]["tflops"], "peak": pk["bf16"],
+                    "unit": "TFLOP/s", "frac": kern[dom]["frac_of_measured_bf16"]}
+    else:
+        roofline = {"kernel": kname, "bound": "hbm", "achieved": kern[dom]["achieved_gbs"], "peak": pk["hbm"],
+                    "unit": "GB/s", "frac": kern[dom]["frac_of_measured_hbm"]}
+    traffic, traffic_src = ncu_traffic(name, kname)
+    roofline.update({"traffic": traffic, "traffic_source": traffic_src, "algorithmic_bytes": ab[dom],
+                     "flop_per_byte": round(intensity, 1) if dom == "entry_attn" else round(2.0 * n_sess, 1),
+                     "peak_source": pk["source"], "share_of_step": round(calls[dom] / sum(calls.values()), 4)})
+    step_bytes = ab["entry_attn"] + ab["ready_dist"]
+    step_gbs = step_bytes / (ms_per_step * 1e-3) / 1e9
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": d.world, "steps": steps, "warmup": warmup,
+        "ms_per_step": ms_per_step, "higher_is_better": False, "scaling": "weak", "vs_baseline": None,
+        "dtype": "bf16", "data": "synthetic",
+        "config": headline_config_dict(spec, d.world),
+        "roofline": roofline,
+        "entry_pass_roofline": {"algorithmic_bytes": step_bytes, "achieved_gbs": round(step_gbs, 1),
+                                "frac_of_measured_hbm": round(step_gbs / pk["hbm"], 4),
+                                "frac_of_8tbs_nominal": round(step_gbs / 8000.0, 4)},
+        "timing": {"mean_us_per_session": round(value, 3), "graph_replay": run_graph_replay(wl)},
+        "kernels": kern,
+        "clocks": res["clocks"],
+        "clocks_per_call_pass": res["clocks_per_call_pass"],
+        "gpu_launches": res["launches"],
+    }
+    if e2e:
+        line["e2e"] = e2e
+    if not args.quick:
+        line["gate_serve"] = run_gate_serve(wl, prepos)
+        line["attn_layer_sequential"] = run_layer_sequential(wl)
+        ft = run_fall_through(wl)
+        if ft:
+            line["fall_through"] = ft
+        if d.world == 1:
+            line["co_schedule"] = run_co_schedule(wl, prepos)
+        if name in ("c2", "c5"):
+            line["scan_logits"] = run_scan_logits(wl, prepos)
+        if name == "c3":
+            line["update_trace"] = run_update_trace(wl, prepos)
+    del wl
+    torch.cuda.empty_cache()
+    if name == "c2" and not args.quick:
+        line["variants"] = run_c2_variants(spec, dev, prepos)
+        torch.cuda.empty_cache()
+    if not args.no_cpu_baseline:
+        line["cpu_baseline"] = cpu_baseline_leg(spec, 12.0 if name == (args.config or HEADLINE) else 5.0)
+    return line
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=None)
     ap.add_argument("--warmup", type=int, default=None)
-    ap.add_argument("--config", default="c2", choices=["c1", "c2", "c3", "c4", "c5"])
+    ap.add_argument("--config", default=None, choices=ALL_CONFIGS,
+                    help="run this one config alone (default: all five, headline " + HEADLINE + ")")
     ap.add_argument("--impl", default="prepos", choices=["prepos", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--quick", action="store_true", help="the timed step only: no side measurements (for ncu runs)")
     ap.add_argument("--attn-path", type=int, default=0, help="0 auto, 1 generic CUDA-core kernel, 2 tcgen05 kernel")
     args = ap.parse_args()
-    defaults = {"c1": (400, 20), "c2": (200, 10), "c3": (60, 5), "c4": (12, 3), "c5": (60, 5)}
-    if args.steps is None:
-        args.steps = defaults[args.config][0]
-    if args.warmup is None:
-        args.warmup = defaults[args.config][1]
-    args.warmup = max(args.warmup, 3)
 
     d = Dist(args.gpus)
     if args.impl == "reference":
@@ -766,90 +1079,17 @@ def main():
     dev = torch.device("cuda", d.local_rank)
     d.init("nccl")
 
-    spec = workload_spec(args.config)
-    wl = Workload(spec, dev, prepos)
-    if args.attn_path:
-        wl.ctx.set_attn_path(args.attn_path)
-    n_sess = wl.n
-    res = run_device_timed(wl, args.steps, args.warmup, d)
-    total_ms = d.max(res["total_ms"], dev)
-    ms_per_step = total_ms / args.steps
-    # weak scaling: every rank pre-positions its own sessions; whole-job us/session = time / (N * sessions)
-    value = ms_per_step * 1e3 / (n_sess * d.world)
-
-    e2e = None
-    if not args.no_e2e:
-        e = run_e2e(wl, max(3, min(args.steps, 50)), 3, d)
-        e_ms = d.max(e["ms_per_step"], dev)
-        e2e = {"value": e_ms * 1e3 / (n_sess * d.world), "unit": UNIT, "h2d_bytes_per_step": e["h2d"], "d2h_bytes_per_step": e["d2h"],
-               "timing": "CUDA events from before the first H2D to after the last D2H; copies on their own streams, two steps in flight"}
-
+    names = [args.config] if args.config else ALL_CONFIGS
+    head = args.config or HEADLINE
+    lines = {}
+    for name in names:
+        lines[name] = run_config(name, args, d, dev, prepos)
     if d.rank == 0:
-        pk = peaks()
-        ab = algorithmic_bytes(spec)
-        calls = res["calls"]
-        kern = {}
-        for name in ("entry_attn", "ready_dist"):
-            gbs = ab[name] / (calls[name] * 1e-3) / 1e9
-            kern[name] = {"ms": round(calls[name], 5), "algorithmic_bytes": ab[name], "achieved_gbs": round(gbs, 1),
-                          "frac_of_measured_hbm": round(gbs / pk["hbm"], 4)}
-        fl = attention_flops(spec)
-        kern["entry_attn"]["tflops"] = round(fl / (calls["entry_attn"] * 1e-3) / 1e12, 1)
-        kern["entry_attn"]["frac_of_measured_bf16"] = round(kern["entry_attn"]["tflops"] / pk["bf16"], 4)
-        kern["invalidate"] = {"ms": round(calls["invalidate"], 5)}
-        kern["gate_serve"] = {"ms": round(calls["gate_serve"], 5), "requests": spec["serves"]}
-        dom = max(("entry_attn", "ready_dist"), key=lambda k: calls[k])
-        s_ = spec["shape"]
-        intensity = fl / max(1, ab["entry_attn"])   # flop per algorithmic byte of the attention call
-        ridge = pk["bf16"] * 1e12 / (pk["hbm"] * 1e9)
-        kname = "attn_umma_kernel" if dom == "entry_attn" else (
-            "ready_dist_batch_kernel" if n_sess > 8 else "ready_dist_kernel")
-        if dom == "entry_attn" and intensity >= 0.9 * ridge:
-            # G * L_entry at or above the ridge: the attention is a tensor-bound dense contraction;
-            # the kernel is timed alone between events: burst peak
-            roofline = {"kernel": kname, "bound": "tensor", "achieved": kern[dom]["tflops"], "peak": pk["bf16"],
-                        "unit": "TFLOP/s", "frac": kern[dom]["frac_of_measured_bf16"]}
-        else:
-            roofline = {"kernel": kname, "bound": "hbm", "achieved": kern[dom]["achieved_gbs"], "peak": pk["hbm"],
-                        "unit": "GB/s", "frac": kern[dom]["frac_of_measured_hbm"]}
-        roofline.update({"traffic": NCU_TRAFFIC.get((args.config, dom)), "algorithmic_bytes": ab[dom],
-                         "flop_per_byte": round(intensity, 1) if dom == "entry_attn" else round(2.0 * n_sess, 1),
-                         "peak_source": pk["source"], "share_of_step": round(calls[dom] / sum(calls.values()), 4)})
-        step_bytes = ab["entry_attn"] + ab["ready_dist"]
-        step_gbs = step_bytes / (ms_per_step * 1e-3) / 1e9
-        line = {
-            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": d.world, "steps": args.steps, "warmup": args.warmup,
-            "ms_per_step": ms_per_step, "higher_is_better": False, "scaling": "weak", "vs_baseline": None,
-            "dtype": "bf16", "data": "synthetic",
-            "config": {"workload": spec["text"], "sessions_per_step": n_sess, "gate_serves_per_step": spec["serves"],
-                       "resident_sets": spec["resident"],
-                       "l2": "flushed between timed steps" if spec["flush_l2"] else
-                             "inputs larger than L2 (rotating resident sets; W_vocab alone is 8x L2)",
-                       "parallelism": f"session-sharded replicas x{d.world}, no collective"},
-            "roofline": roofline,
-            "entry_pass_roofline": {"algorithmic_bytes": step_bytes, "achieved_gbs": round(step_gbs, 1),
-                                    "frac_of_measured_hbm": round(step_gbs / pk["hbm"], 4),
-                                    "frac_of_8tbs_nominal": round(step_gbs / 8000.0, 4)},
-            "kernels": kern,
-            "clocks": res["clocks"],
-            "clocks_per_call_pass": res["clocks_per_call_pass"],
-            "gpu_launches": res["launches"],
-        }
-        if e2e:
-            line["e2e"] = e2e
-        line["gate_serve"] = run_gate_serve(wl, prepos)
-        line["attn_layer_sequential"] = run_layer_sequential(wl)
-        ft = run_fall_through(wl)
-        if ft:
-            line["fall_through"] = ft
-        if d.world == 1:
-            line["co_schedule"] = run_co_schedule(wl, prepos)
-        if not args.no_cpu_baseline:
-            osmp = OracleSample(spec)
-            units, rows = osmp.plan(15.0)
-            full, spent = osmp.run(units, rows)
-            line["cpu_baseline"] = {"value": full * 1e6, "unit": UNIT, "cores": osmp.cores, "kind": "oracle",
-                                    "sample": osmp.describe(units, rows), "sample_seconds": round(spent, 2)}
+        line = lines[head]
+        if len(names) > 1:
+            line["per_config"] = {n: lines[n] for n in names if n != head}
+            line["headline"] = (f"{head}: configs[{int(head[1]) - 1}] of BASELINE.json (the largest per-session pass and the "
+                                "paper's measured model class); per_config holds the other four")
         print(json.dumps(line))
     d.barrier()
     d.close()

@@ -78,12 +78,18 @@ def lib():
         L.oracle_fastset_bitmap.restype = None
         L.oracle_fastset_bitmap.argtypes = [p, C.c_int, C.c_int, p]
         L.oracle_num_threads.restype = C.c_int
+        L.oracle_set_num_threads.restype = None
+        L.oracle_set_num_threads.argtypes = [C.c_int]
         _lib = L
     return _lib
 
 
 def num_threads() -> int:
     return int(lib().oracle_num_threads())
+
+
+def set_num_threads(n: int) -> None:
+    lib().oracle_set_num_threads(int(n))
 
 
 def bf16_bits(t) -> np.ndarray:

@@ -453,6 +453,16 @@ void oracle_fastset_bitmap(const int32_t *ids, int n, int V, uint32_t *bitmap)
             bitmap[ids[r] >> 5] |= 1u << (ids[r] & 31);
 }
 
+/* test-infrastructure plumbing: the 1-thread figure of bench.py's cpu_baseline */
+void oracle_set_num_threads(int n)
+{
+#ifdef _OPENMP
+    omp_set_num_threads(n > 0 ? n : 1);
+#else
+    (void)n;
+#endif
+}
+
 int oracle_num_threads(void)
 {
     int n = 1;

@@ -79,16 +79,17 @@ def _check_append(sb, kp, vp, before, status, layers):
 
 @pytest.mark.parametrize("path", PATHS)
 def test_config1_many_seeds(prepos, oracle, path):
-    """BASELINE config 1 attention: 1 session, n_s=256, L=8, 4/2 heads, d=64 -- 24 seeds, full outputs."""
+    """BASELINE config 1 attention: 1 session, n_s=256, L=8, 4/2 heads, d=64 -- 200 seeds ("many
+    seeds (>= 200)"), every output element, Append(E) on every seed."""
     worst = 0.0
-    for k in range(24):
+    for k in range(200):
         sb = synth.make_sessions(synth.C1, [256], [8], seed=synth.SEED_BASE + 1000 * k)
-        out, kp, vp, before, status, _ = _gpu_run(prepos, sb, path)
+        out, kp, vp, before, status, ctx = _gpu_run(prepos, sb, path)
+        ctx.close()
         outs, st, _, _ = oracle_attn_batch(oracle, sb)
         assert status == [0] and st[0] == 0
         worst = max(worst, check_attn(out, outs, sb))
-        if k < 3:
-            _check_append(sb, kp, vp, before, status, [0])
+        _check_append(sb, kp, vp, before, status, [0])
     assert worst <= ATTN_ATOL
 
 
@@ -101,6 +102,13 @@ SHAPES = {
     "d128_g3": synth.Shape("f", layers=2, Hq=6, Hkv=2, d=128, H=128, V=64, page=16),      # G not a power of two
     "d128_p32": synth.Shape("g", layers=1, Hq=8, Hkv=2, d=128, H=128, V=64, page=32),     # another page size
     "d96_g2": synth.Shape("h", layers=1, Hq=4, Hkv=2, d=96, H=128, V=64, page=16),        # head_dim the tcgen05 path skips
+    # MHA / G = 2 with more than 128 entry tokens: a unit's row chunk spans two entry tiles, so rows of the first
+    # see NO column of the second.  16 layers: ~15 tiles per CTA, units cut at arbitrary tiles and merged by the last
+    # arriver; 1 layer: one tile per CTA, every unit spread over ~35 CTAs and merged by attn_merge_kernel
+    "d128_g1_l16": synth.Shape("i", layers=16, Hq=2, Hkv=2, d=128, H=128, V=64, page=16),
+    "d128_g2_l16": synth.Shape("j", layers=16, Hq=4, Hkv=2, d=128, H=128, V=64, page=16),
+    "d128_g2": synth.Shape("k", layers=1, Hq=4, Hkv=2, d=128, H=128, V=64, page=16),
+    "d64_g1_l8": synth.Shape("l", layers=8, Hq=2, Hkv=2, d=64, H=128, V=64, page=16),
 }
 
 
@@ -120,6 +128,17 @@ SHAPES = {
     ("d128_g3", [150], [11]),                     # CUDA-core kernel only (the tcgen05 path wants G = 2^k)
     ("d128_p32", [333], [24]),
     ("d96_g2", [140], [6]),
+    ("d128_g1_l16", [4096], [129]),
+    ("d128_g1_l16", [4000], [200]),
+    ("d128_g1_l16", [2500, 700], [300, 257]),
+    ("d128_g2_l16", [4096], [129]),
+    ("d128_g2_l16", [3000], [200]),
+    ("d128_g2_l16", [2200], [300]),
+    ("d128_g1", [4096], [200]),
+    ("d128_g1", [1500], [300]),
+    ("d128_g2", [4096], [129]),
+    ("d128_g2", [777], [300]),
+    ("d64_g1_l8", [3000], [260]),
 ])
 def test_shapes_vs_oracle(prepos, oracle, path, shape_key, n_s, l_entry):
     shape = SHAPES[shape_key]
@@ -143,6 +162,24 @@ def test_budget_skip_no_side_effects(prepos, oracle, path):
     check_attn(out, outs, sb)
     r0 = sb.row_offset[1]
     assert torch.isnan(out[:, r0:r0 + 20].float()).all()    # rows of the skipped session untouched
+    _check_append(sb, kp, vp, before, status, range(shape.layers))
+
+
+@pytest.mark.parametrize("path", PATHS)
+def test_nonfinite_rows_of_a_skipped_neighbour_do_not_leak(prepos, oracle, path):
+    """The entry K/V of a budget-skipped session may never have been initialised by the caller.  Its rows sit right
+    behind the previous session's in the packed sum_L axis, inside the last 8-token box that session loads: they must
+    not reach its output (0 x NaN in the PV product)."""
+    shape = SHAPES["d128_g4"]
+    sb = synth.make_sessions(shape, [300, 40, 90], [13, 20, 5], seed=123, tight_capacity=[None, 59, None])
+    r1 = sb.row_offset[1]
+    for t in (sb.k_new, sb.v_new, sb.q):
+        t[:, r1:r1 + 20] = float("nan")
+    out, kp, vp, before, status, _ = _gpu_run(prepos, sb, path)
+    assert status == [0, prepos.SKIPPED_BUDGET, 0]
+    outs, st, _, _ = oracle_attn_batch(oracle, sb, sessions=[0, 2])
+    check_attn(out, outs, sb)
+    assert torch.isnan(out[:, r1:r1 + 20].float()).all()
     _check_append(sb, kp, vp, before, status, range(shape.layers))
 
 
@@ -228,46 +265,136 @@ def _full_size_spec(name):
     return synth.C5, [16384], [32], seed
 
 
-@pytest.mark.parametrize("name", ["c2", "c3", "c4", "c5"])
-def test_full_size_configs_sampled(prepos, oracle, name):
-    """BASELINE configs 2-5 at FULL size in the launch configuration bench.py times (default path, every layer
-    in one launch, inputs generated on the device with bench.py's seeds): sampled (layer, session, head, entry
-    row) outputs against the oracle, which computes each sampled row from the same bits, plus the Append(E)
-    post-condition on the sampled (layer, session) pairs."""
-    shape, n_s, l_e, seed = _full_size_spec(name)
-    sb = synth.make_sessions(shape, n_s, l_e, seed=seed, device="cuda")
-    n = len(n_s)
-    ctx = prepos.Context(shape.layers, shape.Hq, shape.Hkv, shape.d, shape.H, shape.V, shape.page, max_sessions=n)
-    out = torch.full(sb.q.shape, float("nan"), dtype=torch.bfloat16, device="cuda")
-    status = ctx.entry_attn(sb.q, sb.k_new, sb.v_new, sb.k_pool, sb.v_pool, sb.page_table, sb.n_s, sb.l_entry,
-                            sb.capacity, out)
-    ctx.sync()
-    assert status == [0] * n
-    assert torch.isfinite(out.float()).all()
-    rng = np.random.default_rng(seed)
-    sessions = list(range(n)) if n <= 8 else sorted(set(int(x) for x in rng.choice(n, 8, replace=False)) |
-                                                     {int(np.argmax(n_s)), int(np.argmax(l_e))})
+def _expected_pools_after_append(sb):
+    """The pools as Append(E) (Alg. 1 l.5) must leave them: a copy of the pristine pools with K_new / V_new scattered
+    to cache positions n_s .. n_s+L-1 of every session through the page table (torch indexing on the synthetic
+    inputs: data movement only).  Comparing the whole tensors checks every appended slot of every session and layer
+    AND that no other pool element moved."""
+    page = sb.shape.page
+    ke, ve = sb.k_pool.clone(), sb.v_pool.clone()
+    pt = sb.page_table.long()
+    for s in range(sb.n_sessions):
+        j = sb.n_s[s] + torch.arange(sb.l_entry[s], device=ke.device)
+        pg, sl = pt[s, j // page], j % page
+        r0 = sb.row_offset[s]
+        ke[:, pg, :, sl] = sb.k_new[:, r0:r0 + sb.l_entry[s]].permute(1, 0, 2, 3)   # advanced dims lead: [L, layers, Hkv, d]
+        ve[:, pg, :, sl] = sb.v_new[:, r0:r0 + sb.l_entry[s]].permute(1, 0, 2, 3)
+    return ke, ve
+
+
+def _gather_session(sb, s):
+    """Pristine host copy of session s's pages, re-indexed 0..n-1 (the oracle's page-shuffle invariance is pinned):
+    (k [layers, n, Hkv, page, d] uint16, v, table int32 [n])."""
+    n = -(-(sb.n_s[s] + sb.l_entry[s]) // sb.shape.page)
+    idx = sb.page_table[s, :n].long()
+    k = sb.k_pool[:, idx].cpu().contiguous().view(torch.int16).numpy().view(np.uint16)
+    v = sb.v_pool[:, idx].cpu().contiguous().view(torch.int16).numpy().view(np.uint16)
+    return k, v, np.arange(n, dtype=np.int32)
+
+
+def _check_session_every_row(oracle, sb, s, out, pristine):
+    """Every output element of session s, all layers, against O1 on the pristine pages."""
+    k, v, table = pristine
+    r0, L = sb.row_offset[s], sb.l_entry[s]
     worst = 0.0
-    for s in sessions:
-        # a single session: first, last and one random layer; a batch: one random layer per sampled session
-        layers = sorted({0, shape.layers - 1, int(rng.integers(0, shape.layers))}) if n == 1 else [
-            int(rng.integers(0, shape.layers))]
-        for l in layers:
-            L = l_e[s]
-            picks = [(int(rng.integers(0, shape.Hq)), int(rng.integers(0, L))) for _ in range(2)]
-            picks += [(shape.Hq - 1, L - 1), (0, 0)]
-            ref = oracle_attn_rows(oracle, sb, l, s, picks)
-            for (h, i), o in ref.items():
-                got = out[l, sb.row_offset[s] + i, h].cpu().to(torch.float64).numpy()
-                worst = max(worst, float(np.abs(got - o).max()))
-            # Append(E): the session's new cache positions hold K_new / V_new bit for bit
-            pt = sb.page_table[s].cpu()
-            for jp in (0, L // 2, L - 1):
-                j = n_s[s] + jp
-                pg, sl = int(pt[j // shape.page]), j % shape.page
-                r = sb.row_offset[s] + jp
-                assert torch.equal(sb.k_pool[l, pg, :, sl].view(torch.int16), sb.k_new[l, r].view(torch.int16))
-                assert torch.equal(sb.v_pool[l, pg, :, sl].view(torch.int16), sb.v_new[l, r].view(torch.int16))
+    for l in range(k.shape[0]):
+        ref = oracle.entry_attn(bits(sb.q[l, r0:r0 + L]), bits(sb.k_new[l, r0:r0 + L]), bits(sb.v_new[l, r0:r0 + L]),
+                                k[l].copy(), v[l].copy(), table, sb.n_s[s], sb.capacity[s])
+        assert ref["status"] == 0
+        got = out[l, r0:r0 + L].cpu().to(torch.float64).numpy()
+        worst = max(worst, float(np.abs(got - ref["out"]).max()))
+    return worst
+
+
+def _draw_samples(rng, shape, L, n_slices=8, per_slice=8):
+    """64 seeded (layer, head, row) samples of one session, grouped by (layer, kv head) slice."""
+    G = shape.G
+    out = []
+    for _ in range(n_slices):
+        l, g = int(rng.integers(0, shape.layers)), int(rng.integers(0, shape.Hkv))
+        picks = [(int(rng.integers(0, G)), int(rng.integers(0, L))) for _ in range(per_slice - 2)] + [(G - 1, L - 1), (0, 0)]
+        out.append((l, g, picks))
+    return out
+
+
+def _gather_slices(sb, s, samples):
+    """Pristine host copies of the (layer, kv head) slices the samples of session s need."""
+    n = -(-(sb.n_s[s] + sb.l_entry[s]) // sb.shape.page)
+    idx = sb.page_table[s, :n].long()
+    res = []
+    for (l, g, _) in samples:
+        k = sb.k_pool[l, idx, g:g + 1].cpu().contiguous().view(torch.int16).numpy().view(np.uint16)
+        v = sb.v_pool[l, idx, g:g + 1].cpu().contiguous().view(torch.int16).numpy().view(np.uint16)
+        res.append((k, v))
+    return res
+
+
+def _check_samples(oracle, sb, s, out, samples, slices):
+    """Sampled (layer, head, row) outputs of session s against the ranged O1 (one row of one head per call)."""
+    G = sb.shape.G
+    r0, L = sb.row_offset[s], sb.l_entry[s]
+    n = slices[0][0].shape[0]
+    table = np.arange(n, dtype=np.int32)
+    worst = 0.0
+    for (l, g, picks), (k, v) in zip(samples, slices):
+        q = bits(sb.q[l, r0:r0 + L, g * G:(g + 1) * G])
+        kn, vn = bits(sb.k_new[l, r0:r0 + L, g:g + 1]), bits(sb.v_new[l, r0:r0 + L, g:g + 1])
+        for (hh, i) in picks:
+            ref = oracle.entry_attn(q, kn, vn, k.copy(), v.copy(), table, sb.n_s[s], sb.capacity[s],
+                                    heads=(hh, hh + 1), rows=(i, i + 1))["out"][i, hh]
+            got = out[l, r0 + i, g * G + hh].cpu().to(torch.float64).numpy()
+            worst = max(worst, float(np.abs(got - ref).max()))
+    return worst
+
+
+@pytest.mark.parametrize("name", ["c2", "c3", "c4", "c5"])
+def test_full_size_configs(prepos, oracle, name):
+    """BASELINE configs 2-5 at FULL size in the launch configuration bench.py times (default path, every layer in one
+    launch, inputs generated on the device with bench.py's seeds), with the coverage SURVEY.md 8(d) contracts:
+      c2, c3  every output element of every layer (24 576 / 16 384 rows)
+      c5      the sessions bench.py keeps resident (4 independent single-session batches): two of them every row,
+              64 seeded (layer, head, row) samples on each of the others
+      c4      eight whole sessions of the 64 -- including argmax(n_s) (a 16k-token session) and argmax(L) (more than
+              256 query rows: the split row chunk) -- every row; 64 seeded samples on each of the other 56
+    and, on every config, the WHOLE pools after the call against the pristine pools with K_new / V_new scattered to
+    the appended slots: Append(E) of every session on every layer, and every other pool element untouched."""
+    shape, n_s, l_e, seed = _full_size_spec(name)
+    batches = [seed] if name != "c5" else [seed + 100003 * (r + 1) for r in range(4)]    # bench.py's resident sets
+    worst = 0.0
+    for bi, bseed in enumerate(batches):
+        sb = synth.make_sessions(shape, n_s, l_e, seed=bseed, device="cuda")
+        n = len(n_s)
+        rng = np.random.default_rng(bseed)
+        if n == 1:
+            full = [0] if (name != "c5" or bi < 2) else []
+        else:
+            full = sorted(set(int(x) for x in rng.choice(n, 6, replace=False)) | {int(np.argmax(n_s)), int(np.argmax(l_e))})
+            while len(full) < 8:
+                full = sorted(set(full) | {int(rng.integers(0, n))})
+        sampled = [s for s in range(n) if s not in full]
+        pristine = {s: _gather_session(sb, s) for s in full}
+        samples = {s: _draw_samples(rng, shape, l_e[s]) for s in sampled}
+        slices = {s: _gather_slices(sb, s, samples[s]) for s in sampled}
+        ke, ve = _expected_pools_after_append(sb)
+        ctx = prepos.Context(shape.layers, shape.Hq, shape.Hkv, shape.d, shape.H, shape.V, shape.page, max_sessions=n)
+        out = torch.full(sb.q.shape, float("nan"), dtype=torch.bfloat16, device="cuda")
+        status = ctx.entry_attn(sb.q, sb.k_new, sb.v_new, sb.k_pool, sb.v_pool, sb.page_table, sb.n_s, sb.l_entry,
+                                sb.capacity, out)
+        ctx.sync()
+        assert status == [0] * n
+        assert torch.isfinite(out.float()).all()
+        assert torch.equal(sb.k_pool.view(torch.int16), ke.view(torch.int16)), "K pool: append / untouched mismatch"
+        assert torch.equal(sb.v_pool.view(torch.int16), ve.view(torch.int16)), "V pool: append / untouched mismatch"
+        del ke, ve
+        for s in full:
+            worst = max(worst, _check_session_every_row(oracle, sb, s, out, pristine[s]))
+            assert worst <= ATTN_ATOL, (name, bi, s, worst)
+        for s in sampled:
+            worst = max(worst, _check_samples(oracle, sb, s, out, samples[s], slices[s]))
+            assert worst <= ATTN_ATOL, (name, bi, s, worst)
+        ctx.close()
+        del sb, out, pristine, slices
+        torch.cuda.empty_cache()
     assert worst <= ATTN_ATOL, worst
 
 

@@ -147,6 +147,65 @@ def test_config3_trace_invalidate_never_serves_stale(prepos, oracle):
     assert prepos.unpack_records(recs)["flags"].tolist() == [0, 0]
 
 
+def test_publication_is_safe_across_streams(prepos, oracle):
+    """Sec. 3.6 with writer and reader on DIFFERENT streams over ONE record: stream A loops
+    invalidate + ready_dist, alternating a hidden row X (top-1 a in A, gap well above tau) and a row Y (top-1 b in A,
+    b != a, gap well below tau); stream B loops batched gate serves on the same record.  The oracle's two records
+    give the only legal (top1, gap) pairs, so the only token that may ever be SERVED is a: a serve that paired Y's
+    top-1 with X's gap (fields of two publications) would return b.  Every served record must also have been fresh:
+    the decision buffer is checked against the two legal outcomes per request."""
+    shape = synth.Shape("pub", layers=1, Hq=4, Hkv=2, d=64, H=256, V=2048, fast_set=32, tau=3.0, planted_frac=1.0)
+    seed = 4242
+    w = synth.make_w_vocab(shape, seed)
+    fast = synth.make_fast_set(shape, seed)
+    pool, _, _ = synth.make_hidden(shape, 24, w, fast, seed)
+    from helpers import bits
+    refs = [oracle.record(oracle.logits(bits(w), bits(pool[r]))) for r in range(24)]
+    in_a = set(fast.tolist())
+    xs = [r for r in range(24) if refs[r].gap >= shape.tau + 0.5 and refs[r].top1 in in_a]
+    assert xs
+    x = xs[0]
+    ys = [r for r in range(24) if 0.2 <= refs[r].gap <= shape.tau - 0.5 and refs[r].top1 in in_a and refs[r].top1 != refs[x].top1]
+    assert ys
+    y = ys[0]
+    a_tok = refs[x].top1
+    ctx_w = prepos.Context(1, 4, 2, 64, 256, 2048, 16, max_sessions=2)
+    ctx_r = prepos.Context(1, 4, 2, 64, 256, 2048, 16, max_sessions=2)
+    wd, pd = w.cuda(), pool.cuda()
+    recs = prepos.new_records(1)
+    ver = torch.zeros(1, dtype=torch.int64, device="cuda")
+    sid = torch.zeros(1, dtype=torch.int32, device="cuda")
+    bm = prepos.fastset_build(fast, shape.V).cuda()
+    iters, B = 400, 256
+    req = torch.zeros(B, dtype=torch.int32, device="cuda")
+    decs = torch.full((2 * iters, B), -9, dtype=torch.int32, device="cuda")
+    toks = torch.full((2 * iters, B), -9, dtype=torch.int32, device="cuda")
+    exp = torch.arange(1, iters + 1, dtype=torch.int64, device="cuda")   # the version after the i-th invalidate
+    sa, sb_ = torch.cuda.Stream(), torch.cuda.Stream()
+    torch.cuda.synchronize()
+    for i in range(iters):
+        with torch.cuda.stream(sa):
+            ctx_w.invalidate(sid, ver, recs)
+            r = x if i % 2 == 0 else y
+            ctx_w.ready_dist(sid, pd[r:r + 1], wd, recs, ver, expected_version=exp[i:i + 1])
+        with torch.cuda.stream(sb_):
+            for k in range(2):
+                ctx_r.gate_serve(req, recs, ver, bm, shape.tau, decs[2 * i + k], toks[2 * i + k])
+    torch.cuda.synchronize()
+    d, t = decs.cpu().numpy(), toks.cpu().numpy()
+    assert set(np.unique(d).tolist()) <= {prepos.SERVED, prepos.GAP_BELOW_TAU, prepos.STALE_OR_INVALID}
+    served = d == prepos.SERVED
+    assert (t[served] == a_tok).all(), f"served tokens {np.unique(t[served])}, legal: {a_tok}"
+    assert (t[~served] == -1).all()
+    # and in stream order the last publication (row y: gap below tau) is what a serve sees
+    ctx_r.gate_serve(req, recs, ver, bm, shape.tau, decs[0], toks[0])
+    ctx_r.sync()
+    last = x if (iters - 1) % 2 == 0 else y
+    want = prepos.SERVED if last == x else prepos.GAP_BELOW_TAU
+    assert (decs[0].cpu().numpy() == want).all()
+    assert prepos.unpack_records(recs)["seq"].tolist() == [iters]
+
+
 def test_gate_sweep_matches_oracle_risk_coverage(prepos, oracle):
     """prepos_gate_sweep (Eq. 13-14) on records the GPU produced itself: 512 sessions of the
     tiny config with planted margins, a third of them invalidated, full-path tokens that disagree on some rows;

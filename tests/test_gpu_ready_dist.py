@@ -117,6 +117,61 @@ def test_record_stamping_skip_and_ids(prepos, oracle):
         check_record(oracle, rec, s, oracle.logits(bits(w), bits(hidden[row])))
 
 
+def test_expected_version_stamp_and_publication_sequence(prepos, oracle):
+    """Sec. 3.6: the record is stamped with the version its inputs were computed at
+    (`expected_version`), and is VALID only if that is still the live version when the pass ends; a record computed
+    for an older state is written but never served.  Each publication advances the sequence number in flags[2:]."""
+    shape = synth.Shape("ev", layers=1, Hq=4, Hkv=2, d=64, H=128, V=300, fast_set=2)
+    w = synth.make_w_vocab(shape, 21).cuda()
+    hidden = synth.randn_bf16((3, 128), synth.gen(22)).cuda()
+    ctx = prepos.Context(1, 4, 2, 64, 128, 300, 16, max_sessions=4)
+    sid = torch.tensor([0, 1, 2], dtype=torch.int32, device="cuda")
+    ver = torch.tensor([5, 6, 7], dtype=torch.int64, device="cuda")
+    exp = torch.tensor([5, 5, 8], dtype=torch.int64, device="cuda")      # fresh, computed at an older state, newer
+    recs = prepos.new_records(3)
+    bm = prepos.fastset_build(list(range(300)), 300).cuda()
+    dec = torch.zeros(3, dtype=torch.int32, device="cuda")
+    tok = torch.zeros(3, dtype=torch.int32, device="cuda")
+    for rnd in range(3):
+        ctx.ready_dist(sid, hidden, w, recs, ver, expected_version=exp)
+        ctx.gate_serve(sid, recs, ver, bm, -1e30, dec, tok)
+        ctx.sync()
+        rec = prepos.unpack_records(recs)
+        assert rec["flags"].tolist() == [1, 0, 0] and rec["version"].tolist() == [5, 5, 8]
+        assert rec["seq"].tolist() == [rnd + 1] * 3
+        assert dec.cpu().tolist() == [prepos.SERVED, prepos.STALE_OR_INVALID, prepos.STALE_OR_INVALID]
+        check_record(oracle, rec, 1, oracle.logits(bits(w), bits(hidden[1])))    # written, just not valid
+    # a mutation that commits on ANOTHER stream while the pre-position runs must win: full-size vocabulary
+    # (~0.17 ms of streaming), the bump is issued right behind it on a second stream
+    shape2 = synth.C2
+    w2 = synth.make_w_vocab(shape2, 23, "cuda")
+    h2 = synth.randn_bf16((1, shape2.H), synth.gen(24, "cuda"))
+    ctx2 = prepos.Context(shape2.layers, shape2.Hq, shape2.Hkv, shape2.d, shape2.H, shape2.V, 16, max_sessions=1)
+    s0 = torch.zeros(1, dtype=torch.int32, device="cuda")
+    bm2 = prepos.fastset_build(list(range(0, shape2.V, 2)), shape2.V).cuda()
+    a, b = torch.cuda.Stream(), torch.cuda.Stream()
+    raced = 0
+    for it in range(20):
+        recs2 = prepos.new_records(1)
+        ver2 = torch.zeros(1, dtype=torch.int64, device="cuda")
+        exp2 = torch.zeros(1, dtype=torch.int64, device="cuda")
+        d2 = torch.zeros(1, dtype=torch.int32, device="cuda")
+        t2 = torch.zeros(1, dtype=torch.int32, device="cuda")
+        torch.cuda.synchronize()
+        with torch.cuda.stream(a):
+            ctx2.ready_dist(s0, h2, w2, recs2, ver2, expected_version=exp2)
+        with torch.cuda.stream(b):
+            ctx.invalidate(s0, ver2, recs2)
+        torch.cuda.synchronize()
+        ctx2.gate_serve(s0, recs2, ver2, bm2, -1e30, d2, t2)
+        ctx2.sync()
+        r2 = prepos.unpack_records(recs2)
+        assert int(ver2[0]) == 1 and int(r2["version"][0]) == 0          # stamped with the state it was computed at
+        assert (int(d2[0]), int(t2[0])) == (prepos.STALE_OR_INVALID, -1)
+        raced += int(r2["flags"][0]) == 0
+    # (informational: `raced` counts the runs where the bump landed before the pass ended)
+
+
 def test_nonfinite_logit_is_flagged_and_never_served(prepos, oracle):
     shape = synth.Shape("n", layers=1, Hq=4, Hkv=2, d=64, H=128, V=256, fast_set=2)
     w = synth.make_w_vocab(shape, 13)
@@ -167,12 +222,14 @@ def test_scan_logits_matches_oracle_and_shift_invariance(prepos, oracle):
             assert (int(rr["top1"][r]), int(rr["top2"][r])) == (ref.top1, ref.top2)
 
 
-@pytest.mark.parametrize("name,n", [("c2", 1), ("c2", 12), ("c4", 64), ("c5", 1)])
+@pytest.mark.parametrize("name,n", [("c2", 1), ("c2", 12), ("c4", 64), ("c5", 1), ("c5", 4)])
 def test_full_size_vocabulary(prepos, oracle, name, n):
     """BASELINE configs 2, 4 and 5 vocabulary side at full size (V=128256, H=4096 / 8192), in the launch
     configurations bench.py times: one hidden row (streaming kernel), 12 rows and the 64-session batch of config 4
     (one pass of the batched tensor-core kernel), planted fraction 0.6: full logits + records against the oracle;
-    for config 4 also its 4096 gate serves over the 64 records, every decision against O4."""
+    for config 4 also its 4096 gate serves over the 64 records, every decision against O4.  Config 5 with n = 4 is
+    the record of every session bench.py keeps resident.  Config 3's vocabulary side is config 2's launch (same V,
+    H, W_vocab recipe and one hidden row), so ("c2", 1) covers it."""
     shape = {"c2": synth.C2, "c4": synth.C4, "c5": synth.C5}[name]
     seed = synth.SEED_BASE + int(name[1])
     w = synth.make_w_vocab(shape, seed, "cuda")
