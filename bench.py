@@ -804,6 +804,122 @@ def run_scan_logits(wl, prepos, reps=50):
     return res
 
 
+def run_ready_dist_w4(wl, prepos, reps=30):
+    """SURVEY.md 8(f) NEXT-4 (the paper's headline model "runs at 4-bit precision"; format per
+    DESIGN.md reading Q21): prepos_ready_dist_w4 -- the same record from int4 codes + one bf16 scale per (row, 128 k)
+    -- beside the bf16 call it replaces.  Algorithmic bytes: V*H/2 codes + V*H/64 scale bytes + the hidden rows, per
+    pass of up to 8 rows.  Rotates over two copies of the codes (each is larger than L2)."""
+    dev, s = wl.dev, wl.spec["shape"]
+    n = min(wl.n, 8)
+    sets = [synth.make_w_vocab_w4(s, wl.spec["seed"] + 11 * r, dev) for r in range(2)]
+    hidden = wl.sets[0]["hidden"][:n].contiguous()
+    sid = torch.arange(n, dtype=torch.int32, device=dev)
+    recs = prepos.new_records(n, dev)
+    ver = torch.zeros(n, dtype=torch.int64, device=dev)
+    ctx = prepos.Context(s.layers, s.Hq, s.Hkv, s.d, s.H, s.V, s.page, max_sessions=n)
+    ev = []
+    for i in range(reps + 5):
+        w4, sc = sets[i % 2]
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        ctx.ready_dist_w4(sid, hidden, w4, sc, recs, ver)
+        b.record()
+        ev.append((a, b))
+    torch.cuda.synchronize()
+    ms = sorted(a.elapsed_time(b) for a, b in ev[5:])
+    ctx.close()
+    nbytes = s.V * s.H // 2 + s.V * (s.H // 128) * 2 + n * s.H * 2 + n * 48
+    med = statistics.median(ms)
+    return {"rows": n, "ms_median": round(med, 5), "ms_min": round(ms[0], 5), "algorithmic_bytes": nbytes,
+            "achieved_gbs": round(nbytes / (med * 1e-3) / 1e9, 1),
+            "frac_of_measured_hbm": round(nbytes / (med * 1e-3) / 1e9 / peaks()["hbm"], 4),
+            "bf16_call_algorithmic_bytes": s.V * s.H * 2 + n * s.H * 2 + n * 48}
+
+
+def run_yield(wl, prepos, trials=40):
+    """SURVEY.md 8(f) NEXT-2, the request that needs whole SMs ("yields immediately"; Eq. 5 / Eq. 7): the
+    fall-through decode step of one session (L = 1, all layers, its own ctx) issued on a high-priority stream while the
+    pre-position's attention pass (ONE launch, all layers: no caller-side layer chopping) runs on the low-priority
+    stream.  The request first calls prepos_ctx_request_yield: the pass stops at its next segment boundaries, the
+    decode step takes the SMs, and prepos_entry_attn_resume finishes the pass afterwards.  Reported: wall time of the
+    decode step idle / behind the un-yielded pass / with the yield; and what the yield costs the pass (device time of
+    launch + resume against the uninterrupted launch)."""
+    dev, s = wl.dev, wl.spec["shape"]
+    if s.layers < 8:
+        return None
+    s_lo, s_hi = torch.cuda.Stream(priority=0), torch.cuda.Stream(priority=-1)
+    sb0 = wl.sets[0]["sb"]
+    ctx3 = prepos.Context(s.layers, s.Hq, s.Hkv, s.d, s.H, s.V, s.page, max_sessions=1)
+    q1 = sb0.q[:, :1].contiguous()
+    k1, v1 = sb0.k_new[:, :1].contiguous(), sb0.v_new[:, :1].contiguous()
+    o1 = torch.empty_like(q1)
+    ns1, l1, cap1 = wl.n_s_h[:1].clone(), torch.ones(1, dtype=torch.int32), wl.cap_h[:1].clone()
+    q = lambda v, p: round(v[min(len(v) - 1, int(len(v) * p))], 1) if v else None
+
+    def attn(i):
+        st = wl.sets[i % len(wl.sets)]
+        sb = st["sb"]
+        wl.ctx.entry_attn(sb.q, sb.k_new, sb.v_new, sb.k_pool, sb.v_pool, sb.page_table, wl.n_s_h, wl.l_h, wl.cap_h, st["out"])
+
+    def decode(yield_first):
+        t0 = time.perf_counter()
+        with torch.cuda.stream(s_hi):
+            if yield_first:
+                wl.ctx.request_yield()
+            ctx3.entry_attn(q1, k1, v1, sb0.k_pool, sb0.v_pool, sb0.page_table[:1], ns1, l1, cap1, o1)
+        s_hi.synchronize()
+        return (time.perf_counter() - t0) * 1e6
+
+    for _ in range(5):
+        decode(False)
+    idle = sorted(decode(False) for _ in range(trials))
+    # the uninterrupted pass, device time
+    ev = []
+    for i in range(6):
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        with torch.cuda.stream(s_lo):
+            a.record(s_lo)
+            attn(i)
+            b.record(s_lo)
+        ev.append((a, b))
+    torch.cuda.synchronize()
+    pass_ms = statistics.median(a.elapsed_time(b) for a, b in ev[1:])
+    res = {"idle_wall_us_p50": q(idle, 0.5), "pass_ms_uninterrupted": round(pass_ms, 4)}
+    rng = np.random.default_rng(wl.spec["seed"])
+    for label, use_yield in (("behind_the_pass_no_yield", False), ("with_yield", True)):
+        got, cost, caught = [], [], 0
+        for i in range(trials):
+            a, b, c = (torch.cuda.Event(enable_timing=True) for _ in range(3))
+            with torch.cuda.stream(s_lo):
+                a.record(s_lo)
+                attn(i)
+                b.record(s_lo)
+            # the request arrives somewhere inside the pass
+            time.sleep(float(rng.uniform(0.15, 0.7)) * pass_ms * 1e-3)
+            running = not b.query()
+            v = decode(use_yield)
+            if use_yield:
+                with torch.cuda.stream(s_lo):
+                    pend = wl.ctx.entry_attn_pending()
+                    caught += int(pend)
+                    wl.ctx.entry_attn_resume()
+                    c.record(s_lo)
+            torch.cuda.synchronize()
+            if running:
+                got.append(v)
+                if use_yield:
+                    cost.append(a.elapsed_time(c))
+        got.sort()
+        res[label] = {"p50": q(got, 0.5), "p90": q(got, 0.9), "samples": len(got)}
+        if use_yield:
+            res[label]["passes_caught_running"] = caught
+            if cost:
+                # start of the pass to end of its resume, which includes the decode step that ran in between
+                res[label]["pass_plus_decode_plus_resume_ms_median"] = round(statistics.median(cost), 4)
+    ctx3.close()
+    return res
+
+
 def run_update_trace(wl, prepos, n_steps=1000):
     """BASELINE configs[2]'s trace at the config's real vocabulary shape (reading Q16; "triggered after a
     data update"): per update, with probability 0.3 the state version is bumped (prepos_invalidate); then one gate
@@ -1038,8 +1154,13 @@ def run_config(name, args, d, dev, prepos):
             line["fall_through"] = ft
         if d.world == 1:
             line["co_schedule"] = run_co_schedule(wl, prepos)
+            y = run_yield(wl, prepos)
+            if y:
+                line["co_schedule"]["decode_step_with_yield_wall_us"] = y
         if name in ("c2", "c5"):
             line["scan_logits"] = run_scan_logits(wl, prepos)
+        if name in ("c2", "c4", "c5"):
+            line["ready_dist_w4"] = run_ready_dist_w4(wl, prepos)
         if name == "c3":
             line["update_trace"] = run_update_trace(wl, prepos)
     del wl

@@ -166,6 +166,61 @@ int prepos_entry_attn(prepos_ctx *ctx, int layer_begin, int layer_end, int n_ses
                       int32_t *status_per_session, float softmax_scale, void *stream);
 
 /*
+ * prepos_entry_attn over an FP8 KV cache (the paper's headline model "runs at 4-bit
+ * precision", without naming a storage format: DESIGN.md reading Q20).  Same call, same budget
+ * check, same outputs; the session's pages hold OCP e4m3 codes (1-4-3, bias 7, no infinities, max 448):
+ *   k_pool8, v_pool8  DEVICE uint8 [layer][n_pages][Hkv][page_size][d], layer stride pool_layer_stride BYTES (a
+ *                     multiple of 16); d a multiple of 16
+ *   k_scale, v_scale  DEVICE fp32 [layer][n_pages][Hkv], layer stride scale_layer_stride elements: one positive scale
+ *                     per (layer, page, kv head), caller-owned, for EVERY page of the session including the ones the
+ *                     entry is appended to; cached value = decode(code) * scale
+ * Append(E) (Alg. 1 l.5) stores code = e4m3(fp32(x) / scale), division and conversion round-to-nearest-even,
+ * saturating at +-448, for every entry token; Forward(E) (l.6) runs after it, so entry row i sees the entry tokens
+ * j' <= i through their stored codes (pre-positioning L1 then L2 tokens equals pre-positioning L1 + L2).  q, k_new,
+ * v_new and out stay bf16; softmax and accumulation are fp32 as in prepos_entry_attn.
+ */
+int prepos_entry_attn_fp8(prepos_ctx *ctx, int layer_begin, int layer_end, int n_sessions,
+                          const void *q, int64_t q_layer_stride,
+                          const void *k_new, const void *v_new, int64_t kv_new_layer_stride,
+                          void *k_pool8, void *v_pool8, int64_t pool_layer_stride, int64_t n_pages,
+                          const float *k_scale, const float *v_scale, int64_t scale_layer_stride,
+                          const int32_t *page_table, int page_table_stride,
+                          const int32_t *n_s, const int32_t *l_entry, const int32_t *capacity_tokens,
+                          void *out, int64_t out_layer_stride,
+                          int32_t *status_per_session, float softmax_scale, void *stream);
+
+/*
+ * Yield and resume ("runs at the lowest scheduling priority and yields
+ * immediately", Alg. 1 l.1, Eq. 7).  The tcgen05 attention pass is a persistent kernel that
+ * holds every SM; a request that needs whole SMs (the fall-through decode step, Eq. 5) would wait for it to end.
+ * Its CTAs therefore have a yield point at every segment boundary (a segment = the CTA's part of one
+ * (layer, kv head, session row chunk), at most n_s / 128 + 1 KV tiles):
+ *
+ *   prepos_ctx_request_yield   sets the ctx's device yield flag with a 4-byte copy on `stream` (use the request's
+ *                              high-priority stream; the copy engine does not wait for the running kernel).  Every
+ *                              CTA of the running pass finishes its current segment, records how many segments it has
+ *                              completed, and exits; the SMs go to whatever is queued at higher priority.  Outputs of
+ *                              finished segments are final, partials of cut units stay in the ctx workspace.
+ *   prepos_entry_attn_resume   clears the flag and re-issues the SAME launch on `stream`: every CTA skips the
+ *                              segments it completed and carries on.  The result is the one an uninterrupted call
+ *                              gives, bit for bit (same plan, same split, same merge order).  A no-op launch when
+ *                              the pass had already finished; PREPOS_OK without a launch when nothing is open.
+ *   prepos_entry_attn_pending  synchronises `stream` and tells whether the ctx's last attention launch stopped at a
+ *                              yield point (1) or ran to completion (0).
+ *   prepos_ctx_set_attn_slice  n > 0: every launch (the first and each resume) runs at most n segments per CTA --
+ *                              a bounded-residency pass for callers that prefer time slices to a flag; 0 = off.
+ *
+ * Between a yield and its resume the ctx must not be given another prepos_entry_attn call (it would reuse the
+ * workspace the stopped pass still needs; doing so abandons the stopped pass), and nothing queued behind the
+ * stopped launch on its stream may read `out`.  Request a yield only while no further attention call of this ctx is
+ * queued behind the running one.  The generic CUDA-core path has no yield point (its CTAs are short-lived).
+ */
+int prepos_ctx_request_yield(prepos_ctx *ctx, void *stream);
+int prepos_entry_attn_resume(prepos_ctx *ctx, void *stream);
+int prepos_entry_attn_pending(prepos_ctx *ctx, void *stream, int32_t *pending_out /* HOST */);
+int prepos_ctx_set_attn_slice(prepos_ctx *ctx, int max_segments_per_launch);
+
+/*
  * Alg. 1 l.6 (LM head) + l.10-12 and Alg. 2 l.3-4 (Eq. 11):
  * logits l_v = sum_k W[v][k] x_r[k] for each of n hidden rows, reduced in the same pass to the
  * record {max, lse, top1, top2, gap} under the order (logit desc, id asc).  records[session_ids[r]]
@@ -189,6 +244,23 @@ int prepos_ready_dist(prepos_ctx *ctx, int n, const int32_t *session_ids,
                       const int64_t *position_p, const uint64_t *entry_hash, const int32_t *skip_mask,
                       prepos_record *records, const uint64_t *session_version,
                       const uint64_t *expected_version, float *logits_out, void *stream);
+
+/*
+ * prepos_ready_dist over a 4-bit W_vocab (the paper's headline model "runs at 4-bit
+ * precision", without naming a format: DESIGN.md reading Q21).  Same record, same stamping and
+ * publication, same optional logits_out as prepos_ready_dist; only the weights differ:
+ *   w4      DEVICE uint8 [V][H/2]: two's-complement int4 codes in -8..7, two per byte, the element with even k in the
+ *           low nibble
+ *   w_scale DEVICE bf16 [V][H/128]: one scale per (vocabulary row, group of 128 consecutive k)
+ *   W[v][k] = code[v][k] * w_scale[v][k / 128]; l_v = sum_k W[v][k] x[k].  The kernel widens the codes exactly,
+ *   accumulates each group in fp32 and multiplies the group sum by its scale: no weight is ever rounded.
+ * The pass reads V*H/2 + V*H/64 bytes per 8 hidden rows (a batch of n rows takes ceil(n / 8) passes).
+ */
+int prepos_ready_dist_w4(prepos_ctx *ctx, int n, const int32_t *session_ids,
+                         const void *hidden, const void *w4, const void *w_scale,
+                         const int64_t *position_p, const uint64_t *entry_hash, const int32_t *skip_mask,
+                         prepos_record *records, const uint64_t *session_version,
+                         const uint64_t *expected_version, float *logits_out, void *stream);
 
 /*
  * Alg. 2 l.3-4 on stored logits (the paper's serve-time vocabulary scan, Eq. 3):

@@ -13,7 +13,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 SO = os.path.join(HERE, "libprepos.so")
-SOURCES = ["api.cu", "gate.cu", "ready_dist.cu", "attn_generic.cu", "attn_umma.cu"]
+SOURCES = ["api.cu", "gate.cu", "ready_dist.cu", "attn_generic.cu", "attn_fp8.cu", "attn_umma.cu"]
 HEADERS = ["common.cuh", "ptx.cuh", os.path.join("..", "..", "include", "prepos.h")]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo",

@@ -18,7 +18,7 @@ size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 bool aligned16(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15) == 0; }
 
 struct WsLayout {
-    size_t rd_partials, rd_counter, attn_units, attn_partials, attn_counters, total;
+    size_t rd_partials, rd_counter, attn_units, attn_partials, attn_counters, attn_yield, total;
     int max_units;
     size_t attn_counters_n;
 };
@@ -44,6 +44,8 @@ WsLayout ws_layout(const prepos_model_shape &s, int max_sessions)
     w.attn_counters_n = static_cast<size_t>(s.layers) * s.n_kv_heads * w.max_units;
     w.attn_counters = off;
     off = align_up(off + sizeof(unsigned int) * w.attn_counters_n, 256);
+    w.attn_yield = off;   // yield flag, pass state, per-CTA progress
+    off = align_up(off + 256 + sizeof(int) * kAttnMaxCtas, 256);
     w.total = off;
     return w;
 }
@@ -149,6 +151,16 @@ int prepos_ctx_create(prepos_ctx **out, const prepos_model_shape *shape, int max
     c->attn_partials = reinterpret_cast<float *>(c->ws + w.attn_partials);
     c->attn_counters = reinterpret_cast<unsigned int *>(c->ws + w.attn_counters);
     c->attn_counters_n = w.attn_counters_n;
+    c->attn_yield_flag = reinterpret_cast<unsigned int *>(c->ws + w.attn_yield);
+    c->attn_pass_state = c->attn_yield_flag + 1;
+    c->attn_progress = reinterpret_cast<int *>(c->ws + w.attn_yield + 256);
+    c->yield_host = nullptr;
+    c->attn_launch_seq = 0;
+    c->attn_slice = 0;
+    c->yield_dirty = false;
+    c->pass_open = false;
+    c->pass_grid = c->pass_merge_grid = c->pass_head_dim = 0;
+    c->pass_smem = 0;
     c->plan_staging = nullptr;
     c->plan_inflight = false;
     c->tm_k_ptr = c->tm_v_ptr = nullptr;
@@ -160,11 +172,18 @@ int prepos_ctx_create(prepos_ctx **out, const prepos_model_shape *shape, int max
     // arrival counters start at zero and are reset by their last arriver
     cudaError_t e = cudaMemset(c->rd_counter, 0, sizeof(unsigned int) * (kRdMaxRows + 1));
     if (e == cudaSuccess) e = cudaMemset(c->attn_counters, 0, sizeof(unsigned int) * c->attn_counters_n);
+    if (e == cudaSuccess) e = cudaMemset(c->ws + w.attn_yield, 0, 256 + sizeof(int) * kAttnMaxCtas);
+    if (e == cudaSuccess) e = cudaMallocHost(reinterpret_cast<void **>(&c->yield_host), 2 * sizeof(unsigned int));
+    if (e == cudaSuccess) {
+        c->yield_host[0] = 1u;
+        c->yield_host[1] = 0u;
+    }
     if (e == cudaSuccess) e = cudaMallocHost(reinterpret_cast<void **>(&c->plan_staging), sizeof(AttnUnit) * c->max_units);
     if (e == cudaSuccess) e = cudaEventCreateWithFlags(&c->plan_copied, cudaEventDisableTiming);
     if (e != cudaSuccess) {
         prepos_note_cuda_error(e, "ctx setup", __FILE__, __LINE__);
         if (c->plan_staging) cudaFreeHost(c->plan_staging);
+        if (c->yield_host) cudaFreeHost(c->yield_host);
         delete c;
         return PREPOS_E_CUDA;
     }
@@ -178,6 +197,7 @@ int prepos_ctx_destroy(prepos_ctx *ctx)
     if (ctx->plan_inflight) cudaEventSynchronize(ctx->plan_copied);
     cudaEventDestroy(ctx->plan_copied);
     cudaFreeHost(ctx->plan_staging);
+    cudaFreeHost(ctx->yield_host);
     delete ctx;
     return PREPOS_OK;
 }
@@ -201,35 +221,23 @@ int prepos_ctx_set_attn_path(prepos_ctx *ctx, int path)
     return PREPOS_OK;
 }
 
-int prepos_entry_attn(prepos_ctx *ctx, int layer_begin, int layer_end, int n_sessions, const void *q,
-                      int64_t q_layer_stride, const void *k_new, const void *v_new, int64_t kv_new_layer_stride,
-                      void *k_pool, void *v_pool, int64_t pool_layer_stride, int64_t n_pages,
-                      const int32_t *page_table, int page_table_stride, const int32_t *n_s, const int32_t *l_entry,
-                      const int32_t *capacity_tokens, void *out, int64_t out_layer_stride,
-                      int32_t *status_per_session, float softmax_scale, void *stream)
+}  // extern "C" (reopened below: the attention entry points share a host-side planner)
+
+namespace {
+
+// Host-side attention plan shared by the bf16 and the FP8 entry points: argument checks, Alg. 1 l.2-3 budget check
+// (PAPER.md:145-146), one AttnUnit per (session, row chunk of `chunk_tok` entry tokens), cached on the batch
+// geometry and uploaded to the ctx workspace when it changes.  `mode` separates plans of different kernels.
+// `entries_in_cache`: the entry tokens are read from the session's pages like cached ones (the FP8 path appends
+// their codes first), so a unit's tiles cover n_s + tok0 + ntok tokens and it has no entry tiles.
+int plan_attn(prepos_ctx *ctx, int mode, int chunk_tok, bool entries_in_cache, int n_sessions, int page_table_stride,
+              const int32_t *n_s, const int32_t *l_entry, const int32_t *capacity_tokens, int32_t *status_per_session,
+              cudaStream_t stream)
 {
-    if (!ctx) return PREPOS_E_INVALID_ARG;
     const prepos_model_shape &s = ctx->shape;
-    if (layer_begin < 0 || layer_end > s.layers || layer_begin > layer_end || n_sessions < 0) return PREPOS_E_INVALID_ARG;
-    if (n_sessions > ctx->max_sessions) return PREPOS_E_WORKSPACE;
-    if (n_sessions == 0 || layer_begin == layer_end) return PREPOS_OK;
-    if (!q || !k_new || !v_new || !k_pool || !v_pool || !page_table || !n_s || !l_entry || !capacity_tokens || !out)
-        return PREPOS_E_INVALID_ARG;
-    if (!aligned16(q) || !aligned16(k_new) || !aligned16(v_new) || !aligned16(k_pool) || !aligned16(v_pool) ||
-        !aligned16(out) || !aligned16(page_table))
-        return PREPOS_E_ALIGN;
-    if ((q_layer_stride | kv_new_layer_stride | pool_layer_stride | out_layer_stride) & 7) return PREPOS_E_ALIGN;
-    if (n_pages <= 0 || page_table_stride <= 0) return PREPOS_E_INVALID_ARG;
-
-    const int G = s.n_q_heads / s.n_kv_heads;
-    const bool use_umma = (ctx->attn_path == 2) || (ctx->attn_path == 0 && prepos_attn_umma_supported(ctx));
-    // row chunk: entry tokens whose G rows share one unit
-    const int chunk_tok = use_umma ? (kAttnMaxRows / G > 0 ? kAttnMaxRows / G : 1) : (G > 16 ? 1 : 16 / G);
-
-    // ---- plan key: reuse the device copy of the plan when the batch geometry is unchanged
     std::vector<int32_t> key;
     key.reserve(3 * n_sessions + 3);
-    key.push_back(use_umma ? 2 : 1);
+    key.push_back(mode);
     key.push_back(n_sessions);
     key.push_back(page_table_stride);   // the plan was checked against this stride
     for (int i = 0; i < n_sessions; ++i) {
@@ -258,8 +266,15 @@ int prepos_entry_attn(prepos_ctx *ctx, int layer_begin, int layer_end, int n_ses
                     u.tok0 = tok0;
                     u.ntok = (L - tok0 < chunk_tok) ? L - tok0 : chunk_tok;
                     u.row0 = row0;
-                    u.n_cached_tiles = (n_s[i] + kAttnTileTokens - 1) / kAttnTileTokens;
-                    u.n_tiles = u.n_cached_tiles + (tok0 + u.ntok + kAttnTileTokens - 1) / kAttnTileTokens;
+                    if (entries_in_cache) {
+                        u.n_load = n_s[i] + tok0 + u.ntok;
+                        u.n_cached_tiles = (u.n_load + kAttnTileTokens - 1) / kAttnTileTokens;
+                        u.n_tiles = u.n_cached_tiles;
+                    } else {
+                        u.n_load = n_s[i];
+                        u.n_cached_tiles = (n_s[i] + kAttnTileTokens - 1) / kAttnTileTokens;
+                        u.n_tiles = u.n_cached_tiles + (tok0 + u.ntok + kAttnTileTokens - 1) / kAttnTileTokens;
+                    }
                     u.tile_prefix = prefix;
                     prefix += u.n_tiles;
                     units.push_back(u);
@@ -277,17 +292,60 @@ int prepos_entry_attn(prepos_ctx *ctx, int layer_begin, int layer_end, int n_ses
         if (!ctx->plan_units.empty()) {
             memcpy(ctx->plan_staging, ctx->plan_units.data(), sizeof(AttnUnit) * ctx->plan_units.size());
             PREPOS_CUDA_TRY(cudaMemcpyAsync(ctx->attn_units, ctx->plan_staging, sizeof(AttnUnit) * ctx->plan_units.size(),
-                                            cudaMemcpyHostToDevice, static_cast<cudaStream_t>(stream)));
-            PREPOS_CUDA_TRY(cudaEventRecord(ctx->plan_copied, static_cast<cudaStream_t>(stream)));
+                                            cudaMemcpyHostToDevice, stream));
+            PREPOS_CUDA_TRY(cudaEventRecord(ctx->plan_copied, stream));
             ctx->plan_inflight = true;
         }
     }
     if (status_per_session)
         for (int i = 0; i < n_sessions; ++i)
             status_per_session[i] = (l_entry[i] > capacity_tokens[i] - n_s[i]) ? PREPOS_SKIPPED_BUDGET : PREPOS_OK;
+    ctx->pass_open = false;
+    if (ctx->yield_dirty) {
+        // a yield was requested since the last clear: drop a request that outlived its pass, and the arrival counters
+        // of a pass that was stopped and never resumed
+        PREPOS_CUDA_TRY(cudaMemsetAsync(ctx->attn_yield_flag, 0, sizeof(unsigned int), stream));
+        PREPOS_CUDA_TRY(cudaMemsetAsync(ctx->attn_counters, 0, sizeof(unsigned int) * ctx->attn_counters_n, stream));
+        ctx->yield_dirty = false;
+    }
+    return PREPOS_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int prepos_entry_attn(prepos_ctx *ctx, int layer_begin, int layer_end, int n_sessions, const void *q,
+                      int64_t q_layer_stride, const void *k_new, const void *v_new, int64_t kv_new_layer_stride,
+                      void *k_pool, void *v_pool, int64_t pool_layer_stride, int64_t n_pages,
+                      const int32_t *page_table, int page_table_stride, const int32_t *n_s, const int32_t *l_entry,
+                      const int32_t *capacity_tokens, void *out, int64_t out_layer_stride,
+                      int32_t *status_per_session, float softmax_scale, void *stream)
+{
+    if (!ctx) return PREPOS_E_INVALID_ARG;
+    const prepos_model_shape &s = ctx->shape;
+    if (layer_begin < 0 || layer_end > s.layers || layer_begin > layer_end || n_sessions < 0) return PREPOS_E_INVALID_ARG;
+    if (n_sessions > ctx->max_sessions) return PREPOS_E_WORKSPACE;
+    if (n_sessions == 0 || layer_begin == layer_end) return PREPOS_OK;
+    if (!q || !k_new || !v_new || !k_pool || !v_pool || !page_table || !n_s || !l_entry || !capacity_tokens || !out)
+        return PREPOS_E_INVALID_ARG;
+    if (!aligned16(q) || !aligned16(k_new) || !aligned16(v_new) || !aligned16(k_pool) || !aligned16(v_pool) ||
+        !aligned16(out) || !aligned16(page_table))
+        return PREPOS_E_ALIGN;
+    if ((q_layer_stride | kv_new_layer_stride | pool_layer_stride | out_layer_stride) & 7) return PREPOS_E_ALIGN;
+    if (n_pages <= 0 || page_table_stride <= 0) return PREPOS_E_INVALID_ARG;
+
+    const int G = s.n_q_heads / s.n_kv_heads;
+    const bool use_umma = (ctx->attn_path == 2) || (ctx->attn_path == 0 && prepos_attn_umma_supported(ctx));
+    // row chunk: entry tokens whose G rows share one unit
+    const int chunk_tok = use_umma ? (kAttnMaxRows / G > 0 ? kAttnMaxRows / G : 1) : (G > 16 ? 1 : 16 / G);
+    const int st = plan_attn(ctx, use_umma ? 2 : 1, chunk_tok, false, n_sessions, page_table_stride, n_s, l_entry,
+                             capacity_tokens, status_per_session, static_cast<cudaStream_t>(stream));
+    if (st != PREPOS_OK) return st;
     if (ctx->plan_units.empty()) return PREPOS_OK;
 
     AttnArgs a;
+    memset(&a, 0, sizeof a);
     a.layer_begin = layer_begin;
     a.layer_end = layer_end;
     a.n_units = static_cast<int>(ctx->plan_units.size());
@@ -314,6 +372,104 @@ int prepos_entry_attn(prepos_ctx *ctx, int layer_begin, int layer_end, int n_ses
     return prepos_launch_attn_generic(ctx, a, static_cast<cudaStream_t>(stream));
 }
 
+int prepos_entry_attn_fp8(prepos_ctx *ctx, int layer_begin, int layer_end, int n_sessions, const void *q,
+                          int64_t q_layer_stride, const void *k_new, const void *v_new, int64_t kv_new_layer_stride,
+                          void *k_pool8, void *v_pool8, int64_t pool_layer_stride, int64_t n_pages,
+                          const float *k_scale, const float *v_scale, int64_t scale_layer_stride,
+                          const int32_t *page_table, int page_table_stride, const int32_t *n_s,
+                          const int32_t *l_entry, const int32_t *capacity_tokens, void *out, int64_t out_layer_stride,
+                          int32_t *status_per_session, float softmax_scale, void *stream)
+{
+    if (!ctx) return PREPOS_E_INVALID_ARG;
+    const prepos_model_shape &s = ctx->shape;
+    if (layer_begin < 0 || layer_end > s.layers || layer_begin > layer_end || n_sessions < 0) return PREPOS_E_INVALID_ARG;
+    if (n_sessions > ctx->max_sessions) return PREPOS_E_WORKSPACE;
+    if (n_sessions == 0 || layer_begin == layer_end) return PREPOS_OK;
+    if (!q || !k_new || !v_new || !k_pool8 || !v_pool8 || !k_scale || !v_scale || !page_table || !n_s || !l_entry ||
+        !capacity_tokens || !out)
+        return PREPOS_E_INVALID_ARG;
+    if (!aligned16(q) || !aligned16(k_new) || !aligned16(v_new) || !aligned16(k_pool8) || !aligned16(v_pool8) ||
+        !aligned16(out) || !aligned16(page_table) || (reinterpret_cast<uintptr_t>(k_scale) & 3) ||
+        (reinterpret_cast<uintptr_t>(v_scale) & 3))
+        return PREPOS_E_ALIGN;
+    if ((q_layer_stride | kv_new_layer_stride | out_layer_stride) & 7) return PREPOS_E_ALIGN;
+    if (pool_layer_stride & 15) return PREPOS_E_ALIGN;
+    if (s.head_dim % 16 != 0) return PREPOS_E_SHAPE;
+    if (n_pages <= 0 || page_table_stride <= 0) return PREPOS_E_INVALID_ARG;
+
+    const int G = s.n_q_heads / s.n_kv_heads;
+    const int chunk_tok = (G > 16 ? 1 : 16 / G);
+    const int st = plan_attn(ctx, 3, chunk_tok, true, n_sessions, page_table_stride, n_s, l_entry, capacity_tokens,
+                             status_per_session, static_cast<cudaStream_t>(stream));
+    if (st != PREPOS_OK) return st;
+    if (ctx->plan_units.empty()) return PREPOS_OK;
+
+    AttnArgs a;
+    memset(&a, 0, sizeof a);
+    a.layer_begin = layer_begin;
+    a.layer_end = layer_end;
+    a.n_units = static_cast<int>(ctx->plan_units.size());
+    a.sum_rows = 0;
+    for (int i = 0; i < n_sessions; ++i) a.sum_rows += l_entry[i];
+    a.q = static_cast<const __nv_bfloat16 *>(q);
+    a.k_new = static_cast<const __nv_bfloat16 *>(k_new);
+    a.v_new = static_cast<const __nv_bfloat16 *>(v_new);
+    a.k_pool8 = static_cast<uint8_t *>(k_pool8);
+    a.v_pool8 = static_cast<uint8_t *>(v_pool8);
+    a.k_scale = k_scale;
+    a.v_scale = v_scale;
+    a.scale_layer_stride = scale_layer_stride;
+    a.out = static_cast<__nv_bfloat16 *>(out);
+    a.q_layer_stride = q_layer_stride;
+    a.kv_new_layer_stride = kv_new_layer_stride;
+    a.pool_layer_stride = pool_layer_stride;
+    a.out_layer_stride = out_layer_stride;
+    a.n_pages = n_pages;
+    a.page_table = page_table;
+    a.page_table_stride = page_table_stride;
+    a.scale = softmax_scale > 0.f ? softmax_scale : 1.0f / sqrtf(static_cast<float>(s.head_dim));
+    return prepos_launch_attn_fp8(ctx, a, static_cast<cudaStream_t>(stream));
+}
+
+int prepos_ctx_set_attn_slice(prepos_ctx *ctx, int max_segments_per_launch)
+{
+    if (!ctx || max_segments_per_launch < 0) return PREPOS_E_INVALID_ARG;
+    ctx->attn_slice = max_segments_per_launch;
+    return PREPOS_OK;
+}
+
+int prepos_ctx_request_yield(prepos_ctx *ctx, void *stream)
+{
+    if (!ctx) return PREPOS_E_INVALID_ARG;
+    ctx->yield_dirty = true;
+    PREPOS_CUDA_TRY(cudaMemcpyAsync(ctx->attn_yield_flag, ctx->yield_host, sizeof(unsigned int), cudaMemcpyHostToDevice,
+                                    static_cast<cudaStream_t>(stream)));
+    return PREPOS_OK;
+}
+
+int prepos_entry_attn_pending(prepos_ctx *ctx, void *stream, int32_t *pending_out)
+{
+    if (!ctx || !pending_out) return PREPOS_E_INVALID_ARG;
+    *pending_out = 0;
+    if (!ctx->pass_open) return PREPOS_OK;
+    PREPOS_CUDA_TRY(cudaMemcpyAsync(ctx->yield_host + 1, ctx->attn_pass_state, sizeof(unsigned int),
+                                    cudaMemcpyDeviceToHost, static_cast<cudaStream_t>(stream)));
+    PREPOS_CUDA_TRY(cudaStreamSynchronize(static_cast<cudaStream_t>(stream)));
+    *pending_out = (ctx->yield_host[1] == ctx->attn_launch_seq) ? 1 : 0;
+    return PREPOS_OK;
+}
+
+int prepos_entry_attn_resume(prepos_ctx *ctx, void *stream)
+{
+    if (!ctx) return PREPOS_E_INVALID_ARG;
+    if (!ctx->pass_open) return PREPOS_OK;   // nothing to resume (no tcgen05 pass is open on this ctx)
+    if (ctx->yield_dirty) {
+        PREPOS_CUDA_TRY(cudaMemsetAsync(ctx->attn_yield_flag, 0, sizeof(unsigned int), static_cast<cudaStream_t>(stream)));
+        ctx->yield_dirty = false;
+    }
+    return prepos_resume_attn_umma(ctx, static_cast<cudaStream_t>(stream));
+}
+
 int prepos_ready_dist(prepos_ctx *ctx, int n, const int32_t *session_ids, const void *hidden, const void *w_vocab,
                       const int64_t *position_p, const uint64_t *entry_hash, const int32_t *skip_mask,
                       prepos_record *records, const uint64_t *session_version, const uint64_t *expected_version,
@@ -327,6 +483,22 @@ int prepos_ready_dist(prepos_ctx *ctx, int n, const int32_t *session_ids, const 
                                     static_cast<const __nv_bfloat16 *>(w_vocab), position_p, entry_hash, skip_mask,
                                     records, session_version, expected_version, logits_out,
                                     static_cast<cudaStream_t>(stream));
+}
+
+int prepos_ready_dist_w4(prepos_ctx *ctx, int n, const int32_t *session_ids, const void *hidden, const void *w4,
+                         const void *w_scale, const int64_t *position_p, const uint64_t *entry_hash,
+                         const int32_t *skip_mask, prepos_record *records, const uint64_t *session_version,
+                         const uint64_t *expected_version, float *logits_out, void *stream)
+{
+    if (!ctx || n < 0) return PREPOS_E_INVALID_ARG;
+    if (n == 0) return PREPOS_OK;
+    if (!session_ids || !hidden || !w4 || !w_scale || !records || !session_version) return PREPOS_E_INVALID_ARG;
+    if (!aligned16(hidden) || !aligned16(w4) || !aligned16(records) || (reinterpret_cast<uintptr_t>(w_scale) & 1))
+        return PREPOS_E_ALIGN;
+    return prepos_launch_ready_dist_w4(ctx, n, session_ids, static_cast<const __nv_bfloat16 *>(hidden),
+                                       static_cast<const uint8_t *>(w4), static_cast<const __nv_bfloat16 *>(w_scale),
+                                       position_p, entry_hash, skip_mask, records, session_version, expected_version,
+                                       logits_out, static_cast<cudaStream_t>(stream));
 }
 
 int prepos_scan_logits(prepos_ctx *ctx, int n, const float *logits, prepos_record *out, void *stream)

@@ -28,6 +28,7 @@
 // owns M-tile w; with <=128 rows the streams take alternate KV tiles and are merged in the epilogue.
 #include <math_constants.h>
 #include <stdio.h>
+#include <string.h>
 
 #include <type_traits>
 
@@ -64,6 +65,13 @@ struct UmmaParams {
     float *partials;    // [2 * grid] slots of kAttnMaxRows * (D + 2) floats: O as float4 [D / 4][256 rows] (a warp's
                         // 32 rows of one float4 column are 512 contiguous bytes), lse2 [256], pad [256]
     unsigned int *counters;  // [n_lh][n_units] arrival counters of the cross-CTA pass (self-resetting)
+    // ---- yield / resume (the idle-window pass "yields to any request")
+    const unsigned int *yield_flag;  // device word: non-zero asks every CTA to stop at its next segment boundary
+    int *progress;                   // [grid] segments CTA c has completed in this pass (over all its launches)
+    unsigned int *pass_state;        // a CTA that stops early writes launch_seq here
+    unsigned int launch_seq;
+    int resume;                      // 1: CTA c skips its first progress[c] segments
+    int slice;                       // > 0: stop after this many segments per launch (bounded residency)
 };
 
 struct Seg {
@@ -263,6 +271,10 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
     float2 *ml_x = reinterpret_cast<float2 *>(bars + 20);  // [128] (m, l) of stream 1 / the row factors back
     uint32_t *tmem_slot = reinterpret_cast<uint32_t *>(ml_x + 128);
     int *merge_info = reinterpret_cast<int *>(tmem_slot + 1);  // [3]: c0 (or -1 = not last), c1, c0's slot
+    // segment admission (yield / resume): [0] segments admitted in this launch, [1] the first one refused (or
+    // INT_MAX), [2] segments completed in the pass when this launch ends.  Written by lane 0 of the K producer, the
+    // role that reaches a segment first; every other role asks before it starts a segment.
+    int *sched = merge_info + 3;
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
 
@@ -281,11 +293,25 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
         ptx::mbar_init(ptx::smem_u32(q_full), 1);
         ptx::mbar_init(ptx::smem_u32(q_empty), 1);
         ptx::fence_mbar_init();
+        sched[0] = 0;
+        sched[1] = 0x7fffffff;
+        sched[2] = 0;
     }
     if (warp == 2) {
         ptx::tmem_alloc<512>(ptx::smem_u32(tmem_slot));
         ptx::tmem_relinquish();
+    } else if (threadIdx.x == 0) {
+        ptx::prefetch_tmap(&tm_k);
+        ptx::prefetch_tmap(&tm_v);
+        ptx::prefetch_tmap(&tm_kn);
+        ptx::prefetch_tmap(&tm_vn);
+        ptx::prefetch_tmap(&tm_q);
     }
+    // rows of a Q M-tile that no TMA box covers are never written: clear the buffer once so they stay finite (part of
+    // the prologue that overlaps the previous kernel's tail)
+    for (int off = threadIdx.x * 16; off < p.q_tiles * kTileBytes; off += kThreads * 16)
+        *reinterpret_cast<uint4 *>(q_s + off) = make_uint4(0, 0, 0, 0);
+    ptx::fence_proxy_async_smem();
     ptx::tc_fence_before();
     __syncthreads();
     ptx::tc_fence_after();
@@ -297,6 +323,14 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
 
     const long long t0 = cta_begin(p, gridDim.x, blockIdx.x);
     const long long t1 = cta_begin(p, gridDim.x, blockIdx.x + 1);
+    const int skip = p.resume ? p.progress[blockIdx.x] : 0;   // segments this CTA completed before a yield
+    // may the role start the n-th segment of this launch?  (the K producer has admitted it, or refused it)
+    auto admitted = [&](int n) -> bool {
+        while (true) {
+            if (ptx::ld_acquire_cta_smem(&sched[0]) > n) return true;
+            if (ptx::ld_acquire_cta_smem(&sched[1]) <= n) return false;
+        }
+    };
     const int G = p.Hq / p.Hkv;
     const int pages_per_tile = kTile >> p.page_shift;
     const int page_bytes = p.page * D * 2;
@@ -314,17 +348,30 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
         uint64_t *full = is_v ? v_full : k_full, *empty = is_v ? v_empty : k_empty;
         uint8_t *ring = is_v ? v_s : k_s;
         const int n_slots = is_v ? p.nv : kNK;
-        if (lane == 0) {
-            ptx::prefetch_tmap(tm);
-            ptx::prefetch_tmap(tmn);
-        }
         const uint64_t pol = ptx::policy_evict_first();   // the cache is streamed once per pass
         const uint64_t pol_new = ptx::policy_evict_last();  // entry K/V: just produced, re-read by every row chunk
         int slot = 0;
         uint32_t ph = 0;
         SegIter it(p, t0, t1);
         Seg s;
+        int seg = 0, kproc = 0;
+        // the yield flag is read ahead of its use (at launch, then every 8 tiles): never a load on the critical path
+        unsigned int yflag = (!is_v && lane == 0) ? ptx::ld_volatile_global(p.yield_flag) : 0u;
         while (it.next(p, s)) {
+            if (seg++ < skip) continue;
+            if (!is_v) {
+                int stop = 0;
+                if (lane == 0) {
+                    stop = (yflag != 0u) || (p.slice > 0 && kproc >= p.slice);
+                    if (stop) ptx::st_release_cta_smem(&sched[1], kproc);
+                    else ptx::st_release_cta_smem(&sched[0], kproc + 1);
+                }
+                stop = __shfl_sync(0xffffffffu, stop, 0);
+                if (stop) break;
+            } else if (!admitted(kproc)) {
+                break;
+            }
+            ++kproc;
             const int n_pages_valid = (s.u.n_s + p.page - 1) >> p.page_shift;
             const int32_t *pt = p.a.page_table + static_cast<size_t>(s.u.session) * p.a.page_table_stride;
             // this lane's page of tile t (page-table reads run one tile ahead of the TMA issue)
@@ -334,6 +381,7 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
             };
             int pg_next = page_of(s.tb);
             for (int t = s.tb; t < s.te; ++t) {
+                if (!is_v && lane == 0 && ((t - s.tb) & 7) == 7) yflag = ptx::ld_volatile_global(p.yield_flag);
                 const int pg = pg_next;
                 if (t + 1 < s.te) pg_next = page_of(t + 1);
                 if (lane == 0) ptx::mbar_wait(ptx::smem_u32(&empty[slot]), ph ^ 1);
@@ -374,19 +422,16 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
                 }
             }
         }
+        if (!is_v && lane == 0) sched[2] = skip + kproc;   // read after the CTA-wide barrier at the end
     } else if (warp == 2) {
         // ===================== service warp: Q loader, Append(E), cross-CTA merge =====================
         SegIter it(p, t0, t1);
         Seg s;
-        // rows of an M-tile that no box covers are never written: clear the buffer once so they stay finite
-        for (int off = lane * 16; off < p.q_tiles * kTileBytes; off += 32 * 16)
-            *reinterpret_cast<uint4 *>(q_s + off) = make_uint4(0, 0, 0, 0);
-        ptx::fence_proxy_async_smem();
-        __syncwarp();
-        if (lane == 0) ptx::prefetch_tmap(&tm_q);
         const uint64_t pol_q = ptx::policy_evict_last();  // Q is re-read by every CTA that shares the unit
-        int k = 0;
+        int k = 0, seg = 0;
         while (it.next(p, s)) {
+            if (seg++ < skip) continue;
+            if (!admitted(k)) break;
             // ---- Q rows -> smem (swizzled K-major tiles) by TMA, as soon as the previous segment's last QK has read
             // the buffer.  Row r of the unit is entry token tok0 + r / G, query
             // head kvh * G + r % G; rows past the unit hold other tokens' Q or zeros and are never written out.
@@ -424,7 +469,11 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
         uint32_t pph = 0;  // bit w = phase parity of p_ready[w]
         SegIter it(p, t0, t1);
         Seg s;
+        int seg = 0, kproc = 0;
         while (it.next(p, s)) {
+            if (seg++ < skip) continue;
+            if (!admitted(kproc)) break;
+            ++kproc;
             const int rows = s.u.ntok * G;
             const int n_mt = rows > 128 ? 2 : 1;
             const int n_tiles = s.te - s.tb;
@@ -542,7 +591,11 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
         uint32_t sph = 0, oph = 0;
         SegIter it(p, t0, t1);
         Seg s;
+        int seg = 0, kproc = 0;
         while (it.next(p, s)) {
+            if (seg++ < skip) continue;
+            if (!admitted(kproc)) break;
+            ++kproc;
             const int rows = s.u.ntok * G;
             const int n_mt = rows > 128 ? 2 : 1;
             const int n_tiles = s.te - s.tb;
@@ -879,6 +932,10 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
     ptx::tc_fence_before();
     __syncthreads();
     if (warp == 2) ptx::tmem_dealloc<512>(tmem);
+    if (threadIdx.x == 0) {
+        p.progress[blockIdx.x] = sched[2];
+        if (sched[1] != 0x7fffffff) *p.pass_state = p.launch_seq;   // this launch left segments for a resume
+    }
 }
 
 // The cross-CTA pass of units spread over more than kLastArriverMax CTAs (a launch with few units and many CTAs: one
@@ -892,6 +949,8 @@ __global__ void __launch_bounds__(128) attn_merge_kernel(const UmmaParams p, int
 {
     ptx::griddep_launch();
     ptx::griddep_wait();
+    // the attention launch stopped at a yield point: its partials are incomplete, the resume's merge does the work
+    if (ptx::ld_volatile_global(p.pass_state) == p.launch_seq) return;
     constexpr int kVec = D / 4;
     constexpr int kRowBlks = kAttnMaxRows / 32, kColBlks = kVec / 4;
     constexpr int kCB = 8;
@@ -1040,6 +1099,9 @@ int encode_q_map(CUtensorMap *tm, const void *base, const prepos_model_shape &s,
 }
 
 template <int D>
+int issue(prepos_ctx *ctx, cudaStream_t stream, int resume);
+
+template <int D>
 int launch(prepos_ctx *ctx, const AttnArgs &a, int tiles_per_lh, cudaStream_t stream)
 {
     UmmaParams p;
@@ -1062,7 +1124,7 @@ int launch(prepos_ctx *ctx, const AttnArgs &a, int tiles_per_lh, cudaStream_t st
     p.nv = two ? 2 : 3;
     if (D == 64) p.nv = 3;
     constexpr int kTileBytes = kTile * D * 2;
-    const size_t smem = static_cast<size_t>(p.q_tiles + kNK + p.nv) * kTileBytes + 20 * 8 + 128 * 8 + 16;
+    const size_t smem = static_cast<size_t>(p.q_tiles + kNK + p.nv) * kTileBytes + 20 * 8 + 128 * 8 + 32;
     // one CTA per SM; never more CTAs than tiles, never more than the partial slots provisioned
     long long grid = ctx->num_sms;
     if (grid > p.total_tiles) grid = p.total_tiles;
@@ -1172,19 +1234,47 @@ int launch(prepos_ctx *ctx, const AttnArgs &a, int tiles_per_lh, cudaStream_t st
                 }
         }
     }
-    PREPOS_CUDA_TRY(cudaFuncSetAttribute(attn_umma_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                         static_cast<int>(smem)));
-    PREPOS_CUDA_TRY(prepos_launch_pdl(attn_umma_kernel<D>, dim3(static_cast<unsigned>(grid)), dim3(kThreads), smem, stream,
-                                      ctx->tm_k, ctx->tm_v, ctx->tm_kn, ctx->tm_vn, ctx->tm_q, p));
-    ctx->launches += 1;
+    long long mg = 0;
     if (merge_units > 0) {
-        long long mg = merge_units * (kAttnMaxRows / 32) * (D / 16);
+        mg = merge_units * (kAttnMaxRows / 32) * (D / 16);
         const long long cap = static_cast<long long>(ctx->num_sms) * 4;
         mg = mg > cap ? cap : mg;
-        PREPOS_CUDA_TRY(prepos_launch_pdl(attn_merge_kernel<D>, dim3(static_cast<unsigned>(mg)), dim3(128), 0, stream, p,
-                                          static_cast<int>(grid)));
+    }
+    p.yield_flag = ctx->attn_yield_flag;
+    p.progress = ctx->attn_progress;
+    p.pass_state = ctx->attn_pass_state;
+    p.slice = ctx->attn_slice;
+    p.resume = 0;
+    // keep the launch: prepos_entry_attn_resume re-issues it with resume = 1 (same plan, same grid, same partial slots)
+    static_assert(std::is_trivially_copyable<UmmaParams>::value, "UmmaParams is saved as bytes");
+    ctx->pass_params.resize(sizeof(UmmaParams));
+    memcpy(ctx->pass_params.data(), &p, sizeof(UmmaParams));
+    ctx->pass_grid = static_cast<int>(grid);
+    ctx->pass_merge_grid = static_cast<int>(mg);
+    ctx->pass_smem = smem;
+    ctx->pass_head_dim = D;
+    return issue<D>(ctx, stream, 0);
+}
+
+// one launch of the saved pass (fresh or resumed) + the merge launch behind it
+template <int D>
+int issue(prepos_ctx *ctx, cudaStream_t stream, int resume)
+{
+    UmmaParams p;
+    memcpy(&p, ctx->pass_params.data(), sizeof(UmmaParams));
+    p.resume = resume;
+    p.launch_seq = ++ctx->attn_launch_seq;
+    PREPOS_CUDA_TRY(cudaFuncSetAttribute(attn_umma_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                         static_cast<int>(ctx->pass_smem)));
+    PREPOS_CUDA_TRY(prepos_launch_pdl(attn_umma_kernel<D>, dim3(static_cast<unsigned>(ctx->pass_grid)), dim3(kThreads),
+                                      ctx->pass_smem, stream, ctx->tm_k, ctx->tm_v, ctx->tm_kn, ctx->tm_vn, ctx->tm_q, p));
+    ctx->launches += 1;
+    if (ctx->pass_merge_grid > 0) {
+        PREPOS_CUDA_TRY(prepos_launch_pdl(attn_merge_kernel<D>, dim3(static_cast<unsigned>(ctx->pass_merge_grid)), dim3(128),
+                                          0, stream, p, ctx->pass_grid));
         ctx->launches += 1;
     }
+    ctx->pass_open = true;
     return PREPOS_OK;
 }
 
@@ -1196,6 +1286,13 @@ bool prepos_attn_umma_supported(const prepos_ctx *ctx)
     const int G = s.n_q_heads / s.n_kv_heads;
     return (s.head_dim == 64 || s.head_dim == 128) && s.page_size >= 8 && s.page_size <= kTile &&
            (G & (G - 1)) == 0;  // the Q boxes take whole 8-row groups of (token, head) rows
+}
+
+int prepos_resume_attn_umma(prepos_ctx *ctx, cudaStream_t stream)
+{
+    if (ctx->pass_params.size() != sizeof(UmmaParams)) return PREPOS_E_INVALID_ARG;
+    if (ctx->pass_head_dim == 128) return issue<128>(ctx, stream, 1);
+    return issue<64>(ctx, stream, 1);
 }
 
 int prepos_launch_attn_umma(prepos_ctx *ctx, const AttnArgs &a, int tiles_per_lh, cudaStream_t stream)

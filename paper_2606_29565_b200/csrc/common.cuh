@@ -77,7 +77,9 @@ struct AttnUnit {
     int32_t n_cached_tiles;  // ceil(n_s / tile)
     int32_t n_tiles;      // cached tiles + new-token tiles visible to this chunk
     int32_t tile_prefix;  // sum of n_tiles of the units before this one (within one (layer, head))
-    int32_t pad[3];
+    int32_t n_load;       // tokens read from the session's pages: n_s, or n_s + tok0 + ntok when the entry tokens are
+                          // read back from the cache they were appended to (FP8 path)
+    int32_t pad[2];
 };
 static_assert(sizeof(AttnUnit) == 48, "AttnUnit");
 
@@ -99,6 +101,18 @@ struct prepos_ctx {
     float *attn_partials;      // [2 * kAttnMaxCtas] slots of kAttnMaxRows * (d + 2) floats
     unsigned int *attn_counters;  // [layers * Hkv * max_units] arrival counters (self-resetting)
     size_t attn_counters_n;
+    // yield / resume of the tcgen05 attention pass (prepos_ctx_request_yield, prepos_entry_attn_resume)
+    unsigned int *attn_yield_flag;   // device word polled by the persistent CTAs
+    unsigned int *attn_pass_state;   // device word: launch_seq of the last launch that stopped early
+    int *attn_progress;              // device [kAttnMaxCtas]: segments completed per CTA
+    unsigned int *yield_host;        // pinned: [0] = 1 (source of the flag copy), [1] = read-back of pass_state
+    unsigned int attn_launch_seq;
+    int attn_slice;                  // > 0: at most this many segments per CTA and launch
+    bool yield_dirty;                // a yield was requested since the flag / arrival counters were last cleared
+    bool pass_open;                  // the last attention call was a tcgen05 launch that can be resumed
+    std::vector<unsigned char> pass_params;   // its kernel parameters
+    int pass_grid, pass_merge_grid, pass_head_dim;
+    size_t pass_smem;
     // host-side plan cache
     std::vector<AttnUnit> plan_units;
     std::vector<int32_t> plan_key;
@@ -124,6 +138,11 @@ int prepos_launch_ready_dist(prepos_ctx *ctx, int n, const int32_t *session_ids,
                              const __nv_bfloat16 *w, const int64_t *position_p, const uint64_t *entry_hash,
                              const int32_t *skip_mask, prepos_record *records, const uint64_t *session_version,
                              const uint64_t *expected_version, float *logits_out, cudaStream_t stream);
+int prepos_launch_ready_dist_w4(prepos_ctx *ctx, int n, const int32_t *session_ids, const __nv_bfloat16 *hidden,
+                                const uint8_t *w4, const __nv_bfloat16 *w_scale, const int64_t *position_p,
+                                const uint64_t *entry_hash, const int32_t *skip_mask, prepos_record *records,
+                                const uint64_t *session_version, const uint64_t *expected_version, float *logits_out,
+                                cudaStream_t stream);
 int prepos_launch_scan_logits(prepos_ctx *ctx, int n, const float *logits, prepos_record *out, cudaStream_t stream);
 int prepos_launch_gate_serve(prepos_ctx *ctx, int n, const int32_t *session_ids, const uint64_t *req_hash,
                              const prepos_record *records, const uint64_t *session_version,
@@ -144,7 +163,14 @@ struct AttnArgs {
     const int32_t *page_table;
     int page_table_stride;
     float scale;
+    // FP8 (e4m3) KV cache, reading Q20: code pools [layer][n_pages][Hkv][page][d] uint8 (layer stride in
+    // bytes = pool_layer_stride) and one fp32 scale per (layer, page, kv head) for K and for V
+    uint8_t *k_pool8, *v_pool8;
+    const float *k_scale, *v_scale;
+    int64_t scale_layer_stride;
 };
+int prepos_launch_attn_fp8(prepos_ctx *ctx, const AttnArgs &a, cudaStream_t stream);
 int prepos_launch_attn_generic(prepos_ctx *ctx, const AttnArgs &a, cudaStream_t stream);
 int prepos_launch_attn_umma(prepos_ctx *ctx, const AttnArgs &a, int total_tiles_per_lh, cudaStream_t stream);
+int prepos_resume_attn_umma(prepos_ctx *ctx, cudaStream_t stream);
 bool prepos_attn_umma_supported(const prepos_ctx *ctx);

@@ -87,6 +87,24 @@ __device__ __forceinline__ unsigned int ld_acquire_gpu(const unsigned int *p)
     return v;
 }
 
+__device__ __forceinline__ unsigned int ld_volatile_global(const unsigned int *p)
+{
+    unsigned int v;
+    asm volatile("ld.volatile.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+// release / acquire on a shared-memory word among the warps of one CTA
+__device__ __forceinline__ int ld_acquire_cta_smem(const int *p)
+{
+    int v;
+    asm volatile("ld.acquire.cta.shared::cta.b32 %0, [%1];" : "=r"(v) : "r"(smem_u32(p)) : "memory");
+    return v;
+}
+__device__ __forceinline__ void st_release_cta_smem(int *p, int v)
+{
+    asm volatile("st.release.cta.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(p)), "r"(v) : "memory");
+}
+
 // generic-proxy smem writes -> visible to the async proxy (TMA / UMMA)
 __device__ __forceinline__ void fence_proxy_async_smem()
 {

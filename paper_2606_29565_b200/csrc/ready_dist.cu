@@ -383,6 +383,212 @@ ready_dist_kernel(const __grid_constant__ CUtensorMap tm_w, const RdParams p)
     finalize_records(p, warp, lane, kThreads / 32);
 }
 
+// ---- a3 + a4 over a 4-bit W_vocab (reading Q21) -----------
+// w4 [V][H/2]: two's-complement int4 codes, two per byte (even k in the low nibble); w_scale [V][H/128] bf16, one
+// per (vocabulary row, group of 128 consecutive k); W[v][k] = code * scale.  A quarter of the bytes of the bf16 pass
+// (V*H/2 + V*H/64), so a quarter of its HBM time -- and four times the arithmetic per byte: the codes are widened
+// to bf16 in registers (exact: |code| <= 8) and multiplied with the hidden rows by the same warp-level MMA, the
+// fp32 sum of each 128-k group is scaled once (the scale never rounds a weight), and the record is reduced exactly
+// as in ready_dist_kernel.
+//   * one TMA box = one scale group of one vocabulary tile: [128 rows][64 B]; a stage = up to four boxes (512 k)
+//   * thread (g, t) of a warp owns rows g, g+8 of the warp's 16 and the 16 bytes [16t, 16t+16) of each: word j of
+//     them holds k = 32t + 8j + (0..7).  `(w >> 4i) & 0x000f000f` puts nibbles i and i+4 into the two halves of a
+//     register, which is the A fragment (row g; MMA columns 2t, 2t+1) of one m16n8k16 -- so MMA column p stands for
+//     k = 32t + 8j + {0,4 | 1,5} (first MMA of word j) or {2,6 | 3,7} (second).  The hidden rows are laid out in
+//     shared memory in exactly that order when they are loaded, so one 16-byte read yields the B fragments of both.
+constexpr int kW4BoxBytes = kTileRows * 64;               // 8 KB: 128 rows x 128 codes
+constexpr int kW4BoxesPerStage = 4;
+constexpr int kW4StageBytes = kW4BoxesPerStage * kW4BoxBytes;  // 32 KB
+constexpr int kW4Group = 128;
+constexpr int kW4XPad = 32;  // bf16 elements: the row stride of the hidden block is 64 B mod 128 B (bank spread)
+
+// eight int4 codes (one 32-bit word) -> four bf16x2 registers holding codes (i, i + 4), exactly
+__device__ __forceinline__ void w4_widen(uint32_t w, uint32_t (&r)[4])
+{
+    const uint32_t x = w ^ 0x88888888u;           // code + 8 in 0..15
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        const uint32_t b = ((x >> (4 * i)) & 0x000f000fu) | 0x43004300u;   // bf16(128 + code + 8) in both halves
+        asm("sub.rn.bf16x2 %0, %1, %2;" : "=r"(r[i]) : "r"(b), "r"(0x43084308u));  // - 136: exact
+    }
+}
+
+__global__ void __launch_bounds__(kThreads, 1)
+ready_dist_w4_kernel(const __grid_constant__ CUtensorMap tm_w4, const RdParams p, const __nv_bfloat16 *__restrict__ w_scale)
+{
+    extern __shared__ __align__(1024) uint8_t smem_raw[];
+    uint8_t *smem = reinterpret_cast<uint8_t *>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
+    uint8_t *stage_base = smem;
+    const int x_stride = p.H + kW4XPad;  // elements
+    __nv_bfloat16 *xs = reinterpret_cast<__nv_bfloat16 *>(smem + static_cast<size_t>(p.n_stages) * kW4StageBytes);
+    uint64_t *bars = reinterpret_cast<uint64_t *>(reinterpret_cast<uint8_t *>(xs) +
+                                                  ((static_cast<size_t>(p.x_rows) * x_stride * 2 + 15) & ~size_t(15)));
+    uint64_t *full_bar = bars;
+    uint64_t *empty_bar = bars + kMaxStages;
+    RdPartial *warp_part = reinterpret_cast<RdPartial *>(bars + 2 * kMaxStages);  // [kConsumerWarps][kNB]
+    const int warp = threadIdx.x >> 5;
+    const int lane = threadIdx.x & 31;
+    const int n_tiles = (p.V + kTileRows - 1) / kTileRows;
+    const int n_groups = p.H / kW4Group;
+    const int n_kc = (n_groups + kW4BoxesPerStage - 1) / kW4BoxesPerStage;
+
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < p.n_stages; ++s) {
+            ptx::mbar_init(ptx::smem_u32(&full_bar[s]), 1);
+            ptx::mbar_init(ptx::smem_u32(&empty_bar[s]), kConsumerWarps);
+        }
+        ptx::fence_mbar_init();
+    }
+    __syncthreads();
+    ptx::griddep_launch();
+
+    if (warp == kConsumerWarps) {
+        // ===== TMA producer (the weights are never written by a libprepos kernel: fetched before the wait) =====
+        if (lane == 0) {
+            ptx::prefetch_tmap(&tm_w4);
+            const uint64_t pol = ptx::policy_evict_first();
+            int stage = 0;
+            uint32_t phase = 0;
+            for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+                for (int kc = 0; kc < n_kc; ++kc) {
+                    const int nb = (n_groups - kc * kW4BoxesPerStage < kW4BoxesPerStage) ? n_groups - kc * kW4BoxesPerStage
+                                                                                         : kW4BoxesPerStage;
+                    ptx::mbar_wait(ptx::smem_u32(&empty_bar[stage]), phase ^ 1);
+                    const uint32_t fb = ptx::smem_u32(&full_bar[stage]);
+                    ptx::mbar_arrive_expect_tx(fb, nb * kW4BoxBytes);
+                    const uint32_t dst = ptx::smem_u32(stage_base + static_cast<size_t>(stage) * kW4StageBytes);
+                    for (int b = 0; b < nb; ++b)
+                        ptx::tma_load_2d(dst + b * kW4BoxBytes, &tm_w4, fb, (kc * kW4BoxesPerStage + b) * 64,
+                                         tile * kTileRows, pol);
+                    if (++stage == p.n_stages) {
+                        stage = 0;
+                        phase ^= 1;
+                    }
+                }
+            }
+        }
+        ptx::griddep_wait();
+    } else {
+        // ===== consumers: 16 vocabulary rows per warp =====
+        ptx::griddep_wait();
+        {
+            // hidden rows -> smem in MMA order: the 8 elements k0..k0+7 of a word are stored (0,4,1,5,2,6,3,7), and the
+            // words of a group as [j][t] (thread t's word j), so that a quarter-warp reads 64 contiguous bytes per row
+            const int chunks_per_row = p.H / 8;
+            for (int idx = threadIdx.x; idx < p.x_rows * chunks_per_row; idx += kConsumerWarps * 32) {
+                const int r = idx / chunks_per_row, c = idx - r * chunks_per_row;
+                uint4 v = make_uint4(0, 0, 0, 0);
+                if (r < p.n) v = *reinterpret_cast<const uint4 *>(p.hidden + static_cast<size_t>(r) * p.H + c * 8);
+                uint4 o;
+                o.x = __byte_perm(v.x, v.z, 0x5410);  // (x0, x4)
+                o.y = __byte_perm(v.x, v.z, 0x7632);  // (x1, x5)
+                o.z = __byte_perm(v.y, v.w, 0x5410);  // (x2, x6)
+                o.w = __byte_perm(v.y, v.w, 0x7632);  // (x3, x7)
+                const int grp = c >> 4, within = c & 15, t = within >> 2, j = within & 3;
+                *reinterpret_cast<uint4 *>(xs + static_cast<size_t>(r) * x_stride + grp * kW4Group + j * 32 + t * 8) = o;
+            }
+        }
+        ptx::bar_sync(1, kConsumerWarps * 32);
+        Top2Lse st[2];
+        st[0] = t2_init();
+        st[1] = t2_init();
+        const int g = lane >> 2, t = lane & 3;
+        const int n0 = 2 * t;  // this lane's two hidden rows (accumulator columns)
+        const int b_row = min(g, p.x_rows - 1);   // B fragment: hidden row g (absent rows read the zero row)
+        const __nv_bfloat16 *xs_lane = xs + static_cast<size_t>(b_row) * x_stride + t * 8;
+        const int w_off = (warp * 16 + g) * 64 + t * 16;   // this lane's 16 bytes of row g within a box
+
+        int stage = 0;
+        uint32_t phase = 0;
+        for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+            float tot[4] = {0.f, 0.f, 0.f, 0.f};
+            const int v = tile * kTileRows + warp * 16 + g;
+            const __nv_bfloat16 *sc_a = w_scale + static_cast<size_t>(v) * n_groups;
+            const __nv_bfloat16 *sc_b = w_scale + static_cast<size_t>(v + 8) * n_groups;
+            for (int kc = 0; kc < n_kc; ++kc) {
+                const int g0 = kc * kW4BoxesPerStage;
+                const int nb = (n_groups - g0 < kW4BoxesPerStage) ? n_groups - g0 : kW4BoxesPerStage;
+                // the stage's group scales of this lane's two rows: issued before the wait for the codes
+                float sa[kW4BoxesPerStage], sb[kW4BoxesPerStage];
+#pragma unroll
+                for (int b = 0; b < kW4BoxesPerStage; ++b) {
+                    sa[b] = (b < nb && v < p.V) ? __bfloat162float(sc_a[g0 + b]) : 0.f;
+                    sb[b] = (b < nb && v + 8 < p.V) ? __bfloat162float(sc_b[g0 + b]) : 0.f;
+                }
+                ptx::mbar_wait(ptx::smem_u32(&full_bar[stage]), phase);
+                const uint8_t *sbase = stage_base + static_cast<size_t>(stage) * kW4StageBytes;
+#pragma unroll
+                for (int b = 0; b < kW4BoxesPerStage; ++b) {
+                    if (b < nb) {
+                        const uint4 wa = *reinterpret_cast<const uint4 *>(sbase + b * kW4BoxBytes + w_off);
+                        const uint4 wb = *reinterpret_cast<const uint4 *>(sbase + b * kW4BoxBytes + w_off + 8 * 64);
+                        const uint32_t wav[4] = {wa.x, wa.y, wa.z, wa.w}, wbv[4] = {wb.x, wb.y, wb.z, wb.w};
+                        const __nv_bfloat16 *xk = xs_lane + (g0 + b) * kW4Group;
+                        float acc[4] = {0.f, 0.f, 0.f, 0.f};
+#pragma unroll
+                        for (int j = 0; j < 4; ++j) {
+                            const uint4 xb = *reinterpret_cast<const uint4 *>(xk + j * 32);
+                            uint32_t ra[4], rb[4];
+                            w4_widen(wav[j], ra);
+                            w4_widen(wbv[j], rb);
+                            ptx::mma_bf16_16816(acc, ra[0], rb[0], ra[1], rb[1], xb.x, xb.y);
+                            ptx::mma_bf16_16816(acc, ra[2], rb[2], ra[3], rb[3], xb.z, xb.w);
+                        }
+                        tot[0] = fmaf(sa[b], acc[0], tot[0]);
+                        tot[1] = fmaf(sa[b], acc[1], tot[1]);
+                        tot[2] = fmaf(sb[b], acc[2], tot[2]);
+                        tot[3] = fmaf(sb[b], acc[3], tot[3]);
+                    }
+                }
+                __syncwarp();
+                if (lane == 0) ptx::mbar_arrive(ptx::smem_u32(&empty_bar[stage]));
+                if (++stage == p.n_stages) {
+                    stage = 0;
+                    phase ^= 1;
+                }
+            }
+#pragma unroll
+            for (int j = 0; j < 2; ++j) {
+                if (n0 + j < p.n) {
+                    if (v < p.V) t2_push(st[j], tot[j], v);
+                    if (v + 8 < p.V) t2_push(st[j], tot[2 + j], v + 8);
+                    if (p.logits_out) {
+                        float *lo = p.logits_out + static_cast<size_t>(n0 + j) * p.V;
+                        if (v < p.V) lo[v] = tot[j];
+                        if (v + 8 < p.V) lo[v + 8] = tot[2 + j];
+                    }
+                }
+            }
+        }
+#pragma unroll
+        for (int j = 0; j < 2; ++j) {
+#pragma unroll
+            for (int mask = 4; mask < 32; mask <<= 1) {
+                const Top2Lse o = t2_shfl_xor(st[j], mask);
+                t2_merge(st[j], o);
+            }
+        }
+        if (lane < 4) {
+            t2_store(&warp_part[warp * kNB + n0], st[0]);
+            t2_store(&warp_part[warp * kNB + n0 + 1], st[1]);
+        }
+    }
+    __syncthreads();
+    if (threadIdx.x < p.n) {
+        Top2Lse acc = t2_init();
+        for (int w = 0; w < kConsumerWarps; ++w) {
+            const RdPartial *q = &warp_part[w * kNB + threadIdx.x];
+            Top2Lse t;
+            t.m = q->m, t.s = q->s, t.v1 = q->v1, t.v2 = q->v2, t.i1 = q->i1, t.i2 = q->i2, t.nonfinite = q->nonfinite;
+            t2_merge(acc, t);
+        }
+        t2_store(p.partials + static_cast<size_t>(threadIdx.x) * kMaxRdPartials + blockIdx.x, acc);
+        __threadfence();
+    }
+    __syncthreads();
+    finalize_records(p, warp, lane, kThreads / 32);
+}
+
 // ---- a3 + a4 for a batch of sessions (9..128 hidden rows per launch): one pass over W for all of them ----------
 // With more than a handful of hidden rows the LM head is a real contraction [n x H] . [H x V]: tcgen05.mma with the
 // hidden rows as the M operand (rows past n are zero-filled by TMA or never read back), a 128-row vocabulary tile
@@ -714,6 +920,59 @@ int prepos_launch_ready_dist(prepos_ctx *ctx, int n, const int32_t *session_ids,
         PREPOS_CUDA_TRY(cudaFuncSetAttribute(ready_dist_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                              static_cast<int>(smem)));
         PREPOS_CUDA_TRY(prepos_launch_pdl(ready_dist_kernel, dim3(grid), dim3(kThreads), smem, stream, tm, p));
+        ctx->launches += 1;
+    }
+    return PREPOS_OK;
+}
+
+int prepos_launch_ready_dist_w4(prepos_ctx *ctx, int n, const int32_t *session_ids, const __nv_bfloat16 *hidden,
+                                const uint8_t *w4, const __nv_bfloat16 *w_scale, const int64_t *position_p,
+                                const uint64_t *entry_hash, const int32_t *skip_mask, prepos_record *records,
+                                const uint64_t *session_version, const uint64_t *expected_version, float *logits_out,
+                                cudaStream_t stream)
+{
+    const int H = ctx->shape.hidden, V = ctx->shape.vocab;
+    EncodeTiledFn encode = reinterpret_cast<EncodeTiledFn>(prepos_get_encode_tiled());
+    if (!encode) return PREPOS_E_CUDA;
+    CUtensorMap tm;
+    const cuuint64_t dims[2] = {static_cast<cuuint64_t>(H / 2), static_cast<cuuint64_t>(V)};
+    const cuuint64_t strides[1] = {static_cast<cuuint64_t>(H / 2)};
+    const cuuint32_t box[2] = {64, kTileRows};
+    const cuuint32_t estr[2] = {1, 1};
+    if (encode(&tm, CU_TENSOR_MAP_DATA_TYPE_UINT8, 2, const_cast<uint8_t *>(w4), dims, strides, box, estr,
+               CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+               CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+        return PREPOS_E_CUDA;
+    const int n_tiles = (V + kTileRows - 1) / kTileRows;
+    const int grid = n_tiles < ctx->num_sms ? n_tiles : ctx->num_sms;
+    // up to 8 hidden rows per pass over the codes (a batch of more rows takes ceil(n / 8) passes)
+    for (int r0 = 0; r0 < n; r0 += kNB) {
+        RdParams p;
+        p.n = (n - r0 < kNB) ? n - r0 : kNB;
+        p.H = H;
+        p.V = V;
+        p.x_rows = (p.n < kNB) ? p.n + 1 : kNB;
+        const size_t x_bytes = (static_cast<size_t>(p.x_rows) * (H + kW4XPad) * 2 + 15) & ~size_t(15);
+        const size_t fixed = 1024 + x_bytes + 2 * kMaxStages * 8 + kConsumerWarps * kNB * sizeof(RdPartial);
+        int stages = static_cast<int>((232448 - fixed) / kW4StageBytes);
+        if (stages > kMaxStages) stages = kMaxStages;
+        if (stages < 2) return PREPOS_E_SHAPE;
+        p.n_stages = stages;
+        p.hidden = hidden + static_cast<size_t>(r0) * H;
+        p.session_ids = session_ids + r0;
+        p.position_p = position_p ? position_p + r0 : nullptr;
+        p.entry_hash = entry_hash ? entry_hash + r0 : nullptr;
+        p.skip_mask = skip_mask ? skip_mask + r0 : nullptr;
+        p.records = records;
+        p.session_version = session_version;
+        p.expected_version = expected_version ? expected_version + r0 : nullptr;
+        p.logits_out = logits_out ? logits_out + static_cast<size_t>(r0) * V : nullptr;
+        p.partials = ctx->rd_partials;
+        p.counter = ctx->rd_counter;
+        const size_t smem = fixed + static_cast<size_t>(stages) * kW4StageBytes;
+        PREPOS_CUDA_TRY(cudaFuncSetAttribute(ready_dist_w4_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                             static_cast<int>(smem)));
+        PREPOS_CUDA_TRY(prepos_launch_pdl(ready_dist_w4_kernel, dim3(grid), dim3(kThreads), smem, stream, tm, p, w_scale));
         ctx->launches += 1;
     }
     return PREPOS_OK;

@@ -23,8 +23,9 @@ RECORD_BYTES = 48
 
 EXPORTS = [
     "prepos_strerror", "prepos_version", "prepos_workspace_bytes", "prepos_ctx_create", "prepos_ctx_destroy",
-    "prepos_ctx_sync", "prepos_ctx_launch_count", "prepos_ctx_set_attn_path", "prepos_entry_attn",
-    "prepos_ready_dist", "prepos_scan_logits", "prepos_gate_serve", "prepos_invalidate", "prepos_gate_sweep",
+    "prepos_ctx_sync", "prepos_ctx_launch_count", "prepos_ctx_set_attn_path", "prepos_entry_attn", "prepos_entry_attn_fp8",
+    "prepos_ctx_request_yield", "prepos_entry_attn_resume", "prepos_entry_attn_pending", "prepos_ctx_set_attn_slice",
+    "prepos_ready_dist", "prepos_ready_dist_w4", "prepos_scan_logits", "prepos_gate_serve", "prepos_invalidate", "prepos_gate_sweep",
     "prepos_fastset_build",
 ]
 
@@ -70,8 +71,21 @@ def lib() -> C.CDLL:
         L.prepos_entry_attn.restype = i32
         L.prepos_entry_attn.argtypes = [vp, i32, i32, i32, vp, i64, vp, vp, i64, vp, vp, i64, i64, vp, i32, vp, vp, vp,
                                         vp, i64, vp, f32, vp]
+        L.prepos_entry_attn_fp8.restype = i32
+        L.prepos_entry_attn_fp8.argtypes = [vp, i32, i32, i32, vp, i64, vp, vp, i64, vp, vp, i64, i64, vp, vp, i64, vp, i32,
+                                            vp, vp, vp, vp, i64, vp, f32, vp]
+        L.prepos_ctx_request_yield.restype = i32
+        L.prepos_ctx_request_yield.argtypes = [vp, vp]
+        L.prepos_entry_attn_resume.restype = i32
+        L.prepos_entry_attn_resume.argtypes = [vp, vp]
+        L.prepos_entry_attn_pending.restype = i32
+        L.prepos_entry_attn_pending.argtypes = [vp, vp, C.POINTER(C.c_int32)]
+        L.prepos_ctx_set_attn_slice.restype = i32
+        L.prepos_ctx_set_attn_slice.argtypes = [vp, i32]
         L.prepos_ready_dist.restype = i32
         L.prepos_ready_dist.argtypes = [vp, i32, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp]
+        L.prepos_ready_dist_w4.restype = i32
+        L.prepos_ready_dist_w4.argtypes = [vp, i32, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp]
         L.prepos_scan_logits.restype = i32
         L.prepos_scan_logits.argtypes = [vp, i32, vp, vp, vp]
         L.prepos_gate_serve.restype = i32
@@ -217,6 +231,44 @@ class Context:
         _check(st, "prepos_entry_attn")
         return status.tolist()
 
+    def entry_attn_fp8(self, q, k_new, v_new, k_pool8, v_pool8, k_scale, v_scale, page_table, n_s, l_entry,
+                       capacity_tokens, out, layer_begin=0, layer_end=None, softmax_scale=0.0):
+        """prepos_entry_attn_fp8.  Pools [layers, n_pages, Hkv, page, d] uint8 (e4m3 codes), scales
+        [layers, n_pages, Hkv] float32; everything else as entry_attn."""
+        n_s, l_entry, cap = _host_i32(n_s), _host_i32(l_entry), _host_i32(capacity_tokens)
+        n = n_s.numel()
+        layer_end = self.shape.layers if layer_end is None else layer_end
+        status = torch.zeros(n, dtype=torch.int32)
+        for t in (q, k_new, v_new, out):
+            assert t.dtype == torch.bfloat16 and t.is_cuda
+        assert k_pool8.dtype == torch.uint8 and v_pool8.dtype == torch.uint8 and k_pool8.is_cuda and v_pool8.is_cuda
+        assert k_scale.dtype == torch.float32 and v_scale.dtype == torch.float32 and k_scale.stride(0) == v_scale.stride(0)
+        assert page_table.dtype == torch.int32 and page_table.is_cuda and page_table.stride(1) == 1
+        st = lib().prepos_entry_attn_fp8(
+            self._h, layer_begin, layer_end, n,
+            _p(q), q.stride(0), _p(k_new), _p(v_new), k_new.stride(0),
+            _p(k_pool8), _p(v_pool8), k_pool8.stride(0), k_pool8.shape[1],
+            _p(k_scale), _p(v_scale), k_scale.stride(0),
+            _p(page_table), page_table.stride(0), _p(n_s), _p(l_entry), _p(cap),
+            _p(out), out.stride(0), _p(status), float(softmax_scale), _stream())
+        _check(st, "prepos_entry_attn_fp8")
+        return status.tolist()
+
+    def request_yield(self):
+        """prepos_ctx_request_yield on the current stream (use the request's high-priority stream)."""
+        _check(lib().prepos_ctx_request_yield(self._h, _stream()), "prepos_ctx_request_yield")
+
+    def entry_attn_resume(self):
+        _check(lib().prepos_entry_attn_resume(self._h, _stream()), "prepos_entry_attn_resume")
+
+    def entry_attn_pending(self) -> bool:
+        out = C.c_int32(0)
+        _check(lib().prepos_entry_attn_pending(self._h, _stream(), C.byref(out)), "prepos_entry_attn_pending")
+        return bool(out.value)
+
+    def set_attn_slice(self, max_segments_per_launch: int):
+        _check(lib().prepos_ctx_set_attn_slice(self._h, int(max_segments_per_launch)), "prepos_ctx_set_attn_slice")
+
     def ready_dist(self, session_ids, hidden, w_vocab, records, session_version, position_p=None, entry_hash=None,
                    skip_mask=None, logits_out=None, expected_version=None):
         """prepos_ready_dist.  All tensors on the device."""
@@ -226,6 +278,17 @@ class Context:
         _check(lib().prepos_ready_dist(self._h, n, _p(session_ids), _p(hidden), _p(w_vocab), _p(position_p),
                                        _p(entry_hash), _p(skip_mask), _p(records), _p(session_version),
                                        _p(expected_version), _p(logits_out), _stream()), "prepos_ready_dist")
+
+    def ready_dist_w4(self, session_ids, hidden, w4, w_scale, records, session_version, position_p=None,
+                      entry_hash=None, skip_mask=None, logits_out=None, expected_version=None):
+        """prepos_ready_dist_w4: w4 [V, H/2] uint8 (int4 codes), w_scale [V, H/128] bf16.  All tensors on the device."""
+        assert hidden.dtype == torch.bfloat16 and w4.dtype == torch.uint8 and w_scale.dtype == torch.bfloat16
+        assert w4.is_contiguous() and w_scale.is_contiguous()
+        assert session_ids.dtype == torch.int32 and session_version.dtype == torch.int64
+        n = session_ids.numel()
+        _check(lib().prepos_ready_dist_w4(self._h, n, _p(session_ids), _p(hidden), _p(w4), _p(w_scale), _p(position_p),
+                                          _p(entry_hash), _p(skip_mask), _p(records), _p(session_version),
+                                          _p(expected_version), _p(logits_out), _stream()), "prepos_ready_dist_w4")
 
     def scan_logits(self, logits, records_out):
         assert logits.dtype == torch.float32 and logits.is_contiguous()

@@ -132,9 +132,80 @@ def make_sessions(shape: Shape, n_s, l_entry, seed: int, device="cpu", layers: O
     return SessionBatch(shape, n_s, l_entry, capacity, table.to(device), k_pool, v_pool, q, k_new, v_new, row_offset)
 
 
+@dataclass
+class SessionBatchFP8:
+    """The FP8 (e4m3) form of a SessionBatch (DESIGN.md reading Q20): code pools and per-(layer, page, kv head) scales;
+    q / k_new / v_new / page_table / n_s / l_entry / capacity / row_offset are those of `base`."""
+    base: SessionBatch
+    k_pool8: torch.Tensor   # [layers, n_pages, Hkv, page, d] uint8 (e4m3 codes)
+    v_pool8: torch.Tensor
+    k_scale: torch.Tensor   # [layers, n_pages, Hkv] float32
+    v_scale: torch.Tensor
+
+
+def make_sessions_fp8(shape: Shape, n_s, l_entry, seed: int, device="cpu", layers: Optional[int] = None,
+                      extra_pages: int = 0, tight_capacity=None, chunk_pages: int = 4096) -> SessionBatchFP8:
+    """The sessions of `make_sessions` (same seed, same draws) with the KV cache as an FP8 quantiser would leave it:
+    per (layer, page, kv head) scale = fp32(max|x| over the page slab) / 448 (pages that hold nothing yet get the
+    scale of an N(0,1) slab, 4 / 448), code = e4m3(x / scale) through the library's e4m3 (round to nearest even).
+    Input preparation only: both the oracle and the kernels start from these codes and scales; the codes of the entry
+    tokens are each side's own work (Append(E))."""
+    sb = make_sessions(shape, n_s, l_entry, seed, device, layers=layers, extra_pages=extra_pages,
+                       tight_capacity=tight_capacity)
+    page = shape.page
+    n_pages = sb.k_pool.shape[1]
+    # cached tokens per physical page (slots beyond n_s hold nothing yet)
+    filled = torch.zeros(n_pages, dtype=torch.int64)
+    pt = sb.page_table.cpu().long()
+    for s_, n in enumerate(sb.n_s):
+        full, rem = n // page, n % page
+        filled[pt[s_, :full]] = page
+        if rem:
+            filled[pt[s_, full]] = rem
+    slot_ok = (torch.arange(page).view(1, page) < filled.view(n_pages, 1)).to(device)   # [n_pages, page]
+
+    def quant(pool):
+        codes = torch.empty(pool.shape, dtype=torch.uint8, device=pool.device)
+        scales = torch.empty(pool.shape[:3], dtype=torch.float32, device=pool.device)
+        for lo in range(0, n_pages, chunk_pages):
+            x = pool[:, lo:lo + chunk_pages].to(torch.float32)
+            ok = slot_ok[lo:lo + chunk_pages].view(1, -1, 1, page, 1)
+            amax = (x.abs() * ok).amax(dim=(3, 4))
+            sc = torch.where(amax > 0, amax / 448.0, torch.full_like(amax, 4.0 / 448.0))
+            y = (x / sc.view(*sc.shape, 1, 1)).clamp_(-448.0, 448.0)
+            codes[:, lo:lo + chunk_pages] = y.to(torch.float8_e4m3fn).view(torch.uint8)
+            scales[:, lo:lo + chunk_pages] = sc
+        return codes, scales
+
+    k8, ks = quant(sb.k_pool)
+    v8, vs = quant(sb.v_pool)
+    return SessionBatchFP8(sb, k8, v8, ks, vs)
+
+
 def make_w_vocab(shape: Shape, seed: int, device="cpu") -> torch.Tensor:
     """W_vocab ~ N(0, 1/H) i.e. std = 1/sqrt(H) (reading Q13), bf16 [V, H]."""
     return randn_bf16((shape.V, shape.H), gen(seed + 101, device), std=1.0 / math.sqrt(shape.H))
+
+
+def make_w_vocab_w4(shape: Shape, seed: int, device="cpu", group: int = 128, rows: int = 8192):
+    """The 4-bit W_vocab of DESIGN.md reading Q21, as an offline weight quantiser would leave it: the N(0, 1/H)
+    weights of `make_w_vocab` (same seed, so the same matrix) rounded to int4 codes in -8..7 with one bf16 scale
+    per (row, group of `group` consecutive k), scale = bf16(max|w| / 7) of the group.  Returns
+    (w4 [V, H/2] uint8, two codes per byte with even k in the low nibble; w_scale [V, H/group] bf16).
+    Input preparation only: both the oracle and the kernels start from these codes and scales."""
+    w = make_w_vocab(shape, seed, device)
+    V, H = shape.V, shape.H
+    w4 = torch.empty((V, H // 2), dtype=torch.uint8, device=device)
+    sc = torch.empty((V, H // group), dtype=torch.bfloat16, device=device)
+    for lo in range(0, V, rows):
+        wf = w[lo:lo + rows].to(torch.float32).view(-1, H // group, group)
+        s = (wf.abs().amax(dim=2) / 7.0).to(torch.bfloat16)
+        s = torch.where(s.to(torch.float32) > 0, s, torch.ones_like(s))
+        code = torch.round(wf / s.to(torch.float32).unsqueeze(2)).clamp_(-8, 7).to(torch.int16).view(-1, H)
+        nib = (code & 15).to(torch.uint8)
+        w4[lo:lo + rows] = nib[:, 0::2] | (nib[:, 1::2] << 4)
+        sc[lo:lo + rows] = s
+    return w4, sc
 
 
 def make_fast_set(shape: Shape, seed: int) -> torch.Tensor:

@@ -514,3 +514,96 @@ def test_random_geometries_vs_oracle(prepos, oracle, path):
         check_attn(out, outs, sb)
         _check_append(sb, kp, vp, before, status, range(layers))
     assert ran >= 12
+
+
+# ---------------------------------------------------------------- NEXT-2: yield and resume
+@pytest.mark.parametrize("shape_key,n_s,l_entry,slice_n", [
+    ("d128_g4", [700, 15, 300], [24, 96, 64], 1),     # several units per CTA, cut and whole, 96 / 384 / 256 rows
+    ("d128_g4", [2500], [24], 1),                     # one unit per (layer, kv head) spread over many CTAs
+    ("d128_g2_l16", [3000], [200], 2),                # 16 layers: ~7 segments per CTA, two per launch
+    ("d128_g8", [517], [32], 1),
+    ("d64_g2", [333, 64], [8, 40], 1),
+])
+def test_sliced_pass_yield_and_resume_is_bit_identical(prepos, oracle, shape_key, n_s, l_entry, slice_n):
+    """A pass that stops at its yield points and is resumed until nothing is pending must give the result of an
+    uninterrupted call bit for bit (same plan, same split, same merge order) -- and match the oracle, Append(E)
+    included.  `set_attn_slice(n)` makes every launch stop after n segments per CTA, so every segment boundary of the
+    pass is exercised as a yield point, deterministically."""
+    shape = SHAPES[shape_key]
+    sb = synth.make_sessions(shape, n_s, l_entry, seed=4242 + sum(n_s))
+    out_ref, kp_ref, vp_ref, _, status, ctx0 = _gpu_run(prepos, sb, 2, poison=False)
+    ctx0.close()
+    dev = "cuda"
+    kp, vp = sb.k_pool.to(dev).clone(), sb.v_pool.to(dev).clone()
+    before = (kp.clone(), vp.clone())
+    out = torch.full(sb.q.shape, float("nan"), dtype=torch.bfloat16, device=dev)
+    ctx = _ctx(prepos, shape, sb.n_sessions, 2)
+    ctx.set_attn_slice(slice_n)
+    st = ctx.entry_attn(sb.q.to(dev), sb.k_new.to(dev), sb.v_new.to(dev), kp, vp, sb.page_table.to(dev),
+                        sb.n_s, sb.l_entry, sb.capacity, out)
+    launches = 1
+    while ctx.entry_attn_pending():
+        ctx.entry_attn_resume()
+        launches += 1
+        assert launches < 500
+    assert launches >= 2, "the pass never stopped: the slice was not honoured"
+    assert st == status
+    assert torch.equal(out.view(torch.int16), out_ref.view(torch.int16))
+    assert torch.equal(kp.view(torch.int16), kp_ref.view(torch.int16)) and torch.equal(vp.view(torch.int16), vp_ref.view(torch.int16))
+    outs, _, _, _ = oracle_attn_batch(oracle, sb)
+    check_attn(out, outs, sb)
+    _check_append(sb, kp, vp, before, status, range(shape.layers))
+    # an unsliced call on the same ctx afterwards is unaffected (counters and flag left clean)
+    ctx.set_attn_slice(0)
+    out2 = torch.full(sb.q.shape, float("nan"), dtype=torch.bfloat16, device=dev)
+    ctx.entry_attn(sb.q.to(dev), sb.k_new.to(dev), sb.v_new.to(dev), before[0], before[1], sb.page_table.to(dev),
+                   sb.n_s, sb.l_entry, sb.capacity, out2)
+    assert not ctx.entry_attn_pending()
+    assert torch.equal(out2.view(torch.int16), out_ref.view(torch.int16))
+
+
+def test_yield_request_from_another_stream_then_resume(prepos, oracle):
+    """The flag form: a long pass (config 2 geometry, 32 layers) is started on a low-priority stream, a yield is
+    requested from a high-priority stream while it runs, a kernel that needs whole SMs (another ctx's decode step) is
+    run there, then the pass is resumed.  The resumed result equals the uninterrupted one bit for bit, the decode
+    step's result is right, and in at least one of the trials the pass really was caught running (pending)."""
+    shape = synth.C2
+    seed = synth.SEED_BASE + 1
+    sb = synth.make_sessions(shape, [4096], [24], seed=seed, device="cuda", extra_pages=1)
+    k0, v0 = sb.k_pool.clone(), sb.v_pool.clone()
+    ctx = prepos.Context(shape.layers, shape.Hq, shape.Hkv, shape.d, shape.H, shape.V, shape.page, max_sessions=1)
+    ctx_d = prepos.Context(shape.layers, shape.Hq, shape.Hkv, shape.d, shape.H, shape.V, shape.page, max_sessions=1)
+    ref = torch.empty_like(sb.q)
+    ctx.entry_attn(sb.q, sb.k_new, sb.v_new, sb.k_pool, sb.v_pool, sb.page_table, sb.n_s, sb.l_entry, sb.capacity, ref)
+    ctx.sync()
+    # the decode step of another session living in the same pool geometry (its own pools)
+    sd = synth.make_sessions(shape, [2048], [1], seed=seed + 5, device="cuda")
+    dref = torch.empty_like(sd.q)
+    ctx_d.entry_attn(sd.q, sd.k_new, sd.v_new, sd.k_pool.clone(), sd.v_pool.clone(), sd.page_table, sd.n_s, sd.l_entry,
+                     sd.capacity, dref)
+    ctx_d.sync()
+    s_lo, s_hi = torch.cuda.Stream(priority=0), torch.cuda.Stream(priority=-1)
+    caught = 0
+    for trial in range(12):
+        sb.k_pool.copy_(k0)
+        sb.v_pool.copy_(v0)
+        out = torch.full(sb.q.shape, float("nan"), dtype=torch.bfloat16, device="cuda")
+        dout = torch.full(sd.q.shape, float("nan"), dtype=torch.bfloat16, device="cuda")
+        dk, dv = sd.k_pool.clone(), sd.v_pool.clone()
+        torch.cuda.synchronize()
+        with torch.cuda.stream(s_lo):
+            ctx.entry_attn(sb.q, sb.k_new, sb.v_new, sb.k_pool, sb.v_pool, sb.page_table, sb.n_s, sb.l_entry,
+                           sb.capacity, out)
+        with torch.cuda.stream(s_hi):
+            ctx.request_yield()
+            ctx_d.entry_attn(sd.q, sd.k_new, sd.v_new, dk, dv, sd.page_table, sd.n_s, sd.l_entry, sd.capacity, dout)
+        s_hi.synchronize()
+        with torch.cuda.stream(s_lo):
+            pending = ctx.entry_attn_pending()
+            caught += int(pending)
+            ctx.entry_attn_resume()
+            assert not ctx.entry_attn_pending()
+        torch.cuda.synchronize()
+        assert torch.equal(out.view(torch.int16), ref.view(torch.int16)), trial
+        assert torch.equal(dout.view(torch.int16), dref.view(torch.int16)), trial
+    assert caught >= 1, "no trial caught the pass running: the yield path was not exercised"

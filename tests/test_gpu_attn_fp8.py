@@ -1,0 +1,136 @@
+"""GPU parity of prepos_entry_attn_fp8 (a1 + a2 over an e4m3 KV cache, DESIGN.md reading
+Q20) against oracle O7, through the C ABI: every output row within the attention tolerance, and the pools after the
+call -- the codes Append(E) wrote for every entry token, and every other byte untouched -- bit for bit."""
+import numpy as np
+import pytest
+import torch
+
+from paper_2606_29565_b200 import synth
+from helpers import bits, ATTN_ATOL
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def prepos():
+    from paper_2606_29565_b200 import prepos as p
+    p.lib()
+    return p
+
+
+def _oracle_fp8(oracle, fb, layers=None):
+    """O7 per (layer, session) on host copies of the code pools (the oracle appends into them in place).
+    Returns ({(l, s): out fp64 [L, Hq, d]}, {s: status}, k codes after [layers...], v codes after)."""
+    sb = fb.base
+    layers = range(fb.k_pool8.shape[0]) if layers is None else layers
+    pt = sb.page_table.cpu().numpy()
+    k8 = {l: fb.k_pool8[l].cpu().numpy().copy() for l in layers}
+    v8 = {l: fb.v_pool8[l].cpu().numpy().copy() for l in layers}
+    outs, status = {}, {}
+    for l in layers:
+        ks, vs = fb.k_scale[l].cpu().numpy(), fb.v_scale[l].cpu().numpy()
+        for s in range(sb.n_sessions):
+            r0, L = sb.row_offset[s], sb.l_entry[s]
+            res = oracle.entry_attn_fp8(bits(sb.q[l, r0:r0 + L]), bits(sb.k_new[l, r0:r0 + L]), bits(sb.v_new[l, r0:r0 + L]),
+                                        k8[l], v8[l], ks, vs, pt[s], sb.n_s[s], sb.capacity[s])
+            outs[(l, s)] = res["out"]
+            status[s] = res["status"]
+    return outs, status, k8, v8
+
+
+def _run(prepos, fb):
+    sb, shape, dev = fb.base, fb.base.shape, "cuda"
+    ctx = prepos.Context(shape.layers, shape.Hq, shape.Hkv, shape.d, shape.H, shape.V, shape.page,
+                         max_sessions=max(sb.n_sessions, 1))
+    k8, v8 = fb.k_pool8.to(dev).clone(), fb.v_pool8.to(dev).clone()
+    out = torch.full(sb.q.shape, float("nan"), dtype=torch.bfloat16, device=dev)
+    st = ctx.entry_attn_fp8(sb.q.to(dev), sb.k_new.to(dev), sb.v_new.to(dev), k8, v8, fb.k_scale.to(dev),
+                            fb.v_scale.to(dev), sb.page_table.to(dev), sb.n_s, sb.l_entry, sb.capacity, out)
+    ctx.sync()
+    return out, k8, v8, st, ctx
+
+
+SHAPES = {
+    "d128_g4": synth.Shape("a", layers=2, Hq=8, Hkv=2, d=128, H=128, V=64, page=16),
+    "d128_g8": synth.Shape("b", layers=1, Hq=16, Hkv=2, d=128, H=128, V=64, page=16),
+    "d64_g2": synth.Shape("c", layers=2, Hq=4, Hkv=2, d=64, H=128, V=64, page=16),
+    "d128_g1": synth.Shape("d", layers=1, Hq=2, Hkv=2, d=128, H=128, V=64, page=16),
+    "d128_p32": synth.Shape("g", layers=1, Hq=8, Hkv=2, d=128, H=128, V=64, page=32),
+    "d96_g2": synth.Shape("h", layers=1, Hq=4, Hkv=2, d=96, H=128, V=64, page=8),
+}
+
+
+@pytest.mark.parametrize("shape_key,n_s,l_entry,tight", [
+    ("d128_g4", [0], [24], None),                         # n_s = 0: ordinary causal attention over the entry's own codes
+    ("d128_g4", [1], [1], None),
+    ("d128_g4", [127, 128, 129], [5, 16, 33], None),      # ragged pages: appends land in partly filled pages
+    ("d128_g4", [700, 15, 300], [24, 96, 64], None),
+    ("d128_g8", [517], [32], None),
+    ("d64_g2", [333, 64], [8, 40], None),
+    ("d128_g1", [260], [3], None),
+    ("d128_g4", [2500], [24], None),
+    ("d128_g4", [300, 100], [0, 7], None),                # an empty entry next to a real one
+    ("d128_p32", [333], [24], None),
+    ("d96_g2", [140], [6], None),
+    ("d128_g4", [100, 50, 200], [12, 20, 8], [None, 69, 208]),   # a budget skip (Alg. 1 l.2-3): nothing touched
+])
+def test_fp8_shapes_vs_oracle(prepos, oracle, shape_key, n_s, l_entry, tight):
+    shape = SHAPES[shape_key]
+    fb = synth.make_sessions_fp8(shape, n_s, l_entry, seed=3000 + 7 * sum(n_s) + sum(l_entry), tight_capacity=tight)
+    sb = fb.base
+    out, k8, v8, st, _ = _run(prepos, fb)
+    outs, ost, ok8, ov8 = _oracle_fp8(oracle, fb)
+    assert st == [ost[s] for s in range(sb.n_sessions)]
+    worst = 0.0
+    for (l, s), ref in outs.items():
+        r0, L = sb.row_offset[s], sb.l_entry[s]
+        got = out[l, r0:r0 + L].cpu().to(torch.float64).numpy()
+        if st[s] != 0:
+            assert np.isnan(got).all()          # skipped: rows untouched
+            continue
+        assert np.isfinite(got).all()
+        if ref.size:
+            worst = max(worst, float(np.abs(got - ref).max()))
+    assert worst <= ATTN_ATOL, worst
+    # Append(E): the codes the kernel stored == the oracle's, and every other byte of the pools unchanged
+    for l in range(shape.layers):
+        assert np.array_equal(k8[l].cpu().numpy(), ok8[l]), f"K codes differ at layer {l}"
+        assert np.array_equal(v8[l].cpu().numpy(), ov8[l]), f"V codes differ at layer {l}"
+
+
+def test_fp8_two_step_equals_one_step(prepos, oracle):
+    """Reading Q20: Forward(E) sees the entry tokens through their stored codes, so pre-positioning L1 then L2 tokens
+    is the same computation as L1 + L2 in one call: identical pools, rows equal up to the kernel's own rounding."""
+    shape = SHAPES["d128_g4"]
+    L1, L2, n = 10, 14, 200
+    fb = synth.make_sessions_fp8(shape, [n], [L1 + L2], seed=9)
+    sb, dev = fb.base, "cuda"
+    out_one, k1, v1, _, _ = _run(prepos, fb)
+    ctx = prepos.Context(shape.layers, shape.Hq, shape.Hkv, shape.d, shape.H, shape.V, shape.page, max_sessions=1)
+    k8, v8 = fb.k_pool8.to(dev).clone(), fb.v_pool8.to(dev).clone()
+    ks, vs, pt = fb.k_scale.to(dev), fb.v_scale.to(dev), sb.page_table.to(dev)
+    q, kn, vn = sb.q.to(dev), sb.k_new.to(dev), sb.v_new.to(dev)
+    o1 = torch.zeros((shape.layers, L1, shape.Hq, shape.d), dtype=torch.bfloat16, device=dev)
+    o2 = torch.zeros((shape.layers, L2, shape.Hq, shape.d), dtype=torch.bfloat16, device=dev)
+    ctx.entry_attn_fp8(q[:, :L1].contiguous(), kn[:, :L1].contiguous(), vn[:, :L1].contiguous(), k8, v8, ks, vs, pt,
+                       [n], [L1], sb.capacity, o1)
+    ctx.entry_attn_fp8(q[:, L1:].contiguous(), kn[:, L1:].contiguous(), vn[:, L1:].contiguous(), k8, v8, ks, vs, pt,
+                       [n + L1], [L2], sb.capacity, o2)
+    ctx.sync()
+    assert torch.equal(k8, k1) and torch.equal(v8, v1)
+    two = torch.cat([o1, o2], dim=1).float()
+    assert float((two - out_one.float()).abs().max()) <= 2 * ATTN_ATOL
+
+
+def test_fp8_config2_slice_sampled(prepos, oracle):
+    """BASELINE config 2 geometry (32/8 heads, d = 128, n_s = 4096, L = 24) on 2 of its layers at full session
+    length: every row of one layer and the appended codes of both."""
+    shape = synth.Shape("c2f", layers=2, Hq=32, Hkv=8, d=128, H=128, V=64, page=16)
+    fb = synth.make_sessions_fp8(shape, [4096], [24], seed=synth.SEED_BASE + 1, device="cuda")
+    sb = fb.base
+    out, k8, v8, st, _ = _run(prepos, fb)
+    assert st == [0]
+    outs, ost, ok8, ov8 = _oracle_fp8(oracle, fb, layers=[1])
+    got = out[1].cpu().to(torch.float64).numpy()
+    assert float(np.abs(got - outs[(1, 0)]).max()) <= ATTN_ATOL
+    assert np.array_equal(k8[1].cpu().numpy(), ok8[1]) and np.array_equal(v8[1].cpu().numpy(), ov8[1])

@@ -259,3 +259,69 @@ def test_full_size_vocabulary(prepos, oracle, name, n):
         d, _ = check_decision(oracle, int(dec[q]), int(tok[q]), refs[r], True, 0, 0, obm, shape.V, shape.tau)
         fired += d == oracle.SERVED
     assert fired >= 1 or n == 1
+
+
+# ---------------------------------------------------------------- NEXT-4: 4-bit W_vocab (reading Q21, oracle O8)
+def _run_ready_w4(prepos, shape, hidden, w4, sc, with_logits=True):
+    n = hidden.shape[0]
+    ctx = prepos.Context(shape.layers, shape.Hq, shape.Hkv, shape.d, shape.H, shape.V, shape.page, max_sessions=max(n, 1))
+    dev = "cuda"
+    sid = torch.arange(n, dtype=torch.int32, device=dev)
+    recs = prepos.new_records(n)
+    ver = torch.zeros(n, dtype=torch.int64, device=dev)
+    logits = torch.full((n, shape.V), float("nan"), dtype=torch.float32, device=dev) if with_logits else None
+    ctx.ready_dist_w4(sid, hidden.to(dev), w4.to(dev), sc.to(dev), recs, ver, logits_out=logits)
+    ctx.sync()
+    return ctx, recs, ver, logits
+
+
+@pytest.mark.parametrize("V,H,n", [(1024, 256, 1), (1000, 128, 3), (130, 384, 8), (257, 640, 9), (4096, 1024, 8),
+                                   (2, 128, 1), (20000, 512, 5), (513, 2048, 20)])
+def test_w4_ragged_vocab_vs_oracle(prepos, oracle, V, H, n):
+    """prepos_ready_dist_w4 against O8 (logits over the int4 codes and group scales, reading Q21) + O3: every logit
+    and the record, for V not a multiple of the 128-row tile, H / 128 = 1, 2, 3, 4, 5, 8, 16 scale groups (whole and
+    partial 4-box stages), n below, at and above the 8-row pass."""
+    shape = synth.Shape("w4", layers=1, Hq=4, Hkv=2, d=64, H=H, V=V, fast_set=2)
+    w4, sc = synth.make_w_vocab_w4(shape, 5)
+    hidden = synth.randn_bf16((n, H), synth.gen(6))
+    ctx, recs, ver, logits = _run_ready_w4(prepos, shape, hidden, w4, sc)
+    rec = prepos.unpack_records(recs)
+    assert rec["flags"].tolist() == [prepos.FLAG_VALID] * n
+    for r in range(n):
+        check_record(oracle, rec, r, oracle.logits_w4(w4.numpy(), bits(sc), bits(hidden[r])), logits[r].cpu().numpy())
+
+
+def test_w4_extreme_codes_and_unit_scales(prepos, oracle):
+    """Every code value -8..7 in every nibble position with power-of-two scales and a hidden row of small integers:
+    all products and sums are exact in fp32, so the GPU logits must EQUAL the oracle's (catches a wrong nibble order,
+    sign extension or k permutation, which a tolerance could hide)."""
+    V, H = 256, 256
+    shape = synth.Shape("w4x", layers=1, Hq=4, Hkv=2, d=64, H=H, V=V, fast_set=2)
+    g = torch.Generator().manual_seed(3)
+    codes = torch.randint(-8, 8, (V, H), generator=g, dtype=torch.int16)
+    codes[0, :16] = torch.arange(-8, 8, dtype=torch.int16)
+    nib = (codes & 15).to(torch.uint8)
+    w4 = (nib[:, 0::2] | (nib[:, 1::2] << 4)).contiguous()
+    sc = (2.0 ** torch.randint(-3, 3, (V, H // 128), generator=g).float()).to(torch.bfloat16)
+    hidden = torch.randint(-4, 5, (3, H), generator=g).to(torch.bfloat16)
+    hidden[1] = 0
+    hidden[1, 5] = 1          # picks column 5 of W: logits = code[:, 5] * scale
+    ctx, recs, ver, logits = _run_ready_w4(prepos, shape, hidden, w4, sc)
+    for r in range(3):
+        ref = oracle.logits_w4(w4.numpy(), bits(sc), bits(hidden[r]))
+        assert np.array_equal(logits[r].cpu().numpy().astype(np.float64), ref), r
+
+
+@pytest.mark.parametrize("name,n", [("c2", 1), ("c5", 4)])
+def test_w4_full_size_vocabulary(prepos, oracle, name, n):
+    """The int4 LM head at BASELINE's vocabulary shapes (V = 128256, H = 4096 / 8192) in bench.py's launch
+    configuration: every logit of every row and the records against O8 + O3."""
+    shape = synth.C2 if name == "c2" else synth.C5
+    seed = synth.SEED_BASE + int(name[1])
+    w4, sc = synth.make_w_vocab_w4(shape, seed, "cuda")
+    hidden = synth.randn_bf16((n, shape.H), synth.gen(seed + 1, "cuda"))
+    ctx, recs, ver, logits = _run_ready_w4(prepos, shape, hidden, w4, sc)
+    rec = prepos.unpack_records(recs)
+    w4h, sch = w4.cpu().numpy(), bits(sc)
+    for r in range(n):
+        check_record(oracle, rec, r, oracle.logits_w4(w4h, sch, bits(hidden[r])), logits[r].cpu().numpy())
