@@ -215,7 +215,7 @@ int64_t prepos_ctx_launch_count(const prepos_ctx *ctx) { return ctx ? ctx->launc
 int prepos_ctx_set_attn_path(prepos_ctx *ctx, int path)
 {
     if (!ctx || path < 0 || path > 2) return PREPOS_E_INVALID_ARG;
-    if (path == 2 && !prepos_attn_umma_supported(ctx)) return PREPOS_E_SHAPE;
+    if (path == 2 && !prepos_attn_umma_supported(ctx) && !prepos_attn_umma_fp8_supported(ctx)) return PREPOS_E_SHAPE;
     ctx->attn_path = path;
     ctx->plan_key.clear();
     return PREPOS_OK;
@@ -398,9 +398,11 @@ int prepos_entry_attn_fp8(prepos_ctx *ctx, int layer_begin, int layer_end, int n
     if (n_pages <= 0 || page_table_stride <= 0) return PREPOS_E_INVALID_ARG;
 
     const int G = s.n_q_heads / s.n_kv_heads;
-    const int chunk_tok = (G > 16 ? 1 : 16 / G);
-    const int st = plan_attn(ctx, 3, chunk_tok, true, n_sessions, page_table_stride, n_s, l_entry, capacity_tokens,
-                             status_per_session, static_cast<cudaStream_t>(stream));
+    if (ctx->attn_path == 2 && !prepos_attn_umma_fp8_supported(ctx)) return PREPOS_E_SHAPE;
+    const bool use_umma = (ctx->attn_path != 1) && prepos_attn_umma_fp8_supported(ctx);
+    const int chunk_tok = use_umma ? (kAttnMaxRows / G > 0 ? kAttnMaxRows / G : 1) : (G > 16 ? 1 : 16 / G);
+    const int st = plan_attn(ctx, use_umma ? 4 : 3, chunk_tok, true, n_sessions, page_table_stride, n_s, l_entry,
+                             capacity_tokens, status_per_session, static_cast<cudaStream_t>(stream));
     if (st != PREPOS_OK) return st;
     if (ctx->plan_units.empty()) return PREPOS_OK;
 
@@ -428,7 +430,8 @@ int prepos_entry_attn_fp8(prepos_ctx *ctx, int layer_begin, int layer_end, int n
     a.page_table = page_table;
     a.page_table_stride = page_table_stride;
     a.scale = softmax_scale > 0.f ? softmax_scale : 1.0f / sqrtf(static_cast<float>(s.head_dim));
-    return prepos_launch_attn_fp8(ctx, a, static_cast<cudaStream_t>(stream));
+    const AttnUnit &last = ctx->plan_units.back();
+    return prepos_launch_attn_fp8(ctx, a, use_umma, last.tile_prefix + last.n_tiles, static_cast<cudaStream_t>(stream));
 }
 
 int prepos_ctx_set_attn_slice(prepos_ctx *ctx, int max_segments_per_launch)

@@ -11,6 +11,7 @@
 //                       into the session's pages (a1)
 //   attn_fp8_kernel     every row then reads ALL its keys -- the n_s cached tokens and the entry tokens up to its
 //                       own -- from the pages: one load path, the causal limit is just a per-row key count (a2).
+//                       d = 128 with pages of >= 16 tokens takes the tcgen05 kernel instead (attn_umma.cu, kFp8).
 //                       Shape-generic CUDA-core formulation (one CTA per (row chunk, kv head, layer), 32-token tiles
 //                       dequantised into shared memory as fp32, one warp per query row, fp32 online softmax).
 #include <cuda_fp8.h>
@@ -223,7 +224,7 @@ __global__ void __launch_bounds__(kThreads) attn_fp8_kernel(const Fp8Params p)
 
 }  // namespace
 
-int prepos_launch_attn_fp8(prepos_ctx *ctx, const AttnArgs &a, cudaStream_t stream)
+int prepos_launch_attn_fp8(prepos_ctx *ctx, const AttnArgs &a, bool use_umma, int total_tiles_per_lh, cudaStream_t stream)
 {
     Fp8Params p;
     p.a = a;
@@ -243,7 +244,10 @@ int prepos_launch_attn_fp8(prepos_ctx *ctx, const AttnArgs &a, cudaStream_t stre
                                          static_cast<int>(smem)));
     const dim3 grid(a.n_units, p.Hkv, a.layer_end - a.layer_begin);
     PREPOS_CUDA_TRY(prepos_launch_pdl(fp8_append_kernel, grid, dim3(kThreads), 0, stream, p));
+    ctx->launches += 1;
+    // d = 128 with pages of >= 16 tokens: the tcgen05 kernel (attn_umma.cu, kFp8) reads the codes back from the pages
+    if (use_umma) return prepos_launch_attn_umma_fp8(ctx, a, total_tiles_per_lh, stream);
     PREPOS_CUDA_TRY(prepos_launch_pdl(attn_fp8_kernel, grid, dim3(kThreads), smem, stream, p));
-    ctx->launches += 2;
+    ctx->launches += 1;
     return PREPOS_OK;
 }

@@ -242,18 +242,29 @@ __device__ __forceinline__ void append_entry(const UmmaParams &p, const Seg &s, 
     }
 }
 
-template <int D>
+// kFp8 (reading Q20): the pools hold e4m3 codes with one fp32 scale per (page, kv
+// head).  A tile arrives as 128 x D BYTES (half the HBM traffic) in the upper half of its ring slot and is widened in
+// place to the fp16 tile the MMA reads (e4m3 -> fp16 is exact) by a service warp: warp 2 the K tiles, warp 3 the V
+// tiles (which also issues the V loads).  Q is converted bf16 -> fp16 in place by the softmax warps at the start of a
+// segment, P is written as fp16: both MMAs run as f16 x f16.  The page scales never touch an operand: the K scale of
+// a column's page multiplies its score inside the softmax's scale FMA, the V scale multiplies its probability before
+// P is packed.  The entry tokens were appended (quantised) by fp8_append_kernel before this launch and are read back
+// from the pages like cached ones: a unit has no entry tiles, causality is a per-row column limit.
+template <int D, bool kFp8>
 __global__ void __maxnreg__(kLaunchRegs)
 attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__ CUtensorMap tm_v,
                  const __grid_constant__ CUtensorMap tm_kn, const __grid_constant__ CUtensorMap tm_vn,
                  const __grid_constant__ CUtensorMap tm_q,
                  const UmmaParams p)
 {
+    static_assert(!kFp8 || D == 128, "the FP8 tiles are one 128-byte swizzle row per token");
     constexpr int kHalves = D / 64;
     constexpr int kTileBytes = kTile * D * 2;         // one K or V tile / one Q M-tile
+    constexpr int kRawBytes = kTile * D;              // an e4m3 tile as it arrives (kFp8)
     constexpr int kGroupStride = kHalves * 1024;      // bytes between 8-row groups
-    constexpr uint32_t kIdescQK = (1u << 4) | (1u << 7) | (1u << 10) | ((kTile >> 3) << 17) | ((128u >> 4) << 24);
-    constexpr uint32_t kIdescPV = (1u << 4) | (1u << 7) | (1u << 10) | (1u << 16) | ((D >> 3) << 17) | ((128u >> 4) << 24);
+    constexpr uint32_t kFmt = kFp8 ? 0u : 1u;         // kind::f16 operand format: 0 = f16, 1 = bf16
+    constexpr uint32_t kIdescQK = (1u << 4) | (kFmt << 7) | (kFmt << 10) | ((kTile >> 3) << 17) | ((128u >> 4) << 24);
+    constexpr uint32_t kIdescPV = (1u << 4) | (kFmt << 7) | (kFmt << 10) | (1u << 16) | ((D >> 3) << 17) | ((128u >> 4) << 24);
     constexpr uint32_t kDescHi = desc_hi(kGroupStride);
     constexpr int kColS = 0;        // S_w at columns w * 128 (P_w aliases its first 64 columns)
     constexpr int kColO = 256;      // O_w at columns 256 + w * D
@@ -268,13 +279,16 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
     uint64_t *k_full = bars, *k_empty = bars + 3, *v_full = bars + 6, *v_empty = bars + 9;
     uint64_t *s_full = bars + 12, *p_ready = bars + 14, *o_done = bars + 16, *q_full = bars + 18;
     uint64_t *q_empty = bars + 19;    // the segment's last QK has read Q: the loader may overwrite it
-    float2 *ml_x = reinterpret_cast<float2 *>(bars + 20);  // [128] (m, l) of stream 1 / the row factors back
+    uint64_t *k_conv = bars + 20, *v_conv = bars + 23, *q_conv = bars + 26;   // kFp8: tile / Q widened to fp16
+    float2 *ml_x = reinterpret_cast<float2 *>(bars + 27);  // [128] (m, l) of stream 1 / the row factors back
     uint32_t *tmem_slot = reinterpret_cast<uint32_t *>(ml_x + 128);
     int *merge_info = reinterpret_cast<int *>(tmem_slot + 1);  // [3]: c0 (or -1 = not last), c1, c0's slot
     // segment admission (yield / resume): [0] segments admitted in this launch, [1] the first one refused (or
     // INT_MAX), [2] segments completed in the pass when this launch ends.  Written by lane 0 of the K producer, the
     // role that reaches a segment first; every other role asks before it starts a segment.
     int *sched = merge_info + 3;
+    // kFp8: page scales of the last 8 K tiles, [tile % 8][0..7 K scale of 16-column block b | 8..15 V scale]
+    float *sc_s = reinterpret_cast<float *>((reinterpret_cast<uintptr_t>(sched + 3) + 15) & ~uintptr_t(15));
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
 
@@ -292,6 +306,11 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
         }
         ptx::mbar_init(ptx::smem_u32(q_full), 1);
         ptx::mbar_init(ptx::smem_u32(q_empty), 1);
+        for (int i = 0; i < 3; ++i) {
+            ptx::mbar_init(ptx::smem_u32(&k_conv[i]), 1);
+            ptx::mbar_init(ptx::smem_u32(&v_conv[i]), 1);
+        }
+        ptx::mbar_init(ptx::smem_u32(q_conv), 1);
         ptx::fence_mbar_init();
         sched[0] = 0;
         sched[1] = 0x7fffffff;
@@ -303,8 +322,10 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
     } else if (threadIdx.x == 0) {
         ptx::prefetch_tmap(&tm_k);
         ptx::prefetch_tmap(&tm_v);
-        ptx::prefetch_tmap(&tm_kn);
-        ptx::prefetch_tmap(&tm_vn);
+        if constexpr (!kFp8) {
+            ptx::prefetch_tmap(&tm_kn);
+            ptx::prefetch_tmap(&tm_vn);
+        }
         ptx::prefetch_tmap(&tm_q);
     }
     // rows of a Q M-tile that no TMA box covers are never written: clear the buffer once so they stay finite (part of
@@ -335,12 +356,106 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
     const int pages_per_tile = kTile >> p.page_shift;
     const int page_bytes = p.page * D * 2;
     const int page_groups = p.page >> 3;
+    // the role's next segment of this launch (skipping what the pass already completed); false at the end or a yield
+    auto next_seg = [&](SegIter &it, Seg &s, int &seg, int &kproc) -> bool {
+        while (it.next(p, s)) {
+            if (seg++ < skip) continue;
+            if (!admitted(kproc)) return false;
+            ++kproc;
+            return true;
+        }
+        return false;
+    };
+    // kFp8: widen the e4m3 tile in the upper half of `slot` to the fp16 tile the MMA reads, in place, by one warp.
+    // Lane = token row, four batches of 32 rows in ascending order: the output of a batch (8 KB from byte 8 KB x
+    // batch) only ever covers raw rows of earlier batches or of the batch itself, all of which are in registers by
+    // then.  Rows from `zero_from` on are written as zeros (V: P is 0 there, but 0 x NaN would poison O).
+    auto widen_tile = [&](uint8_t *slot, int zero_from) {
+#pragma unroll 1
+        for (int b = 0; b < kTile / 32; ++b) {
+            const int r = b * 32 + lane;
+            uint4 raw[D / 16];
+#pragma unroll
+            for (int c = 0; c < D / 16; ++c)
+                raw[c] = *reinterpret_cast<const uint4 *>(slot + kRawBytes + r * D + ((c ^ (r & 7)) << 4));
+            __syncwarp();
+            const bool live = r < zero_from;
+#pragma unroll
+            for (int c = 0; c < D / 16; ++c) {
+                const uint32_t w[4] = {raw[c].x, raw[c].y, raw[c].z, raw[c].w};
+                uint32_t h[8];
+#pragma unroll
+                for (int i = 0; i < 4; ++i) {
+                    h[2 * i] = live ? ptx::e4m3x2_to_f16x2(w[i] & 0xffffu) : 0u;
+                    h[2 * i + 1] = live ? ptx::e4m3x2_to_f16x2(w[i] >> 16) : 0u;
+                }
+                *reinterpret_cast<uint4 *>(slot + tile_offset<D>(r, 2 * c)) = make_uint4(h[0], h[1], h[2], h[3]);
+                *reinterpret_cast<uint4 *>(slot + tile_offset<D>(r, 2 * c + 1)) = make_uint4(h[4], h[5], h[6], h[7]);
+            }
+            __syncwarp();
+        }
+        ptx::fence_proxy_async_smem();
+        __syncwarp();
+    };
 
     // register budget: launch gives kLaunchRegs x 384 threads.  The four service warps (warpgroup 0) hand theirs
     // down to kServiceRegs; each softmax thread, which holds a 128-wide score row, grows to kSoftmaxRegs.
     if (warp < 4) {
     ptx::setmaxnreg_dec<kServiceRegs>();
-    if (warp == 0 || warp == 3) {
+    if (kFp8 && warp == 3) {
+        // ===================== kFp8: V loads and V widening =====================
+        // Loads run nv - 1 tiles ahead of the widening: tile c is widened, then tile c + nv - 1 is requested into the
+        // slot tile c - 1 leaves (free once its PV has retired).
+        if constexpr (kFp8) {
+            const uint64_t pol = ptx::policy_evict_first();
+            SegIter it_i(p, t0, t1), it_c(p, t0, t1);
+            Seg si, sc;
+            int seg_i = 0, kp_i = 0, seg_c = 0, kp_c = 0;
+            bool more_i = next_seg(it_i, si, seg_i, kp_i), more_c = next_seg(it_c, sc, seg_c, kp_c);
+            int ti = more_i ? si.tb : 0, tc = more_c ? sc.tb : 0;
+            int islot = 0, cslot = 0;
+            uint32_t iph = 0, cph = 0;
+            auto issue_one = [&]() {
+                const int n_pages_valid = (si.u.n_load + p.page - 1) >> p.page_shift;
+                const int32_t *pt = p.a.page_table + static_cast<size_t>(si.u.session) * p.a.page_table_stride;
+                const int idx = ti * pages_per_tile + lane;
+                const int pg = (lane < pages_per_tile && idx < n_pages_valid) ? __ldg(pt + idx) : -1;
+                if (lane == 0) ptx::mbar_wait(ptx::smem_u32(&v_empty[islot]), iph ^ 1);
+                __syncwarp();
+                int nvp = n_pages_valid - ti * pages_per_tile;
+                nvp = nvp < pages_per_tile ? nvp : pages_per_tile;
+                const uint32_t fb = ptx::smem_u32(&v_full[islot]);
+                if (lane == 0) ptx::mbar_arrive_expect_tx(fb, nvp * p.page * D);
+                __syncwarp();
+                if (pg >= 0)
+                    ptx::tma_load_3d(ptx::smem_u32(v_s + islot * kTileBytes + kRawBytes + lane * p.page * D), &tm_v, fb, 0,
+                                     (pg * p.Hkv + si.kvh) * p.page, si.layer, pol);
+                if (++islot == p.nv) {
+                    islot = 0;
+                    iph ^= 1;
+                }
+                if (++ti == si.te) {
+                    more_i = next_seg(it_i, si, seg_i, kp_i);
+                    ti = more_i ? si.tb : 0;
+                }
+            };
+            for (int k = 0; k < p.nv - 1 && more_i; ++k) issue_one();
+            while (more_c) {
+                ptx::mbar_wait(ptx::smem_u32(&v_full[cslot]), cph);
+                widen_tile(v_s + cslot * kTileBytes, sc.u.n_load - tc * kTile);
+                if (lane == 0) ptx::mbar_arrive(ptx::smem_u32(&v_conv[cslot]));
+                if (++cslot == p.nv) {
+                    cslot = 0;
+                    cph ^= 1;
+                }
+                if (++tc == sc.te) {
+                    more_c = next_seg(it_c, sc, seg_c, kp_c);
+                    tc = more_c ? sc.tb : 0;
+                }
+                if (more_i) issue_one();
+            }
+        }
+    } else if (warp == 0 || warp == 3) {
         // ===================== K (warp 0) / V (warp 3) TMA producers =====================
         const bool is_v = (warp == 3);
         const CUtensorMap *tm = is_v ? &tm_v : &tm_k;
@@ -372,7 +487,7 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
                 break;
             }
             ++kproc;
-            const int n_pages_valid = (s.u.n_s + p.page - 1) >> p.page_shift;
+            const int n_pages_valid = (s.u.n_load + p.page - 1) >> p.page_shift;
             const int32_t *pt = p.a.page_table + static_cast<size_t>(s.u.session) * p.a.page_table_stride;
             // this lane's page of tile t (page-table reads run one tile ahead of the TMA issue)
             auto page_of = [&](int t) -> int {
@@ -388,7 +503,16 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
                 __syncwarp();
                 uint8_t *dst = ring + slot * kTileBytes;
                 const uint32_t fb = ptx::smem_u32(&full[slot]);
-                if (t < s.u.n_cached_tiles) {
+                if constexpr (kFp8) {
+                    // e4m3 page slabs ([page tokens][D bytes], 128-byte swizzle) into the upper half of the slot
+                    int nvp = n_pages_valid - t * pages_per_tile;
+                    nvp = nvp < pages_per_tile ? nvp : pages_per_tile;
+                    if (lane == 0) ptx::mbar_arrive_expect_tx(fb, nvp * p.page * D);
+                    __syncwarp();
+                    if (pg >= 0)
+                        ptx::tma_load_3d(ptx::smem_u32(dst + kRawBytes + lane * p.page * D), tm, fb, 0,
+                                         (pg * p.Hkv + s.kvh) * p.page, s.layer, pol);
+                } else if (t < s.u.n_cached_tiles) {
                     int nvp = n_pages_valid - t * pages_per_tile;
                     nvp = nvp < pages_per_tile ? nvp : pages_per_tile;
                     if (lane == 0) ptx::mbar_arrive_expect_tx(fb, nvp * page_bytes);
@@ -429,6 +553,8 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
         Seg s;
         const uint64_t pol_q = ptx::policy_evict_last();  // Q is re-read by every CTA that shares the unit
         int k = 0, seg = 0;
+        int cslot = 0, ktile = 0;   // kFp8: ring slot and running index of the K tile being widened
+        uint32_t cph = 0;
         while (it.next(p, s)) {
             if (seg++ < skip) continue;
             if (!admitted(k)) break;
@@ -457,10 +583,43 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
                 }
             }
             ++k;
-            // ---- Append(E) (Alg. 1 l.5): K_new / V_new -> the session's pages.  Owned by the CTA that runs the last
-            // tile of the session's last row chunk, once per (layer, kv head).  Nothing in this launch reads cache
-            // positions >= n_s, so the copy needs no ordering with the tiles.
-            if (s.u.tok0 + s.u.ntok == s.u.l_entry && s.te == s.u.n_tiles) append_entry<D>(p, s, lane);
+            if constexpr (kFp8) {
+                // ---- widen the segment's K tiles as they land, and put the page scales of each tile's eight 16-column
+                // blocks (lanes 0-7: K, lanes 8-15: V) where the softmax finds them.  Page ids are read two tiles, the
+                // scales one tile ahead of their use.
+                const int n_pages_valid = (s.u.n_load + p.page - 1) >> p.page_shift;
+                const int32_t *pt = p.a.page_table + static_cast<size_t>(s.u.session) * p.a.page_table_stride;
+                const float *scl = (lane < 8 ? p.a.k_scale : p.a.v_scale) + static_cast<size_t>(s.layer) * p.a.scale_layer_stride;
+                auto page_of = [&](int t) -> int {
+                    const int idx = t * pages_per_tile + (((lane & 7) * 16) >> p.page_shift);
+                    return (lane < 16 && t < s.te && idx < n_pages_valid) ? __ldg(pt + idx) : -1;
+                };
+                auto scale_of = [&](int pg) -> float {
+                    return pg >= 0 ? __ldg(scl + static_cast<size_t>(pg) * p.Hkv + s.kvh) : 0.f;
+                };
+                int pg1 = page_of(s.tb + 1);
+                float sc0 = scale_of(page_of(s.tb));
+                for (int t = s.tb; t < s.te; ++t) {
+                    const float sc_now = sc0;
+                    sc0 = scale_of(pg1);
+                    pg1 = page_of(t + 2);
+                    ptx::mbar_wait(ptx::smem_u32(&k_full[cslot]), cph);
+                    widen_tile(k_s + cslot * kTileBytes, kTile);
+                    if (lane < 16) sc_s[(ktile & 7) * 16 + lane] = sc_now;
+                    __syncwarp();
+                    if (lane == 0) ptx::mbar_arrive(ptx::smem_u32(&k_conv[cslot]));
+                    ++ktile;
+                    if (++cslot == kNK) {
+                        cslot = 0;
+                        cph ^= 1;
+                    }
+                }
+            } else {
+                // ---- Append(E) (Alg. 1 l.5): K_new / V_new -> the session's pages.  Owned by the CTA that runs the
+                // last tile of the session's last row chunk, once per (layer, kv head).  Nothing in this launch reads
+                // cache positions >= n_s, so the copy needs no ordering with the tiles.
+                if (s.u.tok0 + s.u.ntok == s.u.l_entry && s.te == s.u.n_tiles) append_entry<D>(p, s, lane);
+            }
         }
     } else if (warp == 1) {
         // ===================== MMA issuer =====================
@@ -478,7 +637,7 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
             const int n_mt = rows > 128 ? 2 : 1;
             const int n_tiles = s.te - s.tb;
             const int n_items = n_tiles * n_mt;
-            ptx::mbar_wait(ptx::smem_u32(q_full), qph);
+            ptx::mbar_wait(ptx::smem_u32(kFp8 ? q_conv : q_full), qph);
             qph ^= 1;
             ptx::tc_fence_after();
 
@@ -488,7 +647,7 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
                 const bool first_use = (n_mt == 1) || w == 0;
                 const bool last_use = (n_mt == 1) || w == 1;
                 if (first_use) {
-                    ptx::mbar_wait(ptx::smem_u32(&k_full[kslot]), kph);
+                    ptx::mbar_wait(ptx::smem_u32(kFp8 ? &k_conv[kslot] : &k_full[kslot]), kph);
                     ptx::tc_fence_after();
                 }
                 // descriptor words are warp-uniform and computed by the whole warp; only the tcgen05 instructions sit
@@ -526,7 +685,9 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
                 const int t = s.tb + (n_mt == 2 ? (i >> 1) : i);
                 const bool first_use = (n_mt == 1) || w == 0;
                 const bool last_use = (n_mt == 1) || w == 1;
-                if (first_use) {
+                if (first_use && kFp8) {
+                    ptx::mbar_wait(ptx::smem_u32(&v_conv[vslot]), vph);   // widened, rows past the valid tokens zeroed
+                } else if (first_use) {
                     ptx::mbar_wait(ptx::smem_u32(&v_full[vslot]), vph);
                     // rows past the valid tokens of a ragged cached tile hold whatever the pool / the ring held, and the
                     // last 8-token box of an entry tile reaches into rows of later tokens or of the NEXT session (which
@@ -534,7 +695,7 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
                     // but 0 * NaN would poison O, so zero them before the MMA reads them.
                     int valid, zero_to;
                     if (t < s.u.n_cached_tiles) {
-                        valid = s.u.n_s - t * kTile;
+                        valid = s.u.n_load - t * kTile;
                         zero_to = kTile;
                     } else {
                         valid = s.u.tok0 + s.u.ntok - (t - s.u.n_cached_tiles) * kTile;
@@ -589,6 +750,8 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
         const uint32_t lane_addr = static_cast<uint32_t>((warp & 3) << 5) << 16;
         const int st = threadIdx.x - 128;                      // 0..255 among softmax threads
         uint32_t sph = 0, oph = 0;
+        uint32_t qph = 0;      // kFp8: parity of q_full
+        int ktile_base = 0;    // kFp8: K tiles of the segments before this one (index of the scale ring)
         SegIter it(p, t0, t1);
         Seg s;
         int seg = 0, kproc = 0;
@@ -603,6 +766,23 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
             const int mt = (n_mt == 2) ? w : 0;
             const int urow = mt * 128 + row;                   // row within the unit
             const int my_tok = s.u.tok0 + urow / G;            // entry token of this row (if urow < rows)
+            if constexpr (kFp8) {
+                // Q arrived as bf16: widen it to fp16 in place (same size, same swizzled layout; exact for
+                // 2^-14 <= |q| < 65504, below that the fp16 subnormal grid 2^-24), then hand it to the MMA warp
+                ptx::mbar_wait(ptx::smem_u32(q_full), qph);
+                qph ^= 1;
+                for (int off = st * 16; off < p.q_tiles * kTileBytes; off += 256 * 16) {
+                    uint4 v = *reinterpret_cast<const uint4 *>(q_s + off);
+                    v.x = ptx::bf16x2_to_f16x2(v.x);
+                    v.y = ptx::bf16x2_to_f16x2(v.y);
+                    v.z = ptx::bf16x2_to_f16x2(v.z);
+                    v.w = ptx::bf16x2_to_f16x2(v.w);
+                    *reinterpret_cast<uint4 *>(q_s + off) = v;
+                }
+                ptx::fence_proxy_async_smem();
+                ptx::bar_sync(1, 256);
+                if (st == 0) ptx::mbar_arrive(ptx::smem_u32(q_conv));
+            }
             float m_used = -CUDART_INF_F, l_sum = 0.f;
             bool have = false;
             for (int i = w; i < n_items; i += 2) {
@@ -610,8 +790,13 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
                 // visible columns of this tile for this row
                 int limit = kTile;
                 if (t < s.u.n_cached_tiles) {
-                    const int valid = s.u.n_s - t * kTile;
+                    const int valid = s.u.n_load - t * kTile;
                     limit = valid < kTile ? valid : kTile;
+                    if constexpr (kFp8) {
+                        // the entry tokens sit in the cache: row i sees keys j <= n_s + i (reading Q5)
+                        const int causal = (urow < rows) ? s.u.n_s + my_tok + 1 - t * kTile : kTile;
+                        limit = causal < limit ? (causal < 0 ? 0 : causal) : limit;
+                    }
                 } else {
                     const int nb = (t - s.u.n_cached_tiles) * kTile;
                     limit = (urow < rows) ? my_tok - nb + 1 : 1;   // causal among the entry tokens (reading Q5)
@@ -708,13 +893,104 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
                     ptx::unpack_f32x2(ptx::add_f32x2(acc_a, acc_b), a0, a1);
                     l_sum += a0 + a1;
                 };
-                if (limit >= kTile) tile_body(std::false_type{});
-                else tile_body(std::true_type{});
+                // kFp8: the same body with the K scale of each 16-column block in the scale FMA (and in the maximum,
+                // block by block) and the V scale on the probabilities before they are packed (fp16)
+                auto tile_body_q = [&](auto masked_tag) {
+                    constexpr bool kMasked = decltype(masked_tag)::value;
+                    const float *scb = sc_s + ((ktile_base + (t - s.tb)) & 7) * 16;
+                    uint32_t sr[128];
+                    {
+                        const uint32_t sa = tmem + lane_addr + kColS + w * 128;
+                        ptx::tmem_ld_32x32b_x32(sa, sr);
+                        ptx::tmem_ld_32x32b_x32(sa + 32, sr + 32);
+                        ptx::tmem_ld_32x32b_x32(sa + 64, sr + 64);
+                        ptx::tmem_ld_32x32b_x32(sa + 96, sr + 96);
+                        ptx::tmem_ld_wait();
+                    }
+                    float mx = -CUDART_INF_F;
+#pragma unroll
+                    for (int b = 0; b < 8; ++b) {
+                        float m0 = -CUDART_INF_F, m1 = -CUDART_INF_F;
+#pragma unroll
+                        for (int c = b * 16; c < b * 16 + 16; c += 2) {
+                            if constexpr (kMasked) {
+                                if (c >= limit) sr[c] = __float_as_uint(-CUDART_INF_F);
+                                if (c + 1 >= limit) sr[c + 1] = __float_as_uint(-CUDART_INF_F);
+                            }
+                            m0 = fmaxf(m0, __uint_as_float(sr[c]));
+                            m1 = fmaxf(m1, __uint_as_float(sr[c + 1]));
+                        }
+                        const float mb = fmaxf(m0, m1);
+                        // a block with no visible column has max -inf (and, past the valid pages, scale 0)
+                        if (mb != -CUDART_INF_F) mx = fmaxf(mx, mb * (scb[b] * p.scale_log2));
+                    }
+                    const float m_new = fmaxf(m_used, mx);
+                    const bool need = (m_new > m_used + kRescaleThreshold);
+                    if (__any_sync(0xffffffffu, need)) {
+                        const float alpha = (m_used == -CUDART_INF_F) ? 0.f : exp2f(m_used - m_new);
+                        l_sum *= alpha;
+                        if (have) {
+                            const uint32_t oa = tmem + lane_addr + kColO + w * D;
+#pragma unroll 1
+                            for (int cb = 0; cb < D; cb += 32) {
+                                uint32_t o[32];
+                                ptx::tmem_ld_32x32b_x32(oa + cb, o);
+                                ptx::tmem_ld_wait();
+#pragma unroll
+                                for (int c = 0; c < 32; ++c) o[c] = __float_as_uint(__uint_as_float(o[c]) * alpha);
+                                ptx::tmem_st_32x32b_x32(oa + cb, o);
+                            }
+                        }
+                        m_used = m_new;
+                    }
+                    const float m_eff = (m_used == -CUDART_INF_F) ? 0.f : m_used;
+                    const float neg_m = -m_eff;
+                    const uint32_t pa = tmem + lane_addr + kColS + w * 128;
+                    const uint64_t nm2 = ptx::pack_f32x2(neg_m, neg_m);
+                    uint64_t acc_a = 0ull, acc_b = 0ull;
+#pragma unroll
+                    for (int cb = 0; cb < 128; cb += 32) {
+                        uint32_t pk[16];
+#pragma unroll
+                        for (int c = 0; c < 32; c += 2) {
+                            const int b = (cb + c) >> 4;
+                            const float ksb = scb[b] * p.scale_log2, vsb = scb[8 + b];
+                            float x0, x1;
+                            if constexpr (kMasked) {
+                                // a masked score is -inf and its block's scale may be 0: keep it -inf, not NaN
+                                const float s0 = __uint_as_float(sr[cb + c]), s1 = __uint_as_float(sr[cb + c + 1]);
+                                x0 = (s0 == -CUDART_INF_F) ? -CUDART_INF_F : fmaf(s0, ksb, neg_m);
+                                x1 = (s1 == -CUDART_INF_F) ? -CUDART_INF_F : fmaf(s1, ksb, neg_m);
+                            } else {
+                                const uint64_t x2 = ptx::fma_f32x2(
+                                    ptx::pack_f32x2(__uint_as_float(sr[cb + c]), __uint_as_float(sr[cb + c + 1])),
+                                    ptx::pack_f32x2(ksb, ksb), nm2);
+                                ptx::unpack_f32x2(x2, x0, x1);
+                            }
+                            const float p0 = ptx::ex2(x0), p1 = ptx::ex2(x1);
+                            if (c & 2) acc_b = ptx::add_f32x2(acc_b, ptx::pack_f32x2(p0, p1));
+                            else acc_a = ptx::add_f32x2(acc_a, ptx::pack_f32x2(p0, p1));
+                            pk[c >> 1] = ptx::pack_f16x2(p0 * vsb, p1 * vsb);
+                        }
+                        ptx::tmem_st_32x32b_x16(pa + (cb >> 1), pk);
+                    }
+                    float a0, a1;
+                    ptx::unpack_f32x2(ptx::add_f32x2(acc_a, acc_b), a0, a1);
+                    l_sum += a0 + a1;
+                };
+                if constexpr (kFp8) {
+                    if (limit >= kTile) tile_body_q(std::false_type{});
+                    else tile_body_q(std::true_type{});
+                } else {
+                    if (limit >= kTile) tile_body(std::false_type{});
+                    else tile_body(std::true_type{});
+                }
                 ptx::tmem_st_wait();
                 ptx::tc_fence_before();
                 ptx::mbar_arrive(ptx::smem_u32(&p_ready[w]));
                 have = true;
             }
+            if constexpr (kFp8) ktile_base += n_tiles;
             // ---- epilogue
             ptx::mbar_wait(ptx::smem_u32(&o_done[w]), oph);
             oph ^= 1;
@@ -1048,6 +1324,29 @@ int encode_pool_map(CUtensorMap *tm, void *pool, const prepos_model_shape &s, in
     return PREPOS_OK;
 }
 
+// e4m3 pool [layer][n_pages][Hkv][page][d] bytes: a box is one (page, kv head) slab, [page tokens][d = 128 bytes],
+// 128-byte swizzle (16-byte chunk c of token row r lands at chunk c ^ (r % 8))
+int encode_pool8_map(CUtensorMap *tm, void *pool, const prepos_model_shape &s, int64_t layer_stride_bytes, int64_t n_pages)
+{
+    EncodeTiledFn encode = reinterpret_cast<EncodeTiledFn>(prepos_get_encode_tiled());
+    if (!encode) return PREPOS_E_CUDA;
+    const int D = s.head_dim;
+    const cuuint64_t dims[3] = {static_cast<cuuint64_t>(D), static_cast<cuuint64_t>(n_pages) * s.n_kv_heads * s.page_size,
+                                static_cast<cuuint64_t>(s.layers)};
+    const cuuint64_t lstride = (s.layers > 1) ? static_cast<cuuint64_t>(layer_stride_bytes) : dims[0] * dims[1];
+    const cuuint64_t strides[2] = {static_cast<cuuint64_t>(D), lstride};
+    const cuuint32_t box[3] = {static_cast<cuuint32_t>(D), static_cast<cuuint32_t>(s.page_size), 1};
+    const cuuint32_t estr[3] = {1, 1, 1};
+    const CUresult r = encode(tm, CU_TENSOR_MAP_DATA_TYPE_UINT8, 3, pool, dims, strides, box, estr,
+                              CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
+                              CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) {
+        fprintf(stderr, "libprepos: cuTensorMapEncodeTiled(e4m3 pool) failed: %d\n", static_cast<int>(r));
+        return PREPOS_E_CUDA;
+    }
+    return PREPOS_OK;
+}
+
 // K_new / V_new [layer][sum_L][Hkv][d]: a box is 8 consecutive tokens of one kv head, laid out like one 8-row group
 // of a pool tile ([64-column half][8 rows][128 B], 128-byte swizzle); tokens past sum_L read as zero.
 int encode_new_map(CUtensorMap *tm, const void *base, const prepos_model_shape &s, int64_t layer_stride, int64_t sum_rows)
@@ -1098,10 +1397,10 @@ int encode_q_map(CUtensorMap *tm, const void *base, const prepos_model_shape &s,
     return PREPOS_OK;
 }
 
-template <int D>
+template <int D, bool kFp8>
 int issue(prepos_ctx *ctx, cudaStream_t stream, int resume);
 
-template <int D>
+template <int D, bool kFp8>
 int launch(prepos_ctx *ctx, const AttnArgs &a, int tiles_per_lh, cudaStream_t stream)
 {
     UmmaParams p;
@@ -1124,7 +1423,8 @@ int launch(prepos_ctx *ctx, const AttnArgs &a, int tiles_per_lh, cudaStream_t st
     p.nv = two ? 2 : 3;
     if (D == 64) p.nv = 3;
     constexpr int kTileBytes = kTile * D * 2;
-    const size_t smem = static_cast<size_t>(p.q_tiles + kNK + p.nv) * kTileBytes + 20 * 8 + 128 * 8 + 32;
+    // tail: 27 barriers, the (m, l) exchange, TMEM slot + merge info + segment admission (+ kFp8: the scale ring)
+    const size_t smem = static_cast<size_t>(p.q_tiles + kNK + p.nv) * kTileBytes + 27 * 8 + 128 * 8 + 40 + (kFp8 ? 8 * 16 * 4 + 16 : 0);
     // one CTA per SM; never more CTAs than tiles, never more than the partial slots provisioned
     long long grid = ctx->num_sms;
     if (grid > p.total_tiles) grid = p.total_tiles;
@@ -1187,8 +1487,19 @@ int launch(prepos_ctx *ctx, const AttnArgs &a, int tiles_per_lh, cudaStream_t st
             }
         }
     }
-    if (ctx->tm_k_ptr != a.k_pool || ctx->tm_v_ptr != a.v_pool || ctx->tm_layer_stride != a.pool_layer_stride ||
-        ctx->tm_n_pages != a.n_pages) {
+    if (kFp8) {
+        if (ctx->tm_k_ptr != a.k_pool8 || ctx->tm_v_ptr != a.v_pool8 || ctx->tm_layer_stride != a.pool_layer_stride ||
+            ctx->tm_n_pages != a.n_pages) {
+            int st = encode_pool8_map(&ctx->tm_k, a.k_pool8, ctx->shape, a.pool_layer_stride, a.n_pages);
+            if (st == PREPOS_OK) st = encode_pool8_map(&ctx->tm_v, a.v_pool8, ctx->shape, a.pool_layer_stride, a.n_pages);
+            if (st != PREPOS_OK) return st;
+            ctx->tm_k_ptr = a.k_pool8;
+            ctx->tm_v_ptr = a.v_pool8;
+            ctx->tm_layer_stride = a.pool_layer_stride;
+            ctx->tm_n_pages = a.n_pages;
+        }
+    } else if (ctx->tm_k_ptr != a.k_pool || ctx->tm_v_ptr != a.v_pool || ctx->tm_layer_stride != a.pool_layer_stride ||
+               ctx->tm_n_pages != a.n_pages) {
         int st = encode_pool_map(&ctx->tm_k, a.k_pool, ctx->shape, a.pool_layer_stride, a.n_pages);
         if (st == PREPOS_OK) st = encode_pool_map(&ctx->tm_v, a.v_pool, ctx->shape, a.pool_layer_stride, a.n_pages);
         if (st != PREPOS_OK) return st;
@@ -1197,9 +1508,9 @@ int launch(prepos_ctx *ctx, const AttnArgs &a, int tiles_per_lh, cudaStream_t st
         ctx->tm_layer_stride = a.pool_layer_stride;
         ctx->tm_n_pages = a.n_pages;
     }
-    // entry K/V maps: they follow the call's K_new / V_new pointers
-    if (ctx->tm_kn_ptr != a.k_new || ctx->tm_vn_ptr != a.v_new || ctx->tm_new_layer_stride != a.kv_new_layer_stride ||
-        ctx->tm_new_rows != a.sum_rows) {
+    // entry K/V maps: they follow the call's K_new / V_new pointers (the FP8 path reads the entry from the cache)
+    if (!kFp8 && (ctx->tm_kn_ptr != a.k_new || ctx->tm_vn_ptr != a.v_new || ctx->tm_new_layer_stride != a.kv_new_layer_stride ||
+        ctx->tm_new_rows != a.sum_rows)) {
         int st = encode_new_map(&ctx->tm_kn, a.k_new, ctx->shape, a.kv_new_layer_stride, a.sum_rows);
         if (st == PREPOS_OK) st = encode_new_map(&ctx->tm_vn, a.v_new, ctx->shape, a.kv_new_layer_stride, a.sum_rows);
         if (st != PREPOS_OK) return st;
@@ -1253,20 +1564,21 @@ int launch(prepos_ctx *ctx, const AttnArgs &a, int tiles_per_lh, cudaStream_t st
     ctx->pass_merge_grid = static_cast<int>(mg);
     ctx->pass_smem = smem;
     ctx->pass_head_dim = D;
-    return issue<D>(ctx, stream, 0);
+    ctx->pass_fp8 = kFp8;
+    return issue<D, kFp8>(ctx, stream, 0);
 }
 
 // one launch of the saved pass (fresh or resumed) + the merge launch behind it
-template <int D>
+template <int D, bool kFp8>
 int issue(prepos_ctx *ctx, cudaStream_t stream, int resume)
 {
     UmmaParams p;
     memcpy(&p, ctx->pass_params.data(), sizeof(UmmaParams));
     p.resume = resume;
     p.launch_seq = ++ctx->attn_launch_seq;
-    PREPOS_CUDA_TRY(cudaFuncSetAttribute(attn_umma_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+    PREPOS_CUDA_TRY(cudaFuncSetAttribute(attn_umma_kernel<D, kFp8>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                          static_cast<int>(ctx->pass_smem)));
-    PREPOS_CUDA_TRY(prepos_launch_pdl(attn_umma_kernel<D>, dim3(static_cast<unsigned>(ctx->pass_grid)), dim3(kThreads),
+    PREPOS_CUDA_TRY(prepos_launch_pdl(attn_umma_kernel<D, kFp8>, dim3(static_cast<unsigned>(ctx->pass_grid)), dim3(kThreads),
                                       ctx->pass_smem, stream, ctx->tm_k, ctx->tm_v, ctx->tm_kn, ctx->tm_vn, ctx->tm_q, p));
     ctx->launches += 1;
     if (ctx->pass_merge_grid > 0) {
@@ -1291,13 +1603,28 @@ bool prepos_attn_umma_supported(const prepos_ctx *ctx)
 int prepos_resume_attn_umma(prepos_ctx *ctx, cudaStream_t stream)
 {
     if (ctx->pass_params.size() != sizeof(UmmaParams)) return PREPOS_E_INVALID_ARG;
-    if (ctx->pass_head_dim == 128) return issue<128>(ctx, stream, 1);
-    return issue<64>(ctx, stream, 1);
+    if (ctx->pass_fp8) return issue<128, true>(ctx, stream, 1);
+    if (ctx->pass_head_dim == 128) return issue<128, false>(ctx, stream, 1);
+    return issue<64, false>(ctx, stream, 1);
 }
 
 int prepos_launch_attn_umma(prepos_ctx *ctx, const AttnArgs &a, int tiles_per_lh, cudaStream_t stream)
 {
     if (!prepos_attn_umma_supported(ctx)) return PREPOS_E_SHAPE;
-    if (ctx->shape.head_dim == 128) return launch<128>(ctx, a, tiles_per_lh, stream);
-    return launch<64>(ctx, a, tiles_per_lh, stream);
+    if (ctx->shape.head_dim == 128) return launch<128, false>(ctx, a, tiles_per_lh, stream);
+    return launch<64, false>(ctx, a, tiles_per_lh, stream);
+}
+
+// the tcgen05 kernel over an e4m3 KV cache: d = 128, pages of 16..128 tokens (one scale per 16-column block or more)
+bool prepos_attn_umma_fp8_supported(const prepos_ctx *ctx)
+{
+    const prepos_model_shape &s = ctx->shape;
+    const int G = s.n_q_heads / s.n_kv_heads;
+    return s.head_dim == 128 && s.page_size >= 16 && s.page_size <= kTile && (G & (G - 1)) == 0;
+}
+
+int prepos_launch_attn_umma_fp8(prepos_ctx *ctx, const AttnArgs &a, int tiles_per_lh, cudaStream_t stream)
+{
+    if (!prepos_attn_umma_fp8_supported(ctx)) return PREPOS_E_SHAPE;
+    return launch<128, true>(ctx, a, tiles_per_lh, stream);
 }

@@ -112,6 +112,7 @@ struct prepos_ctx {
     bool pass_open;                  // the last attention call was a tcgen05 launch that can be resumed
     std::vector<unsigned char> pass_params;   // its kernel parameters
     int pass_grid, pass_merge_grid, pass_head_dim;
+    bool pass_fp8;
     size_t pass_smem;
     // host-side plan cache
     std::vector<AttnUnit> plan_units;
@@ -169,8 +170,10 @@ struct AttnArgs {
     const float *k_scale, *v_scale;
     int64_t scale_layer_stride;
 };
-int prepos_launch_attn_fp8(prepos_ctx *ctx, const AttnArgs &a, cudaStream_t stream);
+int prepos_launch_attn_fp8(prepos_ctx *ctx, const AttnArgs &a, bool use_umma, int total_tiles_per_lh, cudaStream_t stream);
 int prepos_launch_attn_generic(prepos_ctx *ctx, const AttnArgs &a, cudaStream_t stream);
 int prepos_launch_attn_umma(prepos_ctx *ctx, const AttnArgs &a, int total_tiles_per_lh, cudaStream_t stream);
 int prepos_resume_attn_umma(prepos_ctx *ctx, cudaStream_t stream);
+bool prepos_attn_umma_fp8_supported(const prepos_ctx *ctx);
+int prepos_launch_attn_umma_fp8(prepos_ctx *ctx, const AttnArgs &a, int total_tiles_per_lh, cudaStream_t stream);
 bool prepos_attn_umma_supported(const prepos_ctx *ctx);

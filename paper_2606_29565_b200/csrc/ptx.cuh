@@ -332,6 +332,27 @@ __device__ __forceinline__ float ex2(float x)
     return y;
 }
 
+// two e4m3 codes (low 16 bits of x) -> two fp16 values, exactly
+__device__ __forceinline__ uint32_t e4m3x2_to_f16x2(uint32_t x)
+{
+    uint32_t r;
+    asm("{\n.reg .b16 t;\ncvt.u16.u32 t, %1;\ncvt.rn.f16x2.e4m3x2 %0, t;\n}" : "=r"(r) : "r"(x));
+    return r;
+}
+// two bf16 values -> two fp16 values (round to nearest; exact inside fp16's normal range)
+__device__ __forceinline__ uint32_t bf16x2_to_f16x2(uint32_t x)
+{
+    uint32_t r;
+    asm("cvt.rn.f16x2.f32 %0, %1, %2;" : "=r"(r) : "f"(__uint_as_float(x & 0xffff0000u)), "f"(__uint_as_float(x << 16)));
+    return r;
+}
+__device__ __forceinline__ uint32_t pack_f16x2(float lo, float hi)
+{
+    uint32_t r;
+    asm("cvt.rn.f16x2.f32 %0, %1, %2;" : "=r"(r) : "f"(hi), "f"(lo));
+    return r;
+}
+
 // packed fp32 pairs (sm_100: FFMA2 / FADD2 issue two lanes per instruction slot)
 __device__ __forceinline__ uint64_t pack_f32x2(float lo, float hi)
 {
