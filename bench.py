@@ -836,6 +836,43 @@ def run_ready_dist_w4(wl, prepos, reps=30):
             "bf16_call_algorithmic_bytes": s.V * s.H * 2 + n * s.H * 2 + n * 48}
 
 
+def run_attn_fp8(wl, prepos, reps=12):
+    """prepos_entry_attn_fp8 -- the same pass over an e4m3 KV cache (reading Q20: one
+    fp32 scale per (layer, page, kv head)), all layers in one launch, on the workload's sessions quantised in place of
+    their bf16 pools.  Algorithmic bytes: every cached code once (half the bf16 bytes) + the page scales + Q / O +
+    the entry K/V read and their codes written."""
+    s, spec = wl.spec["shape"], wl.spec
+    chunk = max(64, (1 << 28) // (s.layers * s.Hkv * s.page * s.d))   # <= 1 GiB of fp32 per quantiser chunk
+    sets = [synth.quantise_sessions_fp8(st["sb"], chunk_pages=chunk) for st in wl.sets[:2]]
+    ctx = prepos.Context(s.layers, s.Hq, s.Hkv, s.d, s.H, s.V, s.page, max_sessions=wl.n)
+    ev = []
+    for i in range(reps + 3):
+        fb, st = sets[i % len(sets)], wl.sets[i % len(sets)]
+        sb = fb.base
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        ctx.entry_attn_fp8(sb.q, sb.k_new, sb.v_new, fb.k_pool8, fb.v_pool8, fb.k_scale, fb.v_scale, sb.page_table,
+                           wl.n_s_h, wl.l_h, wl.cap_h, st["out"])
+        b.record()
+        ev.append((a, b))
+    torch.cuda.synchronize()
+    ms = sorted(a.elapsed_time(b) for a, b in ev[3:])
+    ctx.close()
+    sum_l, sum_n = sum(spec["l_entry"]), sum(spec["n_s"])
+    n_pages_used = sum(-(-(a + b) // s.page) for a, b in zip(spec["n_s"], spec["l_entry"]))
+    nbytes = (sum_n * s.layers * s.Hkv * s.d * 2                    # K and V codes, one byte each
+              + n_pages_used * s.layers * s.Hkv * 4 * 2             # page scales
+              + sum_l * s.layers * s.Hq * s.d * 2 * 2               # Q read, O written
+              + sum_l * s.layers * s.Hkv * s.d * 2 * (2 + 1 + 1))   # entry K/V read (bf16), codes written and read back
+    med = statistics.median(ms)
+    fl = attention_flops(spec)
+    return {"ms_median": round(med, 5), "ms_min": round(ms[0], 5), "algorithmic_bytes": nbytes,
+            "achieved_gbs": round(nbytes / (med * 1e-3) / 1e9, 1),
+            "frac_of_measured_hbm": round(nbytes / (med * 1e-3) / 1e9 / peaks()["hbm"], 4),
+            "tflops": round(fl / (med * 1e-3) / 1e12, 1),
+            "bf16_call_algorithmic_bytes": algorithmic_bytes(spec)["entry_attn"]}
+
+
 def run_yield(wl, prepos, trials=40):
     """SURVEY.md 8(f) NEXT-2, the request that needs whole SMs ("yields immediately"; Eq. 5 / Eq. 7): the
     fall-through decode step of one session (L = 1, all layers, its own ctx) issued on a high-priority stream while the
@@ -1161,6 +1198,8 @@ def run_config(name, args, d, dev, prepos):
             line["scan_logits"] = run_scan_logits(wl, prepos)
         if name in ("c2", "c4", "c5"):
             line["ready_dist_w4"] = run_ready_dist_w4(wl, prepos)
+        if name in ("c2", "c3", "c5"):
+            line["entry_attn_fp8"] = run_attn_fp8(wl, prepos)
         if name == "c3":
             line["update_trace"] = run_update_trace(wl, prepos)
     del wl

@@ -978,11 +978,14 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
                     ptx::unpack_f32x2(ptx::add_f32x2(acc_a, acc_b), a0, a1);
                     l_sum += a0 + a1;
                 };
+                // the choice must be warp-uniform (the bodies hold warp-collective TMEM accesses and votes), and the
+                // causal limit is per row: a tile is "fully visible" only if it is so for all 32 rows of the warp
+                const bool all_visible = __all_sync(0xffffffffu, limit >= kTile);
                 if constexpr (kFp8) {
-                    if (limit >= kTile) tile_body_q(std::false_type{});
+                    if (all_visible) tile_body_q(std::false_type{});
                     else tile_body_q(std::true_type{});
                 } else {
-                    if (limit >= kTile) tile_body(std::false_type{});
+                    if (all_visible) tile_body(std::false_type{});
                     else tile_body(std::true_type{});
                 }
                 ptx::tmem_st_wait();

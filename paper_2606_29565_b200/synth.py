@@ -145,13 +145,20 @@ class SessionBatchFP8:
 
 def make_sessions_fp8(shape: Shape, n_s, l_entry, seed: int, device="cpu", layers: Optional[int] = None,
                       extra_pages: int = 0, tight_capacity=None, chunk_pages: int = 4096) -> SessionBatchFP8:
-    """The sessions of `make_sessions` (same seed, same draws) with the KV cache as an FP8 quantiser would leave it:
-    per (layer, page, kv head) scale = fp32(max|x| over the page slab) / 448 (pages that hold nothing yet get the
-    scale of an N(0,1) slab, 4 / 448), code = e4m3(x / scale) through the library's e4m3 (round to nearest even).
-    Input preparation only: both the oracle and the kernels start from these codes and scales; the codes of the entry
-    tokens are each side's own work (Append(E))."""
+    """The sessions of `make_sessions` (same seed, same draws) with the KV cache quantised by `quantise_sessions_fp8`."""
     sb = make_sessions(shape, n_s, l_entry, seed, device, layers=layers, extra_pages=extra_pages,
                        tight_capacity=tight_capacity)
+    return quantise_sessions_fp8(sb, chunk_pages)
+
+
+def quantise_sessions_fp8(sb: SessionBatch, chunk_pages: int = 4096) -> SessionBatchFP8:
+    """The KV cache of `sb` as an FP8 quantiser would leave it (reading Q20): per (layer, page, kv head)
+    scale = fp32(max|x| over the cached tokens of the page slab) / 448 (pages that hold nothing yet get the scale of
+    an N(0,1) slab, 4 / 448), code = e4m3(x / scale) through the library's e4m3 (round to nearest even).
+    Input preparation only: both the oracle and the kernels start from these codes and scales; the codes of the entry
+    tokens are each side's own work (Append(E))."""
+    shape = sb.shape
+    device = sb.k_pool.device
     page = shape.page
     n_pages = sb.k_pool.shape[1]
     # cached tokens per physical page (slots beyond n_s hold nothing yet)

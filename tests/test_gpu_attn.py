@@ -517,12 +517,22 @@ def test_random_geometries_vs_oracle(prepos, oracle, path):
 
 
 # ---------------------------------------------------------------- NEXT-2: yield and resume
+def _many_small(n, seed, lo=40, hi=420, l_lo=3, l_hi=48):
+    rng = np.random.default_rng(seed)
+    return [int(x) for x in rng.integers(lo, hi, n)], [int(x) for x in rng.integers(l_lo, l_hi, n)]
+
+
+SHAPES["d128_g4_l8"] = synth.Shape("m", layers=8, Hq=8, Hkv=2, d=128, H=128, V=64, page=16)
+
+
 @pytest.mark.parametrize("shape_key,n_s,l_entry,slice_n", [
-    ("d128_g4", [700, 15, 300], [24, 96, 64], 1),     # several units per CTA, cut and whole, 96 / 384 / 256 rows
-    ("d128_g4", [2500], [24], 1),                     # one unit per (layer, kv head) spread over many CTAs
-    ("d128_g2_l16", [3000], [200], 2),                # 16 layers: ~7 segments per CTA, two per launch
-    ("d128_g8", [517], [32], 1),
-    ("d64_g2", [333, 64], [8, 40], 1),
+    ("d128_g4_l8",) + _many_small(30, 1) + (1,),          # ~5 short units per CTA (whole and cut): a stop after each
+    ("d128_g4_l8",) + _many_small(30, 2) + (2,),          # two segments per launch
+    ("d128_g2_l16", [3000, 1000, 500], [200, 130, 40], 1),   # 160 long units on 148 CTAs: stream-K cuts; a CTA stops
+                                                             # between the tail of one unit and the head of the next
+                                                             # and the partials wait in the workspace
+    ("d128_g1_l16", [2500, 700, 900], [300, 257, 129], 1),   # two row chunks per session, G = 1
+    ("d64_g1_l8",) + _many_small(12, 3, l_hi=200) + (1,),
 ])
 def test_sliced_pass_yield_and_resume_is_bit_identical(prepos, oracle, shape_key, n_s, l_entry, slice_n):
     """A pass that stops at its yield points and is resumed until nothing is pending must give the result of an

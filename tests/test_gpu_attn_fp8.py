@@ -46,7 +46,12 @@ def _run(prepos, fb, path=0):
     ctx = prepos.Context(shape.layers, shape.Hq, shape.Hkv, shape.d, shape.H, shape.V, shape.page,
                          max_sessions=max(sb.n_sessions, 1))
     if path:
-        ctx.set_attn_path(path)
+        try:
+            ctx.set_attn_path(path)
+        except prepos.PreposError as e:
+            if e.status == prepos.E_SHAPE:
+                pytest.skip("shape not taken by the tcgen05 FP8 path")
+            raise
     k8, v8 = fb.k_pool8.to(dev).clone(), fb.v_pool8.to(dev).clone()
     out = torch.full(sb.q.shape, float("nan"), dtype=torch.bfloat16, device=dev)
     try:
