@@ -374,23 +374,40 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
 #pragma unroll 1
         for (int b = 0; b < kTile / 32; ++b) {
             const int r = b * 32 + lane;
+            const uint32_t r7s = static_cast<uint32_t>(r & 7) << 4;
+            const uint8_t *src = slot + kRawBytes + r * D;
+            uint8_t *dst = slot + (r >> 3) * kGroupStride + (r & 7) * 128;   // row r of half 0; half 1 is 1024 B on
             uint4 raw[D / 16];
 #pragma unroll
-            for (int c = 0; c < D / 16; ++c)
-                raw[c] = *reinterpret_cast<const uint4 *>(slot + kRawBytes + r * D + ((c ^ (r & 7)) << 4));
+            for (int c = 0; c < D / 16; ++c) raw[c] = *reinterpret_cast<const uint4 *>(src + ((c << 4) ^ r7s));
             __syncwarp();
-            const bool live = r < zero_from;
+            if (b * 32 + 32 <= zero_from) {   // warp-uniform: every row of the batch is a valid token
 #pragma unroll
-            for (int c = 0; c < D / 16; ++c) {
-                const uint32_t w[4] = {raw[c].x, raw[c].y, raw[c].z, raw[c].w};
-                uint32_t h[8];
-#pragma unroll
-                for (int i = 0; i < 4; ++i) {
-                    h[2 * i] = live ? ptx::e4m3x2_to_f16x2(w[i] & 0xffffu) : 0u;
-                    h[2 * i + 1] = live ? ptx::e4m3x2_to_f16x2(w[i] >> 16) : 0u;
+                for (int c = 0; c < D / 16; ++c) {
+                    uint4 lo, hi;
+                    ptx::e4m3x4_to_f16x4(raw[c].x, lo.x, lo.y);
+                    ptx::e4m3x4_to_f16x4(raw[c].y, lo.z, lo.w);
+                    ptx::e4m3x4_to_f16x4(raw[c].z, hi.x, hi.y);
+                    ptx::e4m3x4_to_f16x4(raw[c].w, hi.z, hi.w);
+                    uint8_t *d = dst + (c >> 2) * 1024;
+                    *reinterpret_cast<uint4 *>(d + ((((2 * c) & 7) << 4) ^ r7s)) = lo;
+                    *reinterpret_cast<uint4 *>(d + ((((2 * c + 1) & 7) << 4) ^ r7s)) = hi;
                 }
-                *reinterpret_cast<uint4 *>(slot + tile_offset<D>(r, 2 * c)) = make_uint4(h[0], h[1], h[2], h[3]);
-                *reinterpret_cast<uint4 *>(slot + tile_offset<D>(r, 2 * c + 1)) = make_uint4(h[4], h[5], h[6], h[7]);
+            } else {
+                const uint32_t keep = (r < zero_from) ? 0xffffffffu : 0u;
+#pragma unroll
+                for (int c = 0; c < D / 16; ++c) {
+                    uint4 lo, hi;
+                    ptx::e4m3x4_to_f16x4(raw[c].x, lo.x, lo.y);
+                    ptx::e4m3x4_to_f16x4(raw[c].y, lo.z, lo.w);
+                    ptx::e4m3x4_to_f16x4(raw[c].z, hi.x, hi.y);
+                    ptx::e4m3x4_to_f16x4(raw[c].w, hi.z, hi.w);
+                    lo.x &= keep, lo.y &= keep, lo.z &= keep, lo.w &= keep;
+                    hi.x &= keep, hi.y &= keep, hi.z &= keep, hi.w &= keep;
+                    uint8_t *d = dst + (c >> 2) * 1024;
+                    *reinterpret_cast<uint4 *>(d + ((((2 * c) & 7) << 4) ^ r7s)) = lo;
+                    *reinterpret_cast<uint4 *>(d + ((((2 * c + 1) & 7) << 4) ^ r7s)) = hi;
+                }
             }
             __syncwarp();
         }
@@ -401,58 +418,24 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
     // register budget: launch gives kLaunchRegs x 384 threads.  The four service warps (warpgroup 0) hand theirs
     // down to kServiceRegs; each softmax thread, which holds a 128-wide score row, grows to kSoftmaxRegs.
     if (warp < 4) {
-    ptx::setmaxnreg_dec<kServiceRegs>();
+    // (setmaxnreg is a warpgroup-wide instruction: the four service warps take the same count.)  kFp8: the widening
+    // warps hold a 128-byte token row per lane: 80 registers for the service warps, 200 for the softmax warps
+    ptx::setmaxnreg_dec<kFp8 ? 80 : kServiceRegs>();
     if (kFp8 && warp == 3) {
-        // ===================== kFp8: V loads and V widening =====================
-        // Loads run nv - 1 tiles ahead of the widening: tile c is widened, then tile c + nv - 1 is requested into the
-        // slot tile c - 1 leaves (free once its PV has retired).
-        if constexpr (kFp8) {
-            const uint64_t pol = ptx::policy_evict_first();
-            SegIter it_i(p, t0, t1), it_c(p, t0, t1);
-            Seg si, sc;
-            int seg_i = 0, kp_i = 0, seg_c = 0, kp_c = 0;
-            bool more_i = next_seg(it_i, si, seg_i, kp_i), more_c = next_seg(it_c, sc, seg_c, kp_c);
-            int ti = more_i ? si.tb : 0, tc = more_c ? sc.tb : 0;
-            int islot = 0, cslot = 0;
-            uint32_t iph = 0, cph = 0;
-            auto issue_one = [&]() {
-                const int n_pages_valid = (si.u.n_load + p.page - 1) >> p.page_shift;
-                const int32_t *pt = p.a.page_table + static_cast<size_t>(si.u.session) * p.a.page_table_stride;
-                const int idx = ti * pages_per_tile + lane;
-                const int pg = (lane < pages_per_tile && idx < n_pages_valid) ? __ldg(pt + idx) : -1;
-                if (lane == 0) ptx::mbar_wait(ptx::smem_u32(&v_empty[islot]), iph ^ 1);
-                __syncwarp();
-                int nvp = n_pages_valid - ti * pages_per_tile;
-                nvp = nvp < pages_per_tile ? nvp : pages_per_tile;
-                const uint32_t fb = ptx::smem_u32(&v_full[islot]);
-                if (lane == 0) ptx::mbar_arrive_expect_tx(fb, nvp * p.page * D);
-                __syncwarp();
-                if (pg >= 0)
-                    ptx::tma_load_3d(ptx::smem_u32(v_s + islot * kTileBytes + kRawBytes + lane * p.page * D), &tm_v, fb, 0,
-                                     (pg * p.Hkv + si.kvh) * p.page, si.layer, pol);
-                if (++islot == p.nv) {
-                    islot = 0;
-                    iph ^= 1;
-                }
-                if (++ti == si.te) {
-                    more_i = next_seg(it_i, si, seg_i, kp_i);
-                    ti = more_i ? si.tb : 0;
-                }
-            };
-            for (int k = 0; k < p.nv - 1 && more_i; ++k) issue_one();
-            while (more_c) {
+        // ===================== kFp8: V widening (the V slabs are requested by warp 0, right behind the K slabs) ====
+        SegIter it(p, t0, t1);
+        Seg s;
+        int seg = 0, kproc = 0, cslot = 0;
+        uint32_t cph = 0;
+        while (next_seg(it, s, seg, kproc)) {
+            for (int t = s.tb; t < s.te; ++t) {
                 ptx::mbar_wait(ptx::smem_u32(&v_full[cslot]), cph);
-                widen_tile(v_s + cslot * kTileBytes, sc.u.n_load - tc * kTile);
+                widen_tile(v_s + cslot * kTileBytes, s.u.n_load - t * kTile);
                 if (lane == 0) ptx::mbar_arrive(ptx::smem_u32(&v_conv[cslot]));
                 if (++cslot == p.nv) {
                     cslot = 0;
                     cph ^= 1;
                 }
-                if (++tc == sc.te) {
-                    more_c = next_seg(it_c, sc, seg_c, kp_c);
-                    tc = more_c ? sc.tb : 0;
-                }
-                if (more_i) issue_one();
             }
         }
     } else if (warp == 0 || warp == 3) {
@@ -467,6 +450,8 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
         const uint64_t pol_new = ptx::policy_evict_last();  // entry K/V: just produced, re-read by every row chunk
         int slot = 0;
         uint32_t ph = 0;
+        int vslot8 = 0;       // kFp8: the V ring, filled by this warp too
+        uint32_t vph8 = 0;
         SegIter it(p, t0, t1);
         Seg s;
         int seg = 0, kproc = 0;
@@ -504,7 +489,9 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
                 uint8_t *dst = ring + slot * kTileBytes;
                 const uint32_t fb = ptx::smem_u32(&full[slot]);
                 if constexpr (kFp8) {
-                    // e4m3 page slabs ([page tokens][D bytes], 128-byte swizzle) into the upper half of the slot
+                    // e4m3 page slabs ([page tokens][D bytes], 128-byte swizzle) into the upper half of the slot; the V
+                    // slabs of the same pages follow into the V ring (one warp requests both: a slab is requested as
+                    // soon as its slot is free, never behind the widening of another tile)
                     int nvp = n_pages_valid - t * pages_per_tile;
                     nvp = nvp < pages_per_tile ? nvp : pages_per_tile;
                     if (lane == 0) ptx::mbar_arrive_expect_tx(fb, nvp * p.page * D);
@@ -512,6 +499,18 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
                     if (pg >= 0)
                         ptx::tma_load_3d(ptx::smem_u32(dst + kRawBytes + lane * p.page * D), tm, fb, 0,
                                          (pg * p.Hkv + s.kvh) * p.page, s.layer, pol);
+                    if (lane == 0) ptx::mbar_wait(ptx::smem_u32(&v_empty[vslot8]), vph8 ^ 1);
+                    __syncwarp();
+                    const uint32_t vfb = ptx::smem_u32(&v_full[vslot8]);
+                    if (lane == 0) ptx::mbar_arrive_expect_tx(vfb, nvp * p.page * D);
+                    __syncwarp();
+                    if (pg >= 0)
+                        ptx::tma_load_3d(ptx::smem_u32(v_s + vslot8 * kTileBytes + kRawBytes + lane * p.page * D), &tm_v, vfb,
+                                         0, (pg * p.Hkv + s.kvh) * p.page, s.layer, pol);
+                    if (++vslot8 == p.nv) {
+                        vslot8 = 0;
+                        vph8 ^= 1;
+                    }
                 } else if (t < s.u.n_cached_tiles) {
                     int nvp = n_pages_valid - t * pages_per_tile;
                     nvp = nvp < pages_per_tile ? nvp : pages_per_tile;
@@ -743,7 +742,7 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
         }
     }
     } else {
-        ptx::setmaxnreg_inc<kSoftmaxRegs>();
+        ptx::setmaxnreg_inc<kFp8 ? 200 : kSoftmaxRegs>();
         // ===================== softmax warpgroups (warps 4-7: stream 0, warps 8-11: stream 1) =====================
         const int w = (warp - 4) >> 2;
         const int row = ((warp & 3) << 5) | lane;              // TMEM lane == row within the M-tile

@@ -339,6 +339,13 @@ __device__ __forceinline__ uint32_t e4m3x2_to_f16x2(uint32_t x)
     asm("{\n.reg .b16 t;\ncvt.u16.u32 t, %1;\ncvt.rn.f16x2.e4m3x2 %0, t;\n}" : "=r"(r) : "r"(x));
     return r;
 }
+// four e4m3 codes (one word) -> four fp16 values in two registers, exactly
+__device__ __forceinline__ void e4m3x4_to_f16x4(uint32_t x, uint32_t &lo, uint32_t &hi)
+{
+    asm("{\n.reg .b16 a, b;\nmov.b32 {a, b}, %2;\ncvt.rn.f16x2.e4m3x2 %0, a;\ncvt.rn.f16x2.e4m3x2 %1, b;\n}"
+        : "=r"(lo), "=r"(hi)
+        : "r"(x));
+}
 // two bf16 values -> two fp16 values (round to nearest; exact inside fp16's normal range)
 __device__ __forceinline__ uint32_t bf16x2_to_f16x2(uint32_t x)
 {

@@ -402,16 +402,17 @@ constexpr int kW4StageBytes = kW4BoxesPerStage * kW4BoxBytes;  // 32 KB
 constexpr int kW4Group = 128;
 constexpr int kW4XPad = 32;  // bf16 elements: the row stride of the hidden block is 64 B mod 128 B (bank spread)
 
-// eight int4 codes (one 32-bit word) -> four bf16x2 registers holding codes (i, i + 4), exactly
+// eight int4 codes (one 32-bit word) -> four bf16x2 registers holding (136 + code_i, 136 + code_{i+4}), exactly:
+// ((w >> 4i) & 0x000f000f) ^ 0x43084308 flips the sign bit of each nibble (code + 8 in 0..15) and sets the bf16
+// exponent of 128 around it -- one shift and one LOP3 per register.  The offset 136 is taken out of the group sum
+// afterwards (sum_k (136 + c_k) x_k = sum_k c_k x_k + 136 sum_k x_k), which costs four FMAs per 128 k instead of a
+// packed subtraction per register: the widening, not the stream, is what the issue slots are spent on.
 __device__ __forceinline__ void w4_widen(uint32_t w, uint32_t (&r)[4])
 {
-    const uint32_t x = w ^ 0x88888888u;           // code + 8 in 0..15
 #pragma unroll
-    for (int i = 0; i < 4; ++i) {
-        const uint32_t b = ((x >> (4 * i)) & 0x000f000fu) | 0x43004300u;   // bf16(128 + code + 8) in both halves
-        asm("sub.rn.bf16x2 %0, %1, %2;" : "=r"(r[i]) : "r"(b), "r"(0x43084308u));  // - 136: exact
-    }
+    for (int i = 0; i < 4; ++i) r[i] = ((w >> (4 * i)) & 0x000f000fu) ^ 0x43084308u;
 }
+constexpr float kW4Offset = 136.f;
 
 __global__ void __launch_bounds__(kThreads, 1)
 ready_dist_w4_kernel(const __grid_constant__ CUtensorMap tm_w4, const RdParams p, const __nv_bfloat16 *__restrict__ w_scale)
@@ -426,6 +427,7 @@ ready_dist_w4_kernel(const __grid_constant__ CUtensorMap tm_w4, const RdParams p
     uint64_t *full_bar = bars;
     uint64_t *empty_bar = bars + kMaxStages;
     RdPartial *warp_part = reinterpret_cast<RdPartial *>(bars + 2 * kMaxStages);  // [kConsumerWarps][kNB]
+    float *xsum = reinterpret_cast<float *>(warp_part + kConsumerWarps * kNB);    // [n_groups][kNB]: sum of x over a group
     const int warp = threadIdx.x >> 5;
     const int lane = threadIdx.x & 31;
     const int n_tiles = (p.V + kTileRows - 1) / kTileRows;
@@ -489,6 +491,22 @@ ready_dist_w4_kernel(const __grid_constant__ CUtensorMap tm_w4, const RdParams p
             }
         }
         ptx::bar_sync(1, kConsumerWarps * 32);
+        // per (group, hidden row) sums of x, in fp32 from the bf16 values the MMA multiplies (for the offset above)
+        for (int idx = threadIdx.x; idx < n_groups * kNB; idx += kConsumerWarps * 32) {
+            const int grp = idx / kNB, r = idx - grp * kNB;
+            float acc = 0.f;
+            if (r < p.n) {   // from the block just written (the order inside a group does not matter for a sum)
+                const uint4 *xr = reinterpret_cast<const uint4 *>(xs + static_cast<size_t>(r) * x_stride + grp * kW4Group);
+                for (int k = 0; k < kW4Group / 8; ++k) {
+                    const uint4 u = xr[k];
+                    const uint32_t w[4] = {u.x, u.y, u.z, u.w};
+#pragma unroll
+                    for (int i = 0; i < 4; ++i) acc += __uint_as_float(w[i] << 16) + __uint_as_float(w[i] & 0xffff0000u);
+                }
+            }
+            xsum[idx] = acc;
+        }
+        ptx::bar_sync(1, kConsumerWarps * 32);
         Top2Lse st[2];
         st[0] = t2_init();
         st[1] = t2_init();
@@ -510,10 +528,20 @@ ready_dist_w4_kernel(const __grid_constant__ CUtensorMap tm_w4, const RdParams p
                 const int nb = (n_groups - g0 < kW4BoxesPerStage) ? n_groups - g0 : kW4BoxesPerStage;
                 // the stage's group scales of this lane's two rows: issued before the wait for the codes
                 float sa[kW4BoxesPerStage], sb[kW4BoxesPerStage];
+                if (nb == kW4BoxesPerStage && (n_groups & 3) == 0 && (reinterpret_cast<uintptr_t>(w_scale) & 7) == 0) {
+                    // four consecutive bf16 scales of a row: one 8-byte load (rows are n_groups * 2 bytes apart)
+                    const uint2 ua = (v < p.V) ? __ldg(reinterpret_cast<const uint2 *>(sc_a + g0)) : make_uint2(0, 0);
+                    const uint2 ub = (v + 8 < p.V) ? __ldg(reinterpret_cast<const uint2 *>(sc_b + g0)) : make_uint2(0, 0);
+                    sa[0] = __uint_as_float(ua.x << 16), sa[1] = __uint_as_float(ua.x & 0xffff0000u);
+                    sa[2] = __uint_as_float(ua.y << 16), sa[3] = __uint_as_float(ua.y & 0xffff0000u);
+                    sb[0] = __uint_as_float(ub.x << 16), sb[1] = __uint_as_float(ub.x & 0xffff0000u);
+                    sb[2] = __uint_as_float(ub.y << 16), sb[3] = __uint_as_float(ub.y & 0xffff0000u);
+                } else {
 #pragma unroll
-                for (int b = 0; b < kW4BoxesPerStage; ++b) {
-                    sa[b] = (b < nb && v < p.V) ? __bfloat162float(sc_a[g0 + b]) : 0.f;
-                    sb[b] = (b < nb && v + 8 < p.V) ? __bfloat162float(sc_b[g0 + b]) : 0.f;
+                    for (int b = 0; b < kW4BoxesPerStage; ++b) {
+                        sa[b] = (b < nb && v < p.V) ? __bfloat162float(sc_a[g0 + b]) : 0.f;
+                        sb[b] = (b < nb && v + 8 < p.V) ? __bfloat162float(sc_b[g0 + b]) : 0.f;
+                    }
                 }
                 ptx::mbar_wait(ptx::smem_u32(&full_bar[stage]), phase);
                 const uint8_t *sbase = stage_base + static_cast<size_t>(stage) * kW4StageBytes;
@@ -534,10 +562,12 @@ ready_dist_w4_kernel(const __grid_constant__ CUtensorMap tm_w4, const RdParams p
                             ptx::mma_bf16_16816(acc, ra[0], rb[0], ra[1], rb[1], xb.x, xb.y);
                             ptx::mma_bf16_16816(acc, ra[2], rb[2], ra[3], rb[3], xb.z, xb.w);
                         }
-                        tot[0] = fmaf(sa[b], acc[0], tot[0]);
-                        tot[1] = fmaf(sa[b], acc[1], tot[1]);
-                        tot[2] = fmaf(sb[b], acc[2], tot[2]);
-                        tot[3] = fmaf(sb[b], acc[3], tot[3]);
+                        const float2 xs2 = *reinterpret_cast<const float2 *>(xsum + (g0 + b) * kNB + n0);
+                        const float o0 = kW4Offset * xs2.x, o1 = kW4Offset * xs2.y;
+                        tot[0] = fmaf(sa[b], acc[0] - o0, tot[0]);
+                        tot[1] = fmaf(sa[b], acc[1] - o1, tot[1]);
+                        tot[2] = fmaf(sb[b], acc[2] - o0, tot[2]);
+                        tot[3] = fmaf(sb[b], acc[3] - o1, tot[3]);
                     }
                 }
                 __syncwarp();
@@ -953,7 +983,8 @@ int prepos_launch_ready_dist_w4(prepos_ctx *ctx, int n, const int32_t *session_i
         p.V = V;
         p.x_rows = (p.n < kNB) ? p.n + 1 : kNB;
         const size_t x_bytes = (static_cast<size_t>(p.x_rows) * (H + kW4XPad) * 2 + 15) & ~size_t(15);
-        const size_t fixed = 1024 + x_bytes + 2 * kMaxStages * 8 + kConsumerWarps * kNB * sizeof(RdPartial);
+        const size_t fixed = 1024 + x_bytes + 2 * kMaxStages * 8 + kConsumerWarps * kNB * sizeof(RdPartial) +
+                             static_cast<size_t>(H / kW4Group) * kNB * sizeof(float);
         int stages = static_cast<int>((232448 - fixed) / kW4StageBytes);
         if (stages > kMaxStages) stages = kMaxStages;
         if (stages < 2) return PREPOS_E_SHAPE;
