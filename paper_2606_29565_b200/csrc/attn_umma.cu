@@ -243,13 +243,20 @@ __device__ __forceinline__ void append_entry(const UmmaParams &p, const Seg &s, 
 }
 
 // kFp8 (reading Q20): the pools hold e4m3 codes with one fp32 scale per (page, kv
-// head).  A tile arrives as 128 x D BYTES (half the HBM traffic) in the upper half of its ring slot and is widened in
-// place to the fp16 tile the MMA reads (e4m3 -> fp16 is exact) by a service warp: warp 2 the K tiles, warp 3 the V
-// tiles (which also issues the V loads).  Q is converted bf16 -> fp16 in place by the softmax warps at the start of a
-// segment, P is written as fp16: both MMAs run as f16 x f16.  The page scales never touch an operand: the K scale of
-// a column's page multiplies its score inside the softmax's scale FMA, the V scale multiplies its probability before
-// P is packed.  The entry tokens were appended (quantised) by fp8_append_kernel before this launch and are read back
-// from the pages like cached ones: a unit has no entry tiles, causality is a per-row column limit.
+// head); a tile arrives as 128 x D BYTES (half the HBM traffic), [token][128 B] with the 128-byte swizzle -- which IS
+// the K-major operand layout of an 8-bit MMA.
+//   S = Q K^T runs on the FP8 tensor path (kind::f8f6f4, K = 32 per instruction) straight from the K slab as it
+//     landed: no conversion of K at all, and a K ring of six 16 KB slots.  Q (bf16, 8 significant bits) is split
+//     exactly into two e4m3 operands at the start of a segment by the softmax warps: per row a power-of-two scale
+//     2^k brings max|q| into [128, 256), Qh = q with the mantissa truncated to 3 bits, Ql = q - Qh (both x 2^k);
+//     S = (Qh + Ql) K^T is two accumulating passes, the same tensor time as one bf16 pass.  (Elements more than 2^10
+//     below their row's maximum lose bits of Ql: an absolute error below 2^-17 of that maximum.)
+//   O += P V stays f16 x f16: P is packed as fp16, the V slab lands in the upper half of its 32 KB slot and is widened
+//     in place to the fp16 tile (cvt e4m3 -> f16 is exact) by warps 2 and 3, 64 token rows each.
+//   The page scales never touch an operand: the K scale of a column's page (times 2^-k of the row) multiplies its
+//   score inside the softmax's scale FMA, the V scale multiplies its probability before P is packed.
+//   The entry tokens were appended (quantised) by fp8_append_kernel before this launch and are read back from the
+//   pages like cached ones: a unit has no entry tiles, causality is a per-row column limit.
 template <int D, bool kFp8>
 __global__ void __maxnreg__(kLaunchRegs)
 attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__ CUtensorMap tm_v,
@@ -261,6 +268,9 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
     constexpr int kHalves = D / 64;
     constexpr int kTileBytes = kTile * D * 2;         // one K or V tile / one Q M-tile
     constexpr int kRawBytes = kTile * D;              // an e4m3 tile as it arrives (kFp8)
+    constexpr int kNK8 = 2 * kNK;                     // kFp8: K slabs are used as they land, 16 KB a slot
+    constexpr uint32_t kDescHi8 = desc_hi(1024);      // 8-bit K-major tile: 8 rows x 128 B per group
+    constexpr uint32_t kIdescQK8 = (1u << 4) | ((kTile >> 3) << 17) | ((128u >> 4) << 24);   // e4m3 x e4m3 -> f32
     constexpr int kGroupStride = kHalves * 1024;      // bytes between 8-row groups
     constexpr uint32_t kFmt = kFp8 ? 0u : 1u;         // kind::f16 operand format: 0 = f16, 1 = bf16
     constexpr uint32_t kIdescQK = (1u << 4) | (kFmt << 7) | (kFmt << 10) | ((kTile >> 3) << 17) | ((128u >> 4) << 24);
@@ -279,8 +289,9 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
     uint64_t *k_full = bars, *k_empty = bars + 3, *v_full = bars + 6, *v_empty = bars + 9;
     uint64_t *s_full = bars + 12, *p_ready = bars + 14, *o_done = bars + 16, *q_full = bars + 18;
     uint64_t *q_empty = bars + 19;    // the segment's last QK has read Q: the loader may overwrite it
-    uint64_t *k_conv = bars + 20, *v_conv = bars + 23, *q_conv = bars + 26;   // kFp8: tile / Q widened to fp16
-    float2 *ml_x = reinterpret_cast<float2 *>(bars + 27);  // [128] (m, l) of stream 1 / the row factors back
+    // kFp8: V widened (two warps arrive), Q split, and the six-slot K ring
+    uint64_t *v_conv = bars + 20, *q_conv = bars + 23, *k_full8 = bars + 24, *k_empty8 = bars + 30;
+    float2 *ml_x = reinterpret_cast<float2 *>(bars + 36);  // [128] (m, l) of stream 1 / the row factors back
     uint32_t *tmem_slot = reinterpret_cast<uint32_t *>(ml_x + 128);
     int *merge_info = reinterpret_cast<int *>(tmem_slot + 1);  // [3]: c0 (or -1 = not last), c1, c0's slot
     // segment admission (yield / resume): [0] segments admitted in this launch, [1] the first one refused (or
@@ -288,7 +299,12 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
     // role that reaches a segment first; every other role asks before it starts a segment.
     int *sched = merge_info + 3;
     // kFp8: page scales of the last 8 K tiles, [tile % 8][0..7 K scale of 16-column block b | 8..15 V scale]
-    float *sc_s = reinterpret_cast<float *>((reinterpret_cast<uintptr_t>(sched + 3) + 15) & ~uintptr_t(15));
+    // (36 barriers + the 1 KB exchange + 4 + 12 + 12 bytes = 1340 -> 1344; plain pointer arithmetic on the shared array,
+    // so that the loads stay shared-memory loads)
+    float *sc_s = reinterpret_cast<float *>(tail + 1344);
+    // kFp8: [128] 2^-k of the rows of M-tile 0 (both streams need it when they share the tile).  Lives in the (m, l)
+    // exchange array, which is idle between a segment's epilogue and its successor's first tile.
+    float *rowf_s = reinterpret_cast<float *>(ml_x);
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
 
@@ -306,9 +322,10 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
         }
         ptx::mbar_init(ptx::smem_u32(q_full), 1);
         ptx::mbar_init(ptx::smem_u32(q_empty), 1);
-        for (int i = 0; i < 3; ++i) {
-            ptx::mbar_init(ptx::smem_u32(&k_conv[i]), 1);
-            ptx::mbar_init(ptx::smem_u32(&v_conv[i]), 1);
+        for (int i = 0; i < 3; ++i) ptx::mbar_init(ptx::smem_u32(&v_conv[i]), 2);
+        for (int i = 0; i < 6; ++i) {
+            ptx::mbar_init(ptx::smem_u32(&k_full8[i]), 1);
+            ptx::mbar_init(ptx::smem_u32(&k_empty8[i]), 1);
         }
         ptx::mbar_init(ptx::smem_u32(q_conv), 1);
         ptx::fence_mbar_init();
@@ -366,13 +383,14 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
         }
         return false;
     };
-    // kFp8: widen the e4m3 tile in the upper half of `slot` to the fp16 tile the MMA reads, in place, by one warp.
-    // Lane = token row, four batches of 32 rows in ascending order: the output of a batch (8 KB from byte 8 KB x
-    // batch) only ever covers raw rows of earlier batches or of the batch itself, all of which are in registers by
-    // then.  Rows from `zero_from` on are written as zeros (V: P is 0 there, but 0 x NaN would poison O).
-    auto widen_tile = [&](uint8_t *slot, int zero_from) {
+    // kFp8: widen 64 token rows (two batches of 32: lane = row) of the e4m3 V tile in the upper half of `slot` to the
+    // fp16 tile the MMA reads, in place.  Warp 2 takes rows 0-63, whose output (bytes 0-16 K) touches no raw byte;
+    // warp 3 takes rows 64-127, whose output (bytes 16-32 K) covers the raw rows 0-63 and its own: it loads a batch
+    // into registers first, and before its first store waits (named barrier 2) until warp 2 has loaded its last batch.
+    // Rows from `zero_from` on are written as zeros (P is 0 there, but 0 x NaN would poison O).
+    auto widen_tile = [&](uint8_t *slot, int zero_from, int upper) {
 #pragma unroll 1
-        for (int b = 0; b < kTile / 32; ++b) {
+        for (int b = 2 * upper; b < 2 * upper + 2; ++b) {
             const int r = b * 32 + lane;
             const uint32_t r7s = static_cast<uint32_t>(r & 7) << 4;
             const uint8_t *src = slot + kRawBytes + r * D;
@@ -381,6 +399,9 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
 #pragma unroll
             for (int c = 0; c < D / 16; ++c) raw[c] = *reinterpret_cast<const uint4 *>(src + ((c << 4) ^ r7s));
             __syncwarp();
+            // warp 2 (b == 1): every raw row below 64 is now in registers or already widened; warp 3 (b == 2): so its
+            // output may overwrite them.  (A sync on both sides: one rendezvous per tile, neither warp runs a tile ahead.)
+            if (b == 1 || b == 2) ptx::bar_sync(2, 64);
             if (b * 32 + 32 <= zero_from) {   // warp-uniform: every row of the batch is a valid token
 #pragma unroll
                 for (int c = 0; c < D / 16; ++c) {
@@ -430,13 +451,97 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
         while (next_seg(it, s, seg, kproc)) {
             for (int t = s.tb; t < s.te; ++t) {
                 ptx::mbar_wait(ptx::smem_u32(&v_full[cslot]), cph);
-                widen_tile(v_s + cslot * kTileBytes, s.u.n_load - t * kTile);
+                widen_tile(v_s + cslot * kTileBytes, s.u.n_load - t * kTile, 1);
                 if (lane == 0) ptx::mbar_arrive(ptx::smem_u32(&v_conv[cslot]));
                 if (++cslot == p.nv) {
                     cslot = 0;
                     cph ^= 1;
                 }
             }
+        }
+    } else if (kFp8 && warp == 0) {
+        // ===================== kFp8: K and V slab requests, page scales =====================
+        // One warp requests both streams (a slab is requested as soon as its slot is free, never behind the widening
+        // of another tile): K slabs into the six 16 KB slots of the K ring, V slabs into the upper half of the V
+        // slots.  Lanes 0-7 / 8-15 also fetch the K / V scale of the tile's eight 16-column blocks and put them into
+        // the scale ring BEFORE the arrive on the K barrier, so that whoever sees the K tile sees its scales.
+        if constexpr (kFp8) {
+            const uint64_t pol = ptx::policy_evict_first();
+            int kslot = 0, vslot = 0, seg = 0, kproc = 0, ktile = 0;
+            uint32_t kph = 0, vph = 0;
+            SegIter it(p, t0, t1);
+            Seg s;
+            unsigned int yflag = (lane == 0) ? ptx::ld_volatile_global(p.yield_flag) : 0u;
+            while (it.next(p, s)) {
+                if (seg++ < skip) continue;
+                int stop = 0;
+                if (lane == 0) {
+                    stop = (yflag != 0u) || (p.slice > 0 && kproc >= p.slice);
+                    if (stop) ptx::st_release_cta_smem(&sched[1], kproc);
+                    else ptx::st_release_cta_smem(&sched[0], kproc + 1);
+                }
+                stop = __shfl_sync(0xffffffffu, stop, 0);
+                if (stop) break;
+                ++kproc;
+                const int n_pages_valid = (s.u.n_load + p.page - 1) >> p.page_shift;
+                const int32_t *pt = p.a.page_table + static_cast<size_t>(s.u.session) * p.a.page_table_stride;
+                const float *scl = (lane < 8 ? p.a.k_scale : p.a.v_scale) + static_cast<size_t>(s.layer) * p.a.scale_layer_stride;
+                auto page_of = [&](int t) -> int {   // the page this lane requests of tile t
+                    const int idx = t * pages_per_tile + lane;
+                    return (t < s.te && lane < pages_per_tile && idx < n_pages_valid) ? __ldg(pt + idx) : -1;
+                };
+                auto scale_page_of = [&](int t) -> int {   // the page of this lane's 16-column block of tile t
+                    const int idx = t * pages_per_tile + (((lane & 7) * 16) >> p.page_shift);
+                    return (t < s.te && lane < 16 && idx < n_pages_valid) ? __ldg(pt + idx) : -1;
+                };
+                auto scale_of = [&](int pg) -> float {
+                    return pg >= 0 ? __ldg(scl + static_cast<size_t>(pg) * p.Hkv + s.kvh) : 0.f;
+                };
+                int pg_next = page_of(s.tb);
+                int spg_next = scale_page_of(s.tb + 1);
+                float sc_next = scale_of(scale_page_of(s.tb));
+                for (int t = s.tb; t < s.te; ++t) {
+                    if (lane == 0 && ((t - s.tb) & 7) == 7) yflag = ptx::ld_volatile_global(p.yield_flag);
+                    const int pg = pg_next;
+                    const float sc_now = sc_next;
+                    pg_next = page_of(t + 1);
+                    sc_next = scale_of(spg_next);
+                    spg_next = scale_page_of(t + 2);
+                    int nvp = n_pages_valid - t * pages_per_tile;
+                    nvp = nvp < pages_per_tile ? nvp : pages_per_tile;
+                    const int coord = (pg * p.Hkv + s.kvh) * p.page;
+                    // ---- K
+                    if (lane == 0) ptx::mbar_wait(ptx::smem_u32(&k_empty8[kslot]), kph ^ 1);
+                    __syncwarp();
+                    if (lane < 16) sc_s[(ktile & 7) * 16 + lane] = sc_now;
+                    __syncwarp();
+                    const uint32_t kfb = ptx::smem_u32(&k_full8[kslot]);
+                    if (lane == 0) ptx::mbar_arrive_expect_tx(kfb, nvp * p.page * D);
+                    __syncwarp();
+                    if (pg >= 0)
+                        ptx::tma_load_3d(ptx::smem_u32(k_s + kslot * kRawBytes + lane * p.page * D), &tm_k, kfb, 0, coord,
+                                         s.layer, pol);
+                    ++ktile;
+                    if (++kslot == kNK8) {
+                        kslot = 0;
+                        kph ^= 1;
+                    }
+                    // ---- V
+                    if (lane == 0) ptx::mbar_wait(ptx::smem_u32(&v_empty[vslot]), vph ^ 1);
+                    __syncwarp();
+                    const uint32_t vfb = ptx::smem_u32(&v_full[vslot]);
+                    if (lane == 0) ptx::mbar_arrive_expect_tx(vfb, nvp * p.page * D);
+                    __syncwarp();
+                    if (pg >= 0)
+                        ptx::tma_load_3d(ptx::smem_u32(v_s + vslot * kTileBytes + kRawBytes + lane * p.page * D), &tm_v, vfb, 0,
+                                         coord, s.layer, pol);
+                    if (++vslot == p.nv) {
+                        vslot = 0;
+                        vph ^= 1;
+                    }
+                }
+            }
+            if (lane == 0) sched[2] = skip + kproc;   // read after the CTA-wide barrier at the end
         }
     } else if (warp == 0 || warp == 3) {
         // ===================== K (warp 0) / V (warp 3) TMA producers =====================
@@ -450,8 +555,6 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
         const uint64_t pol_new = ptx::policy_evict_last();  // entry K/V: just produced, re-read by every row chunk
         int slot = 0;
         uint32_t ph = 0;
-        int vslot8 = 0;       // kFp8: the V ring, filled by this warp too
-        uint32_t vph8 = 0;
         SegIter it(p, t0, t1);
         Seg s;
         int seg = 0, kproc = 0;
@@ -488,30 +591,7 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
                 __syncwarp();
                 uint8_t *dst = ring + slot * kTileBytes;
                 const uint32_t fb = ptx::smem_u32(&full[slot]);
-                if constexpr (kFp8) {
-                    // e4m3 page slabs ([page tokens][D bytes], 128-byte swizzle) into the upper half of the slot; the V
-                    // slabs of the same pages follow into the V ring (one warp requests both: a slab is requested as
-                    // soon as its slot is free, never behind the widening of another tile)
-                    int nvp = n_pages_valid - t * pages_per_tile;
-                    nvp = nvp < pages_per_tile ? nvp : pages_per_tile;
-                    if (lane == 0) ptx::mbar_arrive_expect_tx(fb, nvp * p.page * D);
-                    __syncwarp();
-                    if (pg >= 0)
-                        ptx::tma_load_3d(ptx::smem_u32(dst + kRawBytes + lane * p.page * D), tm, fb, 0,
-                                         (pg * p.Hkv + s.kvh) * p.page, s.layer, pol);
-                    if (lane == 0) ptx::mbar_wait(ptx::smem_u32(&v_empty[vslot8]), vph8 ^ 1);
-                    __syncwarp();
-                    const uint32_t vfb = ptx::smem_u32(&v_full[vslot8]);
-                    if (lane == 0) ptx::mbar_arrive_expect_tx(vfb, nvp * p.page * D);
-                    __syncwarp();
-                    if (pg >= 0)
-                        ptx::tma_load_3d(ptx::smem_u32(v_s + vslot8 * kTileBytes + kRawBytes + lane * p.page * D), &tm_v, vfb,
-                                         0, (pg * p.Hkv + s.kvh) * p.page, s.layer, pol);
-                    if (++vslot8 == p.nv) {
-                        vslot8 = 0;
-                        vph8 ^= 1;
-                    }
-                } else if (t < s.u.n_cached_tiles) {
+                if (t < s.u.n_cached_tiles) {
                     int nvp = n_pages_valid - t * pages_per_tile;
                     nvp = nvp < pages_per_tile ? nvp : pages_per_tile;
                     if (lane == 0) ptx::mbar_arrive_expect_tx(fb, nvp * page_bytes);
@@ -552,7 +632,7 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
         Seg s;
         const uint64_t pol_q = ptx::policy_evict_last();  // Q is re-read by every CTA that shares the unit
         int k = 0, seg = 0;
-        int cslot = 0, ktile = 0;   // kFp8: ring slot and running index of the K tile being widened
+        int cslot = 0;   // kFp8: ring slot of the V tile being widened
         uint32_t cph = 0;
         while (it.next(p, s)) {
             if (seg++ < skip) continue;
@@ -583,32 +663,12 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
             }
             ++k;
             if constexpr (kFp8) {
-                // ---- widen the segment's K tiles as they land, and put the page scales of each tile's eight 16-column
-                // blocks (lanes 0-7: K, lanes 8-15: V) where the softmax finds them.  Page ids are read two tiles, the
-                // scales one tile ahead of their use.
-                const int n_pages_valid = (s.u.n_load + p.page - 1) >> p.page_shift;
-                const int32_t *pt = p.a.page_table + static_cast<size_t>(s.u.session) * p.a.page_table_stride;
-                const float *scl = (lane < 8 ? p.a.k_scale : p.a.v_scale) + static_cast<size_t>(s.layer) * p.a.scale_layer_stride;
-                auto page_of = [&](int t) -> int {
-                    const int idx = t * pages_per_tile + (((lane & 7) * 16) >> p.page_shift);
-                    return (lane < 16 && t < s.te && idx < n_pages_valid) ? __ldg(pt + idx) : -1;
-                };
-                auto scale_of = [&](int pg) -> float {
-                    return pg >= 0 ? __ldg(scl + static_cast<size_t>(pg) * p.Hkv + s.kvh) : 0.f;
-                };
-                int pg1 = page_of(s.tb + 1);
-                float sc0 = scale_of(page_of(s.tb));
+                // ---- widen token rows 0-63 of the segment's V tiles as they land (warp 3 takes rows 64-127)
                 for (int t = s.tb; t < s.te; ++t) {
-                    const float sc_now = sc0;
-                    sc0 = scale_of(pg1);
-                    pg1 = page_of(t + 2);
-                    ptx::mbar_wait(ptx::smem_u32(&k_full[cslot]), cph);
-                    widen_tile(k_s + cslot * kTileBytes, kTile);
-                    if (lane < 16) sc_s[(ktile & 7) * 16 + lane] = sc_now;
-                    __syncwarp();
-                    if (lane == 0) ptx::mbar_arrive(ptx::smem_u32(&k_conv[cslot]));
-                    ++ktile;
-                    if (++cslot == kNK) {
+                    ptx::mbar_wait(ptx::smem_u32(&v_full[cslot]), cph);
+                    widen_tile(v_s + cslot * kTileBytes, s.u.n_load - t * kTile, 0);
+                    if (lane == 0) ptx::mbar_arrive(ptx::smem_u32(&v_conv[cslot]));
+                    if (++cslot == p.nv) {
                         cslot = 0;
                         cph ^= 1;
                     }
@@ -646,17 +706,30 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
                 const bool first_use = (n_mt == 1) || w == 0;
                 const bool last_use = (n_mt == 1) || w == 1;
                 if (first_use) {
-                    ptx::mbar_wait(ptx::smem_u32(kFp8 ? &k_conv[kslot] : &k_full[kslot]), kph);
+                    ptx::mbar_wait(ptx::smem_u32(kFp8 ? &k_full8[kslot] : &k_full[kslot]), kph);
                     ptx::tc_fence_after();
                 }
                 // descriptor words are warp-uniform and computed by the whole warp; only the tcgen05 instructions sit
                 // under elect (a lane-0 branch would drag every operand through ELECT + R2UR per MMA)
                 const uint32_t qlo = desc_lo(ptx::smem_u32(q_s + mt * kTileBytes), 16);
-                const uint32_t klo = desc_lo(ptx::smem_u32(k_s + kslot * kTileBytes), 16);
+                const uint32_t klo = desc_lo(ptx::smem_u32(k_s + kslot * (kFp8 ? kRawBytes : kTileBytes)), 16);
                 const uint32_t sd = tmem + kColS + w * 128;
-                const uint32_t sfb = ptx::smem_u32(&s_full[w]), keb = ptx::smem_u32(&k_empty[kslot]);
+                const uint32_t sfb = ptx::smem_u32(&s_full[w]);
+                const uint32_t keb = ptx::smem_u32(kFp8 ? &k_empty8[kslot] : &k_empty[kslot]);
                 const bool q_last = (i == n_items - 1);
                 if (ptx::elect_one()) {
+                    if constexpr (kFp8) {
+                        // S = Qh K^T + Ql K^T on the 8-bit path: Qh in the first, Ql in the second 16 KB of the M-tile's
+                        // buffer, each [row][128 B] like the K slab; 32 elements (32 bytes) per instruction
+#pragma unroll
+                        for (int part = 0; part < 2; ++part)
+#pragma unroll
+                            for (int ks = 0; ks < 4; ++ks) {
+                                const uint32_t off = (ks * 32) >> 4;
+                                ptx::umma_ss2_f8(sd, qlo + ((part * kRawBytes) >> 4) + off, klo + off, kDescHi8, kIdescQK8,
+                                                 (part | ks) != 0);
+                            }
+                    } else {
 #pragma unroll
                     for (int hf = 0; hf < kHalves; ++hf)
 #pragma unroll
@@ -664,13 +737,14 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
                             const uint32_t off = (hf * 1024 + ks * 32) >> 4;
                             ptx::umma_ss2(sd, qlo + off, klo + off, kDescHi, kIdescQK, (hf | ks) != 0);
                         }
+                    }
                     ptx::umma_commit(sfb);
                     if (last_use) ptx::umma_commit(keb);
                     if (q_last) ptx::umma_commit(ptx::smem_u32(q_empty));  // Q may be overwritten
                 }
                 __syncwarp();
                 if (last_use) {
-                    if (++kslot == kNK) {
+                    if (++kslot == (kFp8 ? kNK8 : kNK)) {
                         kslot = 0;
                         kph ^= 1;
                     }
@@ -765,22 +839,69 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
             const int mt = (n_mt == 2) ? w : 0;
             const int urow = mt * 128 + row;                   // row within the unit
             const int my_tok = s.u.tok0 + urow / G;            // entry token of this row (if urow < rows)
+            float srow = p.scale_log2;   // kFp8: softmax scale x log2(e) x 2^-k of this thread's row
             if constexpr (kFp8) {
-                // Q arrived as bf16: widen it to fp16 in place (same size, same swizzled layout; exact for
-                // 2^-14 <= |q| < 65504, below that the fp16 subnormal grid 2^-24), then hand it to the MMA warp
+                // Q arrived as bf16 (8 significant bits): split it exactly into two e4m3 operands, in place.  The thread
+                // owns its query row: 2^k brings the row's max|q| into [128, 256); Qh = q with the mantissa truncated
+                // to 3 bits, Ql = q - Qh (at most 4 significant bits), both x 2^k; 2^-k goes into the softmax scale.
+                // Qh fills the first, Ql the second 16 KB of the M-tile's buffer, [row][128 B] with the 128-byte swizzle.
                 ptx::mbar_wait(ptx::smem_u32(q_full), qph);
                 qph ^= 1;
-                for (int off = st * 16; off < p.q_tiles * kTileBytes; off += 256 * 16) {
-                    uint4 v = *reinterpret_cast<const uint4 *>(q_s + off);
-                    v.x = ptx::bf16x2_to_f16x2(v.x);
-                    v.y = ptx::bf16x2_to_f16x2(v.y);
-                    v.z = ptx::bf16x2_to_f16x2(v.z);
-                    v.w = ptx::bf16x2_to_f16x2(v.w);
-                    *reinterpret_cast<uint4 *>(q_s + off) = v;
+                const bool conv = (n_mt == 2) || (w == 0);
+                uint8_t *qt = q_s + mt * kTileBytes;
+                uint4 qr[D / 8];
+                if (conv) {
+#pragma unroll
+                    for (int c = 0; c < D / 8; ++c) qr[c] = *reinterpret_cast<const uint4 *>(qt + tile_offset<D>(row, c));
+                }
+                ptx::bar_sync(1, 256);   // every row is in registers before the buffer is rewritten
+                float rowf = 1.f;
+                if (conv) {
+                    uint32_t amax_bits = 0u;   // max over |x| as bf16 bit patterns (monotone in the magnitude)
+#pragma unroll
+                    for (int c = 0; c < D / 8; ++c) {
+                        const uint32_t wds[4] = {qr[c].x, qr[c].y, qr[c].z, qr[c].w};
+#pragma unroll
+                        for (int i = 0; i < 4; ++i) {
+                            amax_bits = max(amax_bits, (wds[i] << 16) & 0x7fff0000u);
+                            amax_bits = max(amax_bits, wds[i] & 0x7fff0000u);
+                        }
+                    }
+                    int k = amax_bits ? 7 + 127 - static_cast<int>(amax_bits >> 23) : 0;
+                    k = k < -100 ? -100 : (k > 100 ? 100 : k);
+                    const float up = __int_as_float((k + 127) << 23);
+                    rowf = __int_as_float((127 - k) << 23);
+                    uint8_t *qrow = qt + (row >> 3) * 1024 + (row & 7) * 128;
+                    const uint32_t r7s = static_cast<uint32_t>(row & 7) << 4;
+#pragma unroll
+                    for (int c = 0; c < D / 16; ++c) {   // 16 elements = two bf16 chunks -> one 16-byte chunk of each part
+                        const uint32_t wds[8] = {qr[2 * c].x, qr[2 * c].y, qr[2 * c].z, qr[2 * c].w,
+                                                 qr[2 * c + 1].x, qr[2 * c + 1].y, qr[2 * c + 1].z, qr[2 * c + 1].w};
+                        uint32_t ph[4], pl[4];
+#pragma unroll
+                        for (int i = 0; i < 4; ++i) {
+                            uint32_t hh = 0u, ll = 0u;
+#pragma unroll
+                            for (int j = 0; j < 2; ++j) {
+                                const uint32_t wd = wds[2 * i + j];
+                                const float x0 = __uint_as_float(wd << 16), x1 = __uint_as_float(wd & 0xffff0000u);
+                                const float h0 = __uint_as_float((wd << 16) & 0xfff00000u), h1 = __uint_as_float(wd & 0xfff00000u);
+                                hh |= ptx::pack_e4m3x2(h0 * up, h1 * up) << (16 * j);
+                                ll |= ptx::pack_e4m3x2((x0 - h0) * up, (x1 - h1) * up) << (16 * j);
+                            }
+                            ph[i] = hh;
+                            pl[i] = ll;
+                        }
+                        *reinterpret_cast<uint4 *>(qrow + ((c << 4) ^ r7s)) = make_uint4(ph[0], ph[1], ph[2], ph[3]);
+                        *reinterpret_cast<uint4 *>(qrow + kRawBytes + ((c << 4) ^ r7s)) = make_uint4(pl[0], pl[1], pl[2], pl[3]);
+                    }
+                    if (n_mt == 1) rowf_s[row] = rowf;
                 }
                 ptx::fence_proxy_async_smem();
                 ptx::bar_sync(1, 256);
                 if (st == 0) ptx::mbar_arrive(ptx::smem_u32(q_conv));
+                if (n_mt == 1 && w == 1) rowf = rowf_s[row];
+                srow = p.scale_log2 * rowf;
             }
             float m_used = -CUDART_INF_F, l_sum = 0.f;
             bool have = false;
@@ -896,7 +1017,15 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
                 // block by block) and the V scale on the probabilities before they are packed (fp16)
                 auto tile_body_q = [&](auto masked_tag) {
                     constexpr bool kMasked = decltype(masked_tag)::value;
-                    const float *scb = sc_s + ((ktile_base + (t - s.tb)) & 7) * 16;
+                    float ksv[8], vsv[8];   // the tile's K scales (x softmax scale x 2^-k of the row) and V scales
+                    {
+                        const float4 *scb = reinterpret_cast<const float4 *>(sc_s + ((ktile_base + (t - s.tb)) & 7) * 16);
+                        const float4 a0 = scb[0], a1 = scb[1], b0 = scb[2], b1 = scb[3];
+                        ksv[0] = a0.x * srow, ksv[1] = a0.y * srow, ksv[2] = a0.z * srow, ksv[3] = a0.w * srow;
+                        ksv[4] = a1.x * srow, ksv[5] = a1.y * srow, ksv[6] = a1.z * srow, ksv[7] = a1.w * srow;
+                        vsv[0] = b0.x, vsv[1] = b0.y, vsv[2] = b0.z, vsv[3] = b0.w;
+                        vsv[4] = b1.x, vsv[5] = b1.y, vsv[6] = b1.z, vsv[7] = b1.w;
+                    }
                     uint32_t sr[128];
                     {
                         const uint32_t sa = tmem + lane_addr + kColS + w * 128;
@@ -921,7 +1050,7 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
                         }
                         const float mb = fmaxf(m0, m1);
                         // a block with no visible column has max -inf (and, past the valid pages, scale 0)
-                        if (mb != -CUDART_INF_F) mx = fmaxf(mx, mb * (scb[b] * p.scale_log2));
+                        if (mb != -CUDART_INF_F) mx = fmaxf(mx, mb * ksv[b]);
                     }
                     const float m_new = fmaxf(m_used, mx);
                     const bool need = (m_new > m_used + kRescaleThreshold);
@@ -953,7 +1082,7 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
 #pragma unroll
                         for (int c = 0; c < 32; c += 2) {
                             const int b = (cb + c) >> 4;
-                            const float ksb = scb[b] * p.scale_log2, vsb = scb[8 + b];
+                            const float ksb = ksv[b], vsb = vsv[b];
                             float x0, x1;
                             if constexpr (kMasked) {
                                 // a masked score is -inf and its block's scale may be 0: keep it -inf, not NaN
@@ -1425,8 +1554,8 @@ int launch(prepos_ctx *ctx, const AttnArgs &a, int tiles_per_lh, cudaStream_t st
     p.nv = two ? 2 : 3;
     if (D == 64) p.nv = 3;
     constexpr int kTileBytes = kTile * D * 2;
-    // tail: 27 barriers, the (m, l) exchange, TMEM slot + merge info + segment admission (+ kFp8: the scale ring)
-    const size_t smem = static_cast<size_t>(p.q_tiles + kNK + p.nv) * kTileBytes + 27 * 8 + 128 * 8 + 40 + (kFp8 ? 8 * 16 * 4 + 16 : 0);
+    // tail: 36 barriers, the (m, l) exchange, TMEM slot + merge info + segment admission (+ kFp8: the scale ring)
+    const size_t smem = static_cast<size_t>(p.q_tiles + kNK + p.nv) * kTileBytes + 36 * 8 + 128 * 8 + 40 + (kFp8 ? 8 * 16 * 4 + 16 : 0);
     // one CTA per SM; never more CTAs than tiles, never more than the partial slots provisioned
     long long grid = ctx->num_sms;
     if (grid > p.total_tiles) grid = p.total_tiles;

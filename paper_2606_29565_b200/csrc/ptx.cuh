@@ -254,6 +254,22 @@ __device__ __forceinline__ void umma_ts2(uint32_t d_tmem, uint32_t a_tmem, uint3
         "r"(a_tmem), "r"(b_lo), "r"(desc_hi), "r"(idesc), "r"(accumulate)
         : "memory");
 }
+// D[tmem] (+)= A[smem desc] * B[smem desc], 8-bit float inputs (formats in idesc), fp32 accumulate: K = 32 per instruction
+__device__ __forceinline__ void umma_ss2_f8(uint32_t d_tmem, uint32_t a_lo, uint32_t b_lo, uint32_t desc_hi,
+                                            uint32_t idesc, uint32_t accumulate)
+{
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        ".reg .b64 da, db;\n"
+        "mov.b64 da, {%1, %3};\n"
+        "mov.b64 db, {%2, %3};\n"
+        "setp.ne.b32 p, %5, 0;\n"
+        "tcgen05.mma.cta_group::1.kind::f8f6f4 [%0], da, db, %4, p;\n"
+        "}\n" ::"r"(d_tmem),
+        "r"(a_lo), "r"(b_lo), "r"(desc_hi), "r"(idesc), "r"(accumulate)
+        : "memory");
+}
 // all prior tcgen05.mma of this thread arrive on the mbarrier when they complete
 __device__ __forceinline__ void umma_commit(uint32_t bar)
 {
@@ -345,6 +361,13 @@ __device__ __forceinline__ void e4m3x4_to_f16x4(uint32_t x, uint32_t &lo, uint32
     asm("{\n.reg .b16 a, b;\nmov.b32 {a, b}, %2;\ncvt.rn.f16x2.e4m3x2 %0, a;\ncvt.rn.f16x2.e4m3x2 %1, b;\n}"
         : "=r"(lo), "=r"(hi)
         : "r"(x));
+}
+// two fp32 values -> two e4m3 codes in the low 16 bits (lo in the low byte), round to nearest even, saturating
+__device__ __forceinline__ uint32_t pack_e4m3x2(float lo, float hi)
+{
+    uint32_t r;
+    asm("{\n.reg .b16 t;\ncvt.rn.satfinite.e4m3x2.f32 t, %1, %2;\ncvt.u32.u16 %0, t;\n}" : "=r"(r) : "f"(hi), "f"(lo));
+    return r;
 }
 // two bf16 values -> two fp16 values (round to nearest; exact inside fp16's normal range)
 __device__ __forceinline__ uint32_t bf16x2_to_f16x2(uint32_t x)
