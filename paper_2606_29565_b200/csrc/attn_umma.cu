@@ -439,9 +439,8 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
     // register budget: launch gives kLaunchRegs x 384 threads.  The four service warps (warpgroup 0) hand theirs
     // down to kServiceRegs; each softmax thread, which holds a 128-wide score row, grows to kSoftmaxRegs.
     if (warp < 4) {
-    // (setmaxnreg is a warpgroup-wide instruction: the four service warps take the same count.)  kFp8: the widening
-    // warps hold a 128-byte token row per lane: 80 registers for the service warps, 200 for the softmax warps
-    ptx::setmaxnreg_dec<kFp8 ? 80 : kServiceRegs>();
+    // (setmaxnreg is a warpgroup-wide instruction: the four service warps take the same count)
+    ptx::setmaxnreg_dec<kServiceRegs>();
     if (kFp8 && warp == 3) {
         // ===================== kFp8: V widening (the V slabs are requested by warp 0, right behind the K slabs) ====
         SegIter it(p, t0, t1);
@@ -816,7 +815,7 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
         }
     }
     } else {
-        ptx::setmaxnreg_inc<kFp8 ? 200 : kSoftmaxRegs>();
+        ptx::setmaxnreg_inc<kSoftmaxRegs>();
         // ===================== softmax warpgroups (warps 4-7: stream 0, warps 8-11: stream 1) =====================
         const int w = (warp - 4) >> 2;
         const int row = ((warp & 3) << 5) | lane;              // TMEM lane == row within the M-tile
@@ -1017,15 +1016,9 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
                 // block by block) and the V scale on the probabilities before they are packed (fp16)
                 auto tile_body_q = [&](auto masked_tag) {
                     constexpr bool kMasked = decltype(masked_tag)::value;
-                    float ksv[8], vsv[8];   // the tile's K scales (x softmax scale x 2^-k of the row) and V scales
-                    {
-                        const float4 *scb = reinterpret_cast<const float4 *>(sc_s + ((ktile_base + (t - s.tb)) & 7) * 16);
-                        const float4 a0 = scb[0], a1 = scb[1], b0 = scb[2], b1 = scb[3];
-                        ksv[0] = a0.x * srow, ksv[1] = a0.y * srow, ksv[2] = a0.z * srow, ksv[3] = a0.w * srow;
-                        ksv[4] = a1.x * srow, ksv[5] = a1.y * srow, ksv[6] = a1.z * srow, ksv[7] = a1.w * srow;
-                        vsv[0] = b0.x, vsv[1] = b0.y, vsv[2] = b0.z, vsv[3] = b0.w;
-                        vsv[4] = b1.x, vsv[5] = b1.y, vsv[6] = b1.z, vsv[7] = b1.w;
-                    }
+                    // the tile's scales: [0..7] K (times the softmax scale and 2^-k of the row below), [8..15] V; read
+                    // where they are used (broadcast shared-memory loads) rather than held in 16 registers
+                    const float *scb = sc_s + ((ktile_base + (t - s.tb)) & 7) * 16;
                     uint32_t sr[128];
                     {
                         const uint32_t sa = tmem + lane_addr + kColS + w * 128;
@@ -1050,7 +1043,7 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
                         }
                         const float mb = fmaxf(m0, m1);
                         // a block with no visible column has max -inf (and, past the valid pages, scale 0)
-                        if (mb != -CUDART_INF_F) mx = fmaxf(mx, mb * ksv[b]);
+                        if (mb != -CUDART_INF_F) mx = fmaxf(mx, mb * (scb[b] * srow));
                     }
                     const float m_new = fmaxf(m_used, mx);
                     const bool need = (m_new > m_used + kRescaleThreshold);
@@ -1082,7 +1075,7 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
 #pragma unroll
                         for (int c = 0; c < 32; c += 2) {
                             const int b = (cb + c) >> 4;
-                            const float ksb = ksv[b], vsb = vsv[b];
+                            const float ksb = scb[b] * srow, vsb = scb[8 + b];
                             float x0, x1;
                             if constexpr (kMasked) {
                                 // a masked score is -inf and its block's scale may be 0: keep it -inf, not NaN
@@ -1095,7 +1088,14 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
                                     ptx::pack_f32x2(ksb, ksb), nm2);
                                 ptx::unpack_f32x2(x2, x0, x1);
                             }
-                            const float p0 = ptx::ex2(x0), p1 = ptx::ex2(x1);
+                            const bool poly = !kMasked && ((c >> 1) & 3) == 3;   // every fourth pair on the FMA pipe, as above
+                            float p0, p1;
+                            if (poly) {
+                                ptx::ex2_poly2(x0, x1, p0, p1);
+                            } else {
+                                p0 = ptx::ex2(x0);
+                                p1 = ptx::ex2(x1);
+                            }
                             if (c & 2) acc_b = ptx::add_f32x2(acc_b, ptx::pack_f32x2(p0, p1));
                             else acc_a = ptx::add_f32x2(acc_a, ptx::pack_f32x2(p0, p1));
                             pk[c >> 1] = ptx::pack_f16x2(p0 * vsb, p1 * vsb);
@@ -1109,7 +1109,12 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
                 // the choice must be warp-uniform (the bodies hold warp-collective TMEM accesses and votes), and the
                 // causal limit is per row: a tile is "fully visible" only if it is so for all 32 rows of the warp
                 const bool all_visible = __all_sync(0xffffffffu, limit >= kTile);
-                if constexpr (kFp8) {
+                // A warp whose 32 rows all lie past the unit's rows (64 or 96 query rows in a 128-row M-tile) has nothing to
+                // compute: its P rows stay whatever S left there, and the O rows they produce are never read (a row of
+                // O depends on its own row of P only).  It still keeps step with the tiles through the barriers.
+                const bool warp_dead = (mt * 128 + (warp & 3) * 32) >= rows;
+                if (warp_dead) {
+                } else if constexpr (kFp8) {
                     if (all_visible) tile_body_q(std::false_type{});
                     else tile_body_q(std::true_type{});
                 } else {
