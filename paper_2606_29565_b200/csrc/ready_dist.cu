@@ -407,10 +407,12 @@ constexpr int kW4XPad = 32;  // bf16 elements: the row stride of the hidden bloc
 // exponent of 128 around it -- one shift and one LOP3 per register.  The offset 136 is taken out of the group sum
 // afterwards (sum_k (136 + c_k) x_k = sum_k c_k x_k + 136 sum_k x_k), which costs four FMAs per 128 k instead of a
 // packed subtraction per register: the widening, not the stream, is what the issue slots are spent on.
-__device__ __forceinline__ void w4_widen(uint32_t w, uint32_t (&r)[4])
+__device__ __forceinline__ void w4_widen(uint32_t w, uint32_t (&r)[4], uint32_t mask, uint32_t magic)
 {
+    // mask = 0x000f000f and magic = 0x43084308 live in registers so that (x & mask) ^ magic is ONE three-input LOP3
 #pragma unroll
-    for (int i = 0; i < 4; ++i) r[i] = ((w >> (4 * i)) & 0x000f000fu) ^ 0x43084308u;
+    for (int i = 0; i < 4; ++i)
+        asm("lop3.b32 %0, %1, %2, %3, 0x6a;" : "=r"(r[i]) : "r"(w >> (4 * i)), "r"(mask), "r"(magic));
 }
 constexpr float kW4Offset = 136.f;
 
@@ -418,7 +420,7 @@ __global__ void __launch_bounds__(kThreads, 1)
 ready_dist_w4_kernel(const __grid_constant__ CUtensorMap tm_w4, const RdParams p, const __nv_bfloat16 *__restrict__ w_scale)
 {
     extern __shared__ __align__(1024) uint8_t smem_raw[];
-    uint8_t *smem = reinterpret_cast<uint8_t *>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
+    uint8_t *smem = smem_raw;   // declared 1024-byte aligned; no integer round trip, so that loads stay LDS
     uint8_t *stage_base = smem;
     const int x_stride = p.H + kW4XPad;  // elements
     __nv_bfloat16 *xs = reinterpret_cast<__nv_bfloat16 *>(smem + static_cast<size_t>(p.n_stages) * kW4StageBytes);
@@ -515,6 +517,8 @@ ready_dist_w4_kernel(const __grid_constant__ CUtensorMap tm_w4, const RdParams p
         const int b_row = min(g, p.x_rows - 1);   // B fragment: hidden row g (absent rows read the zero row)
         const __nv_bfloat16 *xs_lane = xs + static_cast<size_t>(b_row) * x_stride + t * 8;
         const int w_off = (warp * 16 + g) * 64 + t * 16;   // this lane's 16 bytes of row g within a box
+        uint32_t w4_mask, w4_magic;   // opaque to the compiler: kept in registers, not folded into immediates
+        asm volatile("mov.b32 %0, 0x000f000f;\nmov.b32 %1, 0x43084308;" : "=r"(w4_mask), "=r"(w4_magic));
 
         int stage = 0;
         uint32_t phase = 0;
@@ -557,8 +561,8 @@ ready_dist_w4_kernel(const __grid_constant__ CUtensorMap tm_w4, const RdParams p
                         for (int j = 0; j < 4; ++j) {
                             const uint4 xb = *reinterpret_cast<const uint4 *>(xk + j * 32);
                             uint32_t ra[4], rb[4];
-                            w4_widen(wav[j], ra);
-                            w4_widen(wbv[j], rb);
+                            w4_widen(wav[j], ra, w4_mask, w4_magic);
+                            w4_widen(wbv[j], rb, w4_mask, w4_magic);
                             ptx::mma_bf16_16816(acc, ra[0], rb[0], ra[1], rb[1], xb.x, xb.y);
                             ptx::mma_bf16_16816(acc, ra[2], rb[2], ra[3], rb[3], xb.z, xb.w);
                         }
