@@ -154,3 +154,64 @@ def test_fp8_config2_slice_sampled(prepos, oracle):
     got = out[1].cpu().to(torch.float64).numpy()
     assert float(np.abs(got - outs[(1, 0)]).max()) <= ATTN_ATOL
     assert np.array_equal(k8[1].cpu().numpy(), ok8[1]) and np.array_equal(v8[1].cpu().numpy(), ov8[1])
+
+
+@pytest.mark.parametrize("name", ["c2", "c5"])
+def test_fp8_full_size_configs(prepos, oracle, name):
+    """The FP8 pass at BASELINE's full sizes in the launch configuration bench.py times (tcgen05 FP8 kernel, every
+    layer in one launch, sessions generated on the device with bench.py's seeds and quantised by the synthetic
+    quantiser): config 2 -- every output row of every layer; config 5 -- 64 seeded (layer, head, row) samples through
+    the ranged O7; and on both the WHOLE code pools after the call: the codes Append(E) stored for every entry token
+    of every layer equal the oracle's on the sampled layers, and no other byte moved."""
+    shape = synth.C2 if name == "c2" else synth.C5
+    n_s, l_e = ([4096], [24]) if name == "c2" else ([16384], [32])
+    seed = synth.SEED_BASE + int(name[1])
+    chunk = max(64, (1 << 28) // (shape.layers * shape.Hkv * shape.page * shape.d))
+    sb = synth.make_sessions(shape, n_s, l_e, seed=seed, device="cuda")
+    fb = synth.quantise_sessions_fp8(sb, chunk_pages=chunk)
+    del sb.k_pool, sb.v_pool
+    torch.cuda.empty_cache()
+    k0, v0 = fb.k_pool8.clone(), fb.v_pool8.clone()
+    ctx = prepos.Context(shape.layers, shape.Hq, shape.Hkv, shape.d, shape.H, shape.V, shape.page, max_sessions=1)
+    out = torch.full(sb.q.shape, float("nan"), dtype=torch.bfloat16, device="cuda")
+    st = ctx.entry_attn_fp8(sb.q, sb.k_new, sb.v_new, fb.k_pool8, fb.v_pool8, fb.k_scale, fb.v_scale, sb.page_table,
+                            sb.n_s, sb.l_entry, sb.capacity, out)
+    ctx.sync()
+    assert st == [0] and torch.isfinite(out.float()).all()
+    L, page = l_e[0], shape.page
+    n_pg = -(-(n_s[0] + L) // page)
+    idx = sb.page_table[0, :n_pg].long()
+    table = np.arange(n_pg, dtype=np.int32)
+    # untouched bytes: everything outside the L appended slots of this session
+    j = n_s[0] + torch.arange(L, device="cuda")
+    pg, sl = sb.page_table[0].long()[j // page], j % page
+    ka, va = fb.k_pool8.clone(), fb.v_pool8.clone()
+    ka[:, pg, :, sl] = k0[:, pg, :, sl]
+    va[:, pg, :, sl] = v0[:, pg, :, sl]
+    assert torch.equal(ka, k0) and torch.equal(va, v0), "a byte outside the appended slots changed"
+    del ka, va
+    rng = np.random.default_rng(seed)
+    G = shape.G
+    worst = 0.0
+    if name == "c2":
+        layers = range(shape.layers)
+    else:
+        layers = sorted(set(int(x) for x in rng.integers(0, shape.layers, 8)))
+    for l in layers:
+        k8 = k0[l, idx].cpu().numpy().copy()
+        v8 = v0[l, idx].cpu().numpy().copy()
+        ks, vs = fb.k_scale[l, idx].cpu().numpy(), fb.v_scale[l, idx].cpu().numpy()
+        q, kn, vn = bits(sb.q[l]), bits(sb.k_new[l]), bits(sb.v_new[l])
+        if name == "c2":
+            ref = oracle.entry_attn_fp8(q, kn, vn, k8, v8, ks, vs, table, n_s[0], sb.capacity[0])
+            worst = max(worst, float(np.abs(out[l].cpu().to(torch.float64).numpy() - ref["out"]).max()))
+        else:
+            for _ in range(8):
+                h, i = int(rng.integers(0, shape.Hq)), int(rng.integers(0, L))
+                ref = oracle.entry_attn_fp8(q, kn, vn, k8, v8, ks, vs, table, n_s[0], sb.capacity[0],
+                                            heads=(h, h + 1), rows=(i, i + 1))["out"][i, h]
+                worst = max(worst, float(np.abs(out[l, i, h].cpu().to(torch.float64).numpy() - ref).max()))
+        # the oracle appended into its copies: the stored codes of this layer must be the kernel's
+        assert np.array_equal(fb.k_pool8[l, idx].cpu().numpy(), k8), f"K codes differ at layer {l}"
+        assert np.array_equal(fb.v_pool8[l, idx].cpu().numpy(), v8), f"V codes differ at layer {l}"
+    assert worst <= ATTN_ATOL, worst
