@@ -1224,6 +1224,9 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--quick", action="store_true", help="the timed step only: no side measurements (for ncu runs)")
     ap.add_argument("--attn-path", type=int, default=0, help="0 auto, 1 generic CUDA-core kernel, 2 tcgen05 kernel")
+    ap.add_argument("--section", default=None, choices=["entry_attn_fp8", "ready_dist_w4"],
+                    help="run ONE side measurement of --config alone and print it (what the ncu captures of the "
+                         "NEXT-4 kernels use)")
     args = ap.parse_args()
 
     d = Dist(args.gpus)
@@ -1239,6 +1242,13 @@ def main():
     dev = torch.device("cuda", d.local_rank)
     d.init("nccl")
 
+    if args.section:
+        spec = workload_spec(args.config or HEADLINE)
+        spec = dict(spec, resident=min(spec["resident"], 2))
+        wl = Workload(spec, dev, prepos)
+        fn = {"entry_attn_fp8": run_attn_fp8, "ready_dist_w4": run_ready_dist_w4}[args.section]
+        print(json.dumps({"config": spec["name"], args.section: fn(wl, prepos)}))
+        return
     names = [args.config] if args.config else ALL_CONFIGS
     head = args.config or HEADLINE
     lines = {}
