@@ -454,10 +454,10 @@ def test_fall_through_delta_resume_full_size(prepos, oracle):
     assert sample(v3, o3, rng, layers) <= ATTN_ATOL
 
 
-def test_one_launch_per_layer_cooperative_merge(prepos, oracle):
+def test_one_launch_per_layer_merge_kernel(prepos, oracle):
     """Schedule (S): one prepos_entry_attn call per layer.  With 2 kv heads x 25 tiles over 148 persistent CTAs every
-    unit is spread over ~25 CTAs, which takes the cooperative cross-CTA pass (each covering CTA merges its share of
-    the rows); 256 query rows per kv head (config 5's row geometry) and a ragged last tile.  Oracle on every row,
+    unit is spread over ~25 CTAs, whose partials are combined by the dependent attn_merge_kernel; 256 query rows per
+    kv head (config 5's row geometry) and a ragged last tile.  Oracle on every row,
     Append(E) on every layer, and a second round of launches on the same context (the self-resetting counters)."""
     shape = synth.Shape("s_sched", layers=3, Hq=16, Hkv=2, d=128, H=128, V=64, page=16)
     sb = synth.make_sessions(shape, [3100], [32], seed=77)
@@ -617,3 +617,34 @@ def test_yield_request_from_another_stream_then_resume(prepos, oracle):
         assert torch.equal(out.view(torch.int16), ref.view(torch.int16)), trial
         assert torch.equal(dout.view(torch.int16), dref.view(torch.int16)), trial
     assert caught >= 1, "no trial caught the pass running: the yield path was not exercised"
+
+
+def test_two_contexts_one_launch_per_layer_on_two_streams(prepos, oracle):
+    """Two contexts (two replicas of the library on one GPU) issue their attention one launch per layer at the same
+    time on two streams: every unit is spread over many CTAs and merged across them, and neither pass may depend on
+    having the whole GPU to itself (round 1's in-kernel merge spun on co-residency and could deadlock here).  Both
+    results against the oracle, every row; three rounds on the same contexts."""
+    shape = synth.Shape("two_ctx", layers=6, Hq=16, Hkv=2, d=128, H=128, V=64, page=16)
+    sbs = [synth.make_sessions(shape, [3100], [32], seed=91), synth.make_sessions(shape, [2300, 900], [24, 40], seed=92)]
+    dev = "cuda"
+    ctxs = [prepos.Context(shape.layers, shape.Hq, shape.Hkv, shape.d, shape.H, shape.V, shape.page, max_sessions=2)
+            for _ in sbs]
+    for c in ctxs:
+        c.set_attn_path(2)
+    refs = [oracle_attn_batch(oracle, sb)[0] for sb in sbs]
+    streams = [torch.cuda.Stream(), torch.cuda.Stream()]
+    dv = [dict(q=sb.q.to(dev), kn=sb.k_new.to(dev), vn=sb.v_new.to(dev), pt=sb.page_table.to(dev)) for sb in sbs]
+    for rnd in range(3):
+        pools = [(sb.k_pool.to(dev).clone(), sb.v_pool.to(dev).clone()) for sb in sbs]
+        outs = [torch.full(sb.q.shape, float("nan"), dtype=torch.bfloat16, device=dev) for sb in sbs]
+        torch.cuda.synchronize()
+        for l in range(shape.layers):
+            for k in (0, 1):
+                with torch.cuda.stream(streams[k]):
+                    st = ctxs[k].entry_attn(dv[k]["q"], dv[k]["kn"], dv[k]["vn"], pools[k][0], pools[k][1], dv[k]["pt"],
+                                            sbs[k].n_s, sbs[k].l_entry, sbs[k].capacity, outs[k],
+                                            layer_begin=l, layer_end=l + 1)
+                    assert st == [0] * sbs[k].n_sessions
+        torch.cuda.synchronize()
+        for k in (0, 1):
+            check_attn(outs[k], refs[k], sbs[k])
