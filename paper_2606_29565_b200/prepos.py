@@ -13,7 +13,8 @@ import os
 import torch
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-_SO = os.path.join(_HERE, "libprepos.so")
+# PREPOS_LIB names another build of the same library (kernel tuning experiments); the default is the in-tree build
+_SO = os.environ.get("PREPOS_LIB") or os.path.join(_HERE, "libprepos.so")
 
 OK, SKIPPED_BUDGET = 0, 1
 E_INVALID_ARG, E_SHAPE, E_ALIGN, E_CUDA, E_WORKSPACE, E_NO_DEVICE = -1, -2, -3, -4, -5, -6
