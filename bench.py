@@ -586,8 +586,24 @@ def run_layer_sequential(wl, reps=10):
         gms = timed(lambda i: graphs[i % len(graphs)].replay())
         out["graph_replay"] = {"attn_ms": round(gms, 5), "achieved_gbs": round(ab / (gms * 1e-3) / 1e9, 1),
                                "frac_of_measured_hbm": round(ab / (gms * 1e-3) / 1e9 / peaks()["hbm"], 4)}
+        # the same graph with prepos_ctx_set_kv_prefetch: a layer's launch requests its cached K/V tiles while the previous
+        # layer's merge is still running (legal between the layers of one pass: layer l appends to layer l's pages only)
+        wl.ctx.set_kv_prefetch(True)
+        graphs2 = []
+        for st in wl.sets:
+            g = torch.cuda.CUDAGraph()
+            side.wait_stream(torch.cuda.current_stream())
+            with torch.cuda.graph(g, stream=side):
+                issue(st)
+            graphs2.append(g)
+        torch.cuda.current_stream().wait_stream(side)
+        gms2 = timed(lambda i: graphs2[i % len(graphs2)].replay())
+        wl.ctx.set_kv_prefetch(False)
+        out["graph_replay_kv_prefetch"] = {"attn_ms": round(gms2, 5), "achieved_gbs": round(ab / (gms2 * 1e-3) / 1e9, 1),
+                                           "frac_of_measured_hbm": round(ab / (gms2 * 1e-3) / 1e9 / peaks()["hbm"], 4)}
     except Exception as e:  # capture is a convenience of this measurement, not part of the path
         out["graph_replay"] = {"unavailable": str(e)[:120]}
+        wl.ctx.set_kv_prefetch(False)
         torch.cuda.synchronize()
     return out
 

@@ -166,6 +166,18 @@ int prepos_entry_attn(prepos_ctx *ctx, int layer_begin, int layer_end, int n_ses
                       int32_t *status_per_session, float softmax_scale, void *stream);
 
 /*
+ * Early KV streaming for the one-launch-per-layer schedule.  By default every access of a prepos_entry_attn launch
+ * waits for the previous kernel in the stream to end (programmatic dependent launch).  With on = 1 the launch may
+ * request the CACHED K/V tiles (positions < n_s of the call's layers) as soon as its CTAs are resident -- while the
+ * previous layer's merge is still running -- and only Q, the entry K/V, the appends and the outputs wait.  The
+ * caller guarantees that no kernel still running when the call is issued writes those cached tokens or the page
+ * table: true between the layers of one pass (layer l's launch appends to layer l's pages only), NOT true for a call
+ * that reads what the call right before it appended (a delta resume on the same layers: leave it off or put any
+ * ordinary operation in between).  Applies to the bf16 tcgen05 path.
+ */
+int prepos_ctx_set_kv_prefetch(prepos_ctx *ctx, int on);
+
+/*
  * prepos_entry_attn over an FP8 KV cache (the paper's headline model "runs at 4-bit
  * precision", without naming a storage format: DESIGN.md reading Q20).  Same call, same budget
  * check, same outputs; the session's pages hold OCP e4m3 codes (1-4-3, bias 7, no infinities, max 448):

@@ -157,6 +157,7 @@ int prepos_ctx_create(prepos_ctx **out, const prepos_model_shape *shape, int max
     c->yield_host = nullptr;
     c->attn_launch_seq = 0;
     c->attn_slice = 0;
+    c->attn_kv_prefetch = 0;
     c->yield_dirty = false;
     c->pass_open = false;
     c->pass_grid = c->pass_merge_grid = c->pass_head_dim = 0;
@@ -438,6 +439,13 @@ int prepos_ctx_set_attn_slice(prepos_ctx *ctx, int max_segments_per_launch)
 {
     if (!ctx || max_segments_per_launch < 0) return PREPOS_E_INVALID_ARG;
     ctx->attn_slice = max_segments_per_launch;
+    return PREPOS_OK;
+}
+
+int prepos_ctx_set_kv_prefetch(prepos_ctx *ctx, int on)
+{
+    if (!ctx) return PREPOS_E_INVALID_ARG;
+    ctx->attn_kv_prefetch = on ? 1 : 0;
     return PREPOS_OK;
 }
 

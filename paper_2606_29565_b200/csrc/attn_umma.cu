@@ -72,6 +72,7 @@ struct UmmaParams {
     unsigned int launch_seq;
     int resume;                      // 1: CTA c skips its first progress[c] segments
     int slice;                       // > 0: stop after this many segments per launch (bounded residency)
+    int early_kv;                    // 1: the cached K/V tiles may be requested before the previous kernel has ended
 };
 
 struct Seg {
@@ -355,8 +356,13 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
     ptx::tc_fence_after();
     const uint32_t tmem = *tmem_slot;
     // everything above touched only this CTA's shared memory and TMEM; from here on the kernel reads what earlier
-    // kernels in the stream wrote (the plan, the pools, Q)
-    ptx::griddep_wait();
+    // kernels in the stream wrote (the plan, the pools, Q).  With early_kv (prepos_ctx_set_kv_prefetch: the caller
+    // guarantees that no kernel still running writes the CACHED tokens this call reads) the K / V producers start
+    // streaming cached tiles right away -- the rings fill while the predecessor's merge is still running, which in the
+    // one-launch-per-layer schedule hides the first-byte latency of every layer -- and every other access (Q, the
+    // entry K/V, the appends, out, the partial slots) waits for the predecessor where it is first needed.
+    const bool early = p.early_kv && !p.resume;
+    if (!early) ptx::griddep_wait();
     ptx::griddep_launch();
 
     const long long t0 = cta_begin(p, gridDim.x, blockIdx.x);
@@ -554,6 +560,7 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
         const uint64_t pol_new = ptx::policy_evict_last();  // entry K/V: just produced, re-read by every row chunk
         int slot = 0;
         uint32_t ph = 0;
+        bool dep_waited = false;
         SegIter it(p, t0, t1);
         Seg s;
         int seg = 0, kproc = 0;
@@ -599,6 +606,10 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
                         ptx::tma_load_5d(ptx::smem_u32(dst + lane * page_bytes), tm, fb, 0, 0, 0,
                                          (pg * p.Hkv + s.kvh) * page_groups, s.layer, pol);
                 } else {
+                    if (early && !dep_waited) {   // K_new / V_new are the predecessor's business
+                        ptx::griddep_wait();
+                        dep_waited = true;
+                    }
                     // entry-token tile: one box per 8 tokens straight from K_new / V_new.  Tokens past the ones this
                     // unit can see (later tokens, the next session's, or out of bounds = zero) are finite and masked
                     // by the softmax; V rows that no box covers are zeroed so that P = 0 never meets stale NaNs.
@@ -630,6 +641,7 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
         SegIter it(p, t0, t1);
         Seg s;
         const uint64_t pol_q = ptx::policy_evict_last();  // Q is re-read by every CTA that shares the unit
+        if (early) ptx::griddep_wait();   // Q, the appends and (kFp8) nothing else of this warp precede the predecessor's end
         int k = 0, seg = 0;
         int cslot = 0;   // kFp8: ring slot of the V tile being widened
         uint32_t cph = 0;
@@ -816,6 +828,7 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
     }
     } else {
         ptx::setmaxnreg_inc<kSoftmaxRegs>();
+        if (early) ptx::griddep_wait();   // out, the partial slots and the counters are shared with the predecessor
         // ===================== softmax warpgroups (warps 4-7: stream 0, warps 8-11: stream 1) =====================
         const int w = (warp - 4) >> 2;
         const int row = ((warp & 3) << 5) | lane;              // TMEM lane == row within the M-tile
@@ -1691,6 +1704,7 @@ int launch(prepos_ctx *ctx, const AttnArgs &a, int tiles_per_lh, cudaStream_t st
     p.progress = ctx->attn_progress;
     p.pass_state = ctx->attn_pass_state;
     p.slice = ctx->attn_slice;
+    p.early_kv = (ctx->attn_kv_prefetch && !kFp8) ? 1 : 0;   // (the FP8 path reads the entry's codes back from the pages)
     p.resume = 0;
     // keep the launch: prepos_entry_attn_resume re-issues it with resume = 1 (same plan, same grid, same partial slots)
     static_assert(std::is_trivially_copyable<UmmaParams>::value, "UmmaParams is saved as bytes");

@@ -108,6 +108,7 @@ struct prepos_ctx {
     unsigned int *yield_host;        // pinned: [0] = 1 (source of the flag copy), [1] = read-back of pass_state
     unsigned int attn_launch_seq;
     int attn_slice;                  // > 0: at most this many segments per CTA and launch
+    int attn_kv_prefetch;            // 1: cached K/V tiles may be requested before the previous kernel has ended
     bool yield_dirty;                // a yield was requested since the flag / arrival counters were last cleared
     bool pass_open;                  // the last attention call was a tcgen05 launch that can be resumed
     std::vector<unsigned char> pass_params;   // its kernel parameters

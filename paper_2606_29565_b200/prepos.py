@@ -26,6 +26,7 @@ EXPORTS = [
     "prepos_strerror", "prepos_version", "prepos_workspace_bytes", "prepos_ctx_create", "prepos_ctx_destroy",
     "prepos_ctx_sync", "prepos_ctx_launch_count", "prepos_ctx_set_attn_path", "prepos_entry_attn", "prepos_entry_attn_fp8",
     "prepos_ctx_request_yield", "prepos_entry_attn_resume", "prepos_entry_attn_pending", "prepos_ctx_set_attn_slice",
+    "prepos_ctx_set_kv_prefetch",
     "prepos_ready_dist", "prepos_ready_dist_w4", "prepos_scan_logits", "prepos_gate_serve", "prepos_invalidate", "prepos_gate_sweep",
     "prepos_fastset_build",
 ]
@@ -83,6 +84,8 @@ def lib() -> C.CDLL:
         L.prepos_entry_attn_pending.argtypes = [vp, vp, C.POINTER(C.c_int32)]
         L.prepos_ctx_set_attn_slice.restype = i32
         L.prepos_ctx_set_attn_slice.argtypes = [vp, i32]
+        L.prepos_ctx_set_kv_prefetch.restype = i32
+        L.prepos_ctx_set_kv_prefetch.argtypes = [vp, i32]
         L.prepos_ready_dist.restype = i32
         L.prepos_ready_dist.argtypes = [vp, i32, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp]
         L.prepos_ready_dist_w4.restype = i32
@@ -269,6 +272,9 @@ class Context:
 
     def set_attn_slice(self, max_segments_per_launch: int):
         _check(lib().prepos_ctx_set_attn_slice(self._h, int(max_segments_per_launch)), "prepos_ctx_set_attn_slice")
+
+    def set_kv_prefetch(self, on: bool):
+        _check(lib().prepos_ctx_set_kv_prefetch(self._h, int(bool(on))), "prepos_ctx_set_kv_prefetch")
 
     def ready_dist(self, session_ids, hidden, w_vocab, records, session_version, position_p=None, entry_hash=None,
                    skip_mask=None, logits_out=None, expected_version=None):

@@ -454,7 +454,8 @@ def test_fall_through_delta_resume_full_size(prepos, oracle):
     assert sample(v3, o3, rng, layers) <= ATTN_ATOL
 
 
-def test_one_launch_per_layer_merge_kernel(prepos, oracle):
+@pytest.mark.parametrize("kv_prefetch", [False, True])
+def test_one_launch_per_layer_merge_kernel(prepos, oracle, kv_prefetch):
     """Schedule (S): one prepos_entry_attn call per layer.  With 2 kv heads x 25 tiles over 148 persistent CTAs every
     unit is spread over ~25 CTAs, whose partials are combined by the dependent attn_merge_kernel; 256 query rows per
     kv head (config 5's row geometry) and a ragged last tile.  Oracle on every row,
@@ -464,6 +465,9 @@ def test_one_launch_per_layer_merge_kernel(prepos, oracle):
     dev = "cuda"
     ctx = prepos.Context(shape.layers, shape.Hq, shape.Hkv, shape.d, shape.H, shape.V, shape.page, max_sessions=1)
     ctx.set_attn_path(2)
+    # with kv_prefetch a layer's launch streams its cached tiles while the previous layer's merge is still running
+    # (prepos_ctx_set_kv_prefetch: legal here, layer l's launch writes layer l's pages only)
+    ctx.set_kv_prefetch(kv_prefetch)
     outs, _, _, _ = oracle_attn_batch(oracle, sb)
     for rnd in range(2):
         kp, vp = sb.k_pool.to(dev).clone(), sb.v_pool.to(dev).clone()
@@ -631,6 +635,7 @@ def test_two_contexts_one_launch_per_layer_on_two_streams(prepos, oracle):
             for _ in sbs]
     for c in ctxs:
         c.set_attn_path(2)
+    ctxs[1].set_kv_prefetch(True)      # one of the two also streams its cached tiles ahead of the dependency wait
     refs = [oracle_attn_batch(oracle, sb)[0] for sb in sbs]
     streams = [torch.cuda.Stream(), torch.cuda.Stream()]
     dv = [dict(q=sb.q.to(dev), kn=sb.k_new.to(dev), vn=sb.v_new.to(dev), pt=sb.page_table.to(dev)) for sb in sbs]
