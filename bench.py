@@ -422,9 +422,20 @@ def run_gate_serve(wl, prepos, reps=200):
             both_h.copy_(both, non_blocking=True)
             torch.cuda.synchronize()
             walls.append((time.perf_counter() - t0) * 1e6)
+        # the same serve with the decisions written straight into pinned host memory (the outputs are plain pointers:
+        # pinned memory is device-addressable), so a serve is ONE launch + one sync, no copy call
+        zc = torch.zeros((2, B), dtype=torch.int32).pin_memory()
+        walls_zc = []
+        for _ in range(reps):
+            t0 = time.perf_counter()
+            ctx.gate_serve(req, recs, ver, wl.bitmap, s.tau, zc[0], zc[1])
+            torch.cuda.synchronize()
+            walls_zc.append((time.perf_counter() - t0) * 1e6)
+        assert torch.equal(zc, both_h), "zero-copy serve disagrees with the copied one"
         res[f"B{B}"] = {"device_us_per_call": round(dev_us, 3), "device_us_per_serve": round(dev_us / B, 5),
                         "wall_us_per_call_p50": round(statistics.median(walls), 2),
                         "wall_us_per_serve_p50": round(statistics.median(walls) / B, 5),
+                        "wall_us_per_call_pinned_out_p50": round(statistics.median(walls_zc), 2),
                         "served": int((dec_h == 0).sum())}
     ctx.close()
     return res

@@ -289,7 +289,8 @@ int prepos_scan_logits(prepos_ctx *ctx, int n, const float *logits, prepos_recor
  *   top1 not in A                                                                    -> NOT_IN_FAST_SET
  *   gap < tau (strict_gt: gap <= tau, the paper's Eq. 12 form)                        -> GAP_BELOW_TAU
  *   otherwise SERVED with token_out[r] = top1.  token_out[r] = -1 unless SERVED.
- * All arrays DEVICE.  request_entry_hash nullable (= all relaxed).  fast_set_bitmap: ceil(V/32) words,
+ * All arrays DEVICE (decision_out / token_out may be pinned host memory, which the device addresses directly: a lone
+ * serve is then one launch and one sync, no copy).  request_entry_hash nullable (= all relaxed).  fast_set_bitmap: ceil(V/32) words,
  * bit (id & 31) of word (id >> 5).  The version compare is the authority (Sec. 3.6): a record whose
  * session was invalidated earlier in stream order is never served.
  */
