@@ -115,14 +115,12 @@ def _check(status: int, where: str) -> int:
 
 
 def _p(t):
-    """device/host pointer of a tensor (None -> NULL)."""
-    if t is None:
-        return None
-    return C.c_void_p(t.data_ptr())
+    """device/host pointer of a tensor as a plain int (None -> NULL); ctypes converts it per the argtypes"""
+    return None if t is None else t.data_ptr()
 
 
 def _stream():
-    return C.c_void_p(torch.cuda.current_stream().cuda_stream)
+    return torch.cuda.current_stream().cuda_stream
 
 
 def _host_i32(v) -> torch.Tensor:
