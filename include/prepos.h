@@ -68,7 +68,8 @@ enum {
     PREPOS_E_ALIGN = -3,     /* a device pointer or stride is not 16-byte aligned */
     PREPOS_E_CUDA = -4,      /* a CUDA runtime/driver call or an earlier kernel failed */
     PREPOS_E_WORKSPACE = -5, /* the workspace given to prepos_ctx_create is too small for this call */
-    PREPOS_E_NO_DEVICE = -6  /* no sm_100 device / driver: there is no CPU fallback */
+    PREPOS_E_NO_DEVICE = -6, /* no sm_100 device / driver: there is no CPU fallback */
+    PREPOS_E_FIXED_SCRATCH = -7 /* the request exceeds the built-in scratch of a no-allocation entry point */
 };
 
 /* serve decisions written by prepos_gate_serve (Alg. 2) */
@@ -281,6 +282,48 @@ int prepos_ready_dist_w4(prepos_ctx *ctx, int n, const int32_t *session_ids,
  * logits DEVICE fp32 [n][V]; out DEVICE [n].
  */
 int prepos_scan_logits(prepos_ctx *ctx, int n, const float *logits, prepos_record *out, void *stream);
+
+/*
+ * prepos_scan_logits for callers that cannot allocate device memory.
+ *
+ * Who that is.  The scan is the serve-time fast path (Alg. 2 l.3-4; T_scan(V), Eq. 3):
+ * it runs inside a serving engine's request handler.  Such an engine has normally handed all of the GPU's memory to
+ * its own pool (weights + KV cache) at start-up, so a cudaMalloc from a plug-in either fails or, when it succeeds,
+ * stalls every stream of the device while the driver maps the memory -- on the one path the paper wants at ~1 ms.
+ * The same holds for a component that is loaded into a process it does not own and has no say over that process's
+ * allocator.  Every other libprepos call needs a prepos_ctx, and a ctx needs a caller-allocated device workspace (and
+ * creates pinned host buffers); this call needs neither.
+ *
+ * What it does instead.  The kernel's scratch -- one 32-byte partial per (row, CTA) and one arrival counter per row
+ * for its single cross-CTA pass -- is a fixed array inside the library image:
+ * PREPOS_SCAN_NOALLOC_SCRATCH_BYTES (65 792) bytes of device memory on every GPU that loads libprepos, held until the
+ * process exits whether or not this call is ever made.  The call itself issues one 4*n-byte cudaMemsetAsync and one
+ * kernel on `stream`; it calls no cudaMalloc / cudaFree / cudaMallocHost and no library routine that allocates.
+ *
+ * Limits (the price of a fixed array): n <= PREPOS_SCAN_NOALLOC_MAX_ROWS and vocab <= PREPOS_SCAN_NOALLOC_MAX_VOCAB,
+ * otherwise PREPOS_E_FIXED_SCRATCH and nothing is launched; larger batches belong to prepos_scan_logits.
+ *
+ * Result: exactly what prepos_scan_logits writes -- out[r] gets max_logit, lse, top1, top2, gap and the NONFINITE
+ * flag of logits[r][0..vocab), the other fields of out[r] are left as they are.
+ *
+ * First call on a device.  The first call made while a given device is current looks up the array's device address
+ * (cudaGetSymbolAddress, which also makes the CUDA runtime load the library's kernels onto that device) and checks
+ * that the device is sm_100; the address is kept for later calls.  Make that first call during start-up, on every
+ * device you will use, before any stream capture begins.  Later calls do no set-up.
+ *
+ * Sharing.  There is ONE array per GPU and process, every call uses it, and it keeps the previous call's contents
+ * (the call re-zeroes the counters it needs; the partials are overwritten before they are read).  Two calls that can
+ * run on the same GPU at the same time -- different streams, different host threads -- race on it and may write wrong
+ * records: order them (same stream, or an event between them).  Calls on different GPUs do not interact.
+ *
+ * logits DEVICE fp32 [n][vocab], 4-byte aligned; out DEVICE [n], 16-byte aligned; the current device must be the one
+ * that owns them.  Errors: PREPOS_E_INVALID_ARG (n < 0, vocab < 2, null pointer), PREPOS_E_FIXED_SCRATCH,
+ * PREPOS_E_ALIGN, PREPOS_E_NO_DEVICE, PREPOS_E_CUDA.
+ */
+#define PREPOS_SCAN_NOALLOC_MAX_ROWS 32
+#define PREPOS_SCAN_NOALLOC_MAX_VOCAB (1 << 24)
+#define PREPOS_SCAN_NOALLOC_SCRATCH_BYTES (256 + 32 * 64 * PREPOS_SCAN_NOALLOC_MAX_ROWS)
+int prepos_scan_logits_noalloc(int n, int vocab, const float *logits, prepos_record *out, void *stream);
 
 /*
  * Alg. 2, batched.  For request r on session sid = session_ids[r]:

@@ -98,6 +98,9 @@ const char *prepos_strerror(int status)
         case PREPOS_E_CUDA: return g_last_cuda_error[0] ? g_last_cuda_error : "CUDA error";
         case PREPOS_E_WORKSPACE: return "workspace too small";
         case PREPOS_E_NO_DEVICE: return "no sm_100 CUDA device available (libprepos has no CPU fallback)";
+        case PREPOS_E_FIXED_SCRATCH:
+            return "request exceeds the built-in scratch of the no-allocation entry point (prepos_scan_logits_noalloc: "
+                   "n <= 32 rows, vocab <= 2^24; use prepos_scan_logits for more)";
         default: return "unknown status";
     }
 }

@@ -18,6 +18,8 @@
 //     the reduction tree.
 #include <math_constants.h>
 
+#include <mutex>
+
 #include "common.cuh"
 #include "ptx.cuh"
 
@@ -1027,5 +1029,154 @@ int prepos_launch_scan_logits(prepos_ctx *ctx, int n, const float *logits, prepo
         PREPOS_CUDA_TRY(cudaGetLastError());
         ctx->launches += 1;
     }
+    return PREPOS_OK;
+}
+
+// ---- a4' for callers that cannot allocate: prepos_scan_logits_noalloc ------------------------------------------
+// The serve-time vocabulary scan (Alg. 2 l.3-4; T_scan(V) of Eq. 3) needs a little
+// scratch for its single cross-CTA pass: one 32-byte partial per (row, CTA) and one arrival counter per row.
+// prepos_scan_logits takes it from the ctx workspace, which somebody had to allocate.  The variant below takes it
+// from a fixed array that is part of the library image instead, so that the call needs neither a ctx nor a
+// workspace nor any allocation of its own (who needs that, and the limits: include/prepos.h).
+//
+// g_scan_noalloc_scratch lives in the device memory of every GPU that loads libprepos, from module load until the
+// process exits.  Layout: [0, 256) arrival counters (one uint32 per row), then [row][kNaMaxParts] RdPartial.
+constexpr int kNaMaxRows = PREPOS_SCAN_NOALLOC_MAX_ROWS;
+constexpr int kNaMaxParts = 64;          // CTAs per row (the grid's x extent is capped at this)
+constexpr int kNaCounterBytes = 256;
+constexpr size_t kNaScratchBytes = kNaCounterBytes + sizeof(RdPartial) * kNaMaxRows * kNaMaxParts;
+static_assert(kNaMaxRows * sizeof(unsigned int) <= kNaCounterBytes, "counter block");
+static_assert(kNaScratchBytes == PREPOS_SCAN_NOALLOC_SCRATCH_BYTES, "header and kernel disagree on the scratch size");
+
+static __device__ __align__(256) unsigned char g_scan_noalloc_scratch[kNaScratchBytes];
+
+namespace {
+
+// scan_logits_kernel with the partials packed [row][kNaMaxParts] (gridDim.x <= kNaMaxParts): same per-thread scan,
+// same warp / CTA reduction, same merge order in the last-arriving CTA (lane c takes partials c and c + 32 in that
+// order, then the xor tree), so the records equal the ones prepos_scan_logits writes for the same grid.
+__global__ void __launch_bounds__(kScanThreads)
+scan_logits_noalloc_kernel(int V, const float *__restrict__ logits, prepos_record *__restrict__ out,
+                           RdPartial *partials, unsigned int *counters)
+{
+    const int row = blockIdx.y;
+    const float *lg = logits + static_cast<size_t>(row) * V;
+    Top2Lse st = t2_init();
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const bool vec_ok = ((reinterpret_cast<uintptr_t>(lg) & 15) == 0);
+    const int v4 = vec_ok ? V / 4 : 0;
+    for (int i = blockIdx.x * kScanThreads + threadIdx.x; i < v4; i += gridDim.x * kScanThreads) {
+        const float4 x = __ldg(reinterpret_cast<const float4 *>(lg) + i);
+        t2_push(st, x.x, 4 * i);
+        t2_push(st, x.y, 4 * i + 1);
+        t2_push(st, x.z, 4 * i + 2);
+        t2_push(st, x.w, 4 * i + 3);
+    }
+    for (int i = v4 * 4 + blockIdx.x * kScanThreads + threadIdx.x; i < V; i += gridDim.x * kScanThreads)
+        t2_push(st, __ldg(lg + i), i);
+#pragma unroll
+    for (int mask = 1; mask < 32; mask <<= 1) {
+        const Top2Lse o = t2_shfl_xor(st, mask);
+        t2_merge(st, o);
+    }
+    __shared__ RdPartial s_part[kScanThreads / 32];
+    __shared__ int s_is_last;
+    if (lane == 0) t2_store(&s_part[warp], st);
+    __syncthreads();
+    RdPartial *row_parts = partials + static_cast<size_t>(row) * kNaMaxParts;
+    if (threadIdx.x == 0) {
+        Top2Lse acc = t2_init();
+        for (int w = 0; w < kScanThreads / 32; ++w) {
+            const RdPartial *q = &s_part[w];
+            Top2Lse t;
+            t.m = q->m, t.s = q->s, t.v1 = q->v1, t.v2 = q->v2, t.i1 = q->i1, t.i2 = q->i2, t.nonfinite = q->nonfinite;
+            t2_merge(acc, t);
+        }
+        t2_store(row_parts + blockIdx.x, acc);
+        __threadfence();
+        const unsigned int prev = atomicAdd(&counters[row], 1u);
+        s_is_last = (prev == gridDim.x - 1);
+    }
+    __syncthreads();
+    if (!s_is_last) return;
+    __threadfence();
+    if (warp == 0) {
+        Top2Lse acc = t2_init();
+        const int n_parts = static_cast<int>(gridDim.x);
+        Top2Lse part[kNaMaxParts / 32];
+#pragma unroll
+        for (int j = 0; j < kNaMaxParts / 32; ++j)
+            if (lane + 32 * j < n_parts) part[j] = t2_load(row_parts + lane + 32 * j);
+#pragma unroll
+        for (int j = 0; j < kNaMaxParts / 32; ++j)
+            if (lane + 32 * j < n_parts) t2_merge(acc, part[j]);
+#pragma unroll
+        for (int mask = 1; mask < 32; mask <<= 1) {
+            const Top2Lse o = t2_shfl_xor(acc, mask);
+            t2_merge(acc, o);
+        }
+        if (lane == 0) {
+            prepos_record *rec = out + row;
+            write_record_fields(rec, acc);
+            const uint32_t f = rec->flags & ~PREPOS_FLAG_NONFINITE;
+            rec->flags = f | (acc.nonfinite ? PREPOS_FLAG_NONFINITE : 0u);
+        }
+    }
+}
+
+// Device address of g_scan_noalloc_scratch, per device ordinal.  In host code the array's name only stands in for
+// the symbol: it is not an address a kernel (or cudaMemsetAsync) can use.  The real address is asked for once per
+// device, with that device current, and kept.
+constexpr int kNaMaxDevices = 64;
+std::mutex g_na_mutex;
+unsigned char *g_na_scratch_addr[kNaMaxDevices] = {};
+
+int scan_noalloc_scratch(unsigned char **addr)
+{
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) {
+        cudaGetLastError();
+        return PREPOS_E_NO_DEVICE;
+    }
+    int dev = 0;
+    PREPOS_CUDA_TRY(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= kNaMaxDevices) return PREPOS_E_NO_DEVICE;
+    std::lock_guard<std::mutex> lock(g_na_mutex);
+    if (!g_na_scratch_addr[dev]) {
+        int major = 0;
+        PREPOS_CUDA_TRY(cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev));
+        if (major != 10) return PREPOS_E_NO_DEVICE;  // built for sm_100a only
+        unsigned char *p = nullptr;
+        PREPOS_CUDA_TRY(cudaGetSymbolAddress(reinterpret_cast<void **>(&p), g_scan_noalloc_scratch));
+        if (!p) return PREPOS_E_CUDA;
+        g_na_scratch_addr[dev] = p;
+    }
+    *addr = g_na_scratch_addr[dev];
+    return PREPOS_OK;
+}
+
+}  // namespace
+
+extern "C" int prepos_scan_logits_noalloc(int n, int vocab, const float *logits, prepos_record *out, void *stream)
+{
+    if (n < 0 || vocab < 2) return PREPOS_E_INVALID_ARG;
+    if (n > PREPOS_SCAN_NOALLOC_MAX_ROWS || vocab > PREPOS_SCAN_NOALLOC_MAX_VOCAB) return PREPOS_E_FIXED_SCRATCH;
+    if (n == 0) return PREPOS_OK;
+    if (!logits || !out) return PREPOS_E_INVALID_ARG;
+    if ((reinterpret_cast<uintptr_t>(out) & 15) || (reinterpret_cast<uintptr_t>(logits) & 3)) return PREPOS_E_ALIGN;
+    unsigned char *scratch = nullptr;
+    const int st = scan_noalloc_scratch(&scratch);
+    if (st != PREPOS_OK) return st;
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    unsigned int *counters = reinterpret_cast<unsigned int *>(scratch);
+    RdPartial *partials = reinterpret_cast<RdPartial *>(scratch + kNaCounterBytes);
+    // the array keeps whatever the previous call left: the arrival counters must start at zero, the partials are
+    // fully overwritten before they are read
+    PREPOS_CUDA_TRY(cudaMemsetAsync(counters, 0, sizeof(unsigned int) * n, s));
+    int gx = (vocab + kScanThreads * 16 - 1) / (kScanThreads * 16);  // as prepos_scan_logits: >= 16 logits per thread
+    if (gx > kNaMaxParts) gx = kNaMaxParts;
+    if (gx < 1) gx = 1;
+    scan_logits_noalloc_kernel<<<dim3(gx, n), kScanThreads, 0, s>>>(vocab, logits, out, partials, counters);
+    PREPOS_CUDA_TRY(cudaGetLastError());
     return PREPOS_OK;
 }

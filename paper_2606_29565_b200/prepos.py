@@ -17,17 +17,18 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _SO = os.environ.get("PREPOS_LIB") or os.path.join(_HERE, "libprepos.so")
 
 OK, SKIPPED_BUDGET = 0, 1
-E_INVALID_ARG, E_SHAPE, E_ALIGN, E_CUDA, E_WORKSPACE, E_NO_DEVICE = -1, -2, -3, -4, -5, -6
+E_INVALID_ARG, E_SHAPE, E_ALIGN, E_CUDA, E_WORKSPACE, E_NO_DEVICE, E_FIXED_SCRATCH = -1, -2, -3, -4, -5, -6, -7
 SERVED, GAP_BELOW_TAU, NOT_IN_FAST_SET, STALE_OR_INVALID, INELIGIBLE = 0, 1, 2, 3, 4
 FLAG_VALID, FLAG_NONFINITE, FLAG_MASK = 1, 2, 3
 RECORD_BYTES = 48
+SCAN_NOALLOC_MAX_ROWS, SCAN_NOALLOC_MAX_VOCAB = 32, 1 << 24   # PREPOS_SCAN_NOALLOC_* of include/prepos.h
 
 EXPORTS = [
     "prepos_strerror", "prepos_version", "prepos_workspace_bytes", "prepos_ctx_create", "prepos_ctx_destroy",
     "prepos_ctx_sync", "prepos_ctx_launch_count", "prepos_ctx_set_attn_path", "prepos_entry_attn", "prepos_entry_attn_fp8",
     "prepos_ctx_request_yield", "prepos_entry_attn_resume", "prepos_entry_attn_pending", "prepos_ctx_set_attn_slice",
     "prepos_ctx_set_kv_prefetch",
-    "prepos_ready_dist", "prepos_ready_dist_w4", "prepos_scan_logits", "prepos_gate_serve", "prepos_invalidate", "prepos_gate_sweep",
+    "prepos_ready_dist", "prepos_ready_dist_w4", "prepos_scan_logits", "prepos_scan_logits_noalloc", "prepos_gate_serve", "prepos_invalidate", "prepos_gate_sweep",
     "prepos_fastset_build",
 ]
 
@@ -92,6 +93,8 @@ def lib() -> C.CDLL:
         L.prepos_ready_dist_w4.argtypes = [vp, i32, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp]
         L.prepos_scan_logits.restype = i32
         L.prepos_scan_logits.argtypes = [vp, i32, vp, vp, vp]
+        L.prepos_scan_logits_noalloc.restype = i32
+        L.prepos_scan_logits_noalloc.argtypes = [i32, i32, vp, vp, vp]
         L.prepos_gate_serve.restype = i32
         L.prepos_gate_serve.argtypes = [vp, i32, vp, vp, vp, vp, vp, f32, i32, vp, vp, vp]
         L.prepos_invalidate.restype = i32
@@ -136,6 +139,18 @@ def fastset_build(ids, V: int) -> torch.Tensor:
     bm = torch.zeros((V + 31) // 32, dtype=torch.int32)
     _check(lib().prepos_fastset_build(_p(ids), ids.numel(), V, _p(bm)), "prepos_fastset_build")
     return bm
+
+
+def scan_logits_noalloc(logits: torch.Tensor, records_out: torch.Tensor):
+    """prepos_scan_logits_noalloc on the current stream: the scan of stored logits for callers that cannot allocate
+    device memory (no Context, hence no workspace; the kernel's scratch is a fixed array inside libprepos.so).
+    logits [n, V] fp32 on the current device, n <= SCAN_NOALLOC_MAX_ROWS, V <= SCAN_NOALLOC_MAX_VOCAB (beyond that:
+    PreposError with status E_FIXED_SCRATCH); records_out a record table with at least n rows.  One scratch array per
+    GPU is shared by every call: do not let two calls overlap on the same GPU.  Make the first call on each device
+    during start-up (it looks up the array's address once)."""
+    assert logits.dtype == torch.float32 and logits.dim() == 2 and logits.is_contiguous()
+    _check(lib().prepos_scan_logits_noalloc(logits.shape[0], logits.shape[1], _p(logits), _p(records_out), _stream()),
+           "prepos_scan_logits_noalloc")
 
 
 def new_records(n_sessions: int, device="cuda") -> torch.Tensor:

@@ -81,6 +81,26 @@ def test_fails_loudly_without_device(lib):
     assert lib.prepos_ready_dist(None, 1, None, None, None, None, None, None, None, None, None, None, None) == prepos.E_INVALID_ARG
 
 
+def test_noalloc_scan_checks_its_fixed_limits_before_anything_else(lib):
+    """prepos_scan_logits_noalloc (the entry point for callers that cannot allocate): sizes beyond its built-in
+    scratch are refused with their own status on any box; the header's byte count is what the limits imply."""
+    from paper_2606_29565_b200 import prepos
+    hdr = open(os.path.join(ROOT, "include", "prepos.h")).read()
+    assert re.search(r"#define PREPOS_SCAN_NOALLOC_MAX_ROWS 32\b", hdr) and prepos.SCAN_NOALLOC_MAX_ROWS == 32
+    assert re.search(r"#define PREPOS_SCAN_NOALLOC_MAX_VOCAB \(1 << 24\)", hdr) and prepos.SCAN_NOALLOC_MAX_VOCAB == 1 << 24
+    assert re.search(r"PREPOS_E_FIXED_SCRATCH = -7\b", hdr) and prepos.E_FIXED_SCRATCH == -7
+    f = lib.prepos_scan_logits_noalloc
+    assert f(33, 1024, None, None, None) == prepos.E_FIXED_SCRATCH
+    assert f(1, (1 << 24) + 1, None, None, None) == prepos.E_FIXED_SCRATCH
+    assert f(-1, 1024, None, None, None) == prepos.E_INVALID_ARG and f(1, 1, None, None, None) == prepos.E_INVALID_ARG
+    assert f(0, 1024, None, None, None) == prepos.OK
+    assert f(1, 1024, None, None, None) == prepos.E_INVALID_ARG      # null pointers
+    assert "prepos_scan_logits" in prepos.strerror(prepos.E_FIXED_SCRATCH)
+    if not torch.cuda.is_available():
+        buf = torch.zeros(1024 + 16, dtype=torch.float32)
+        assert f(1, 1024, buf.data_ptr(), (buf.data_ptr() + 15) // 16 * 16, None) == prepos.E_NO_DEVICE
+
+
 def test_product_never_imports_oracle():
     """The product path must not route through the oracle (and vice versa)."""
     pkg = os.path.join(ROOT, "paper_2606_29565_b200")
