@@ -11,10 +11,12 @@ sessions, every stage through the C ABI of libprepos (ctypes binding, paper_2606
     prepos_ready_dist   LM head at the last entry position fused with the vocabulary reduction (a3-a4)
     prepos_gate_serve   the request(s) that arrive next are answered from the cached record (a5)
 
-Without --config it runs ALL FIVE BASELINE.json configs and prints ONE JSON line: the top-level fields are
-those of the headline workload, configs[4] (70B-shaped: the paper's measured model class, and the
-largest per-session pass: 7.56 GB), and `per_config` carries the same fields for c1..c4.  --config cN runs that one
-config alone (what the ncu captures under profiles/ use).  See DESIGN.md "Measurement" for every field.
+It prints ONE compact JSON line on stdout (a few KB: the contract fields of the headline workload, which the driver
+parses) and writes every side measurement to gpurun_out/bench_detail.json.  Without --config the headline is
+configs[4] (70B-shaped: the paper's measured model class, and the largest per-session pass: 7.56 GB),
+timed with the caller's --steps / --warmup; the other four configs then run with their own defaults and appear in the
+line only as `other_configs` (us/session + roofline fraction; everything else about them is in the detail file).
+--config cN runs that one config alone (what the ncu captures under profiles/ use).  See DESIGN.md "Measurement".
 `--impl reference` times the CPU oracle (oracle/) on a bounded sample of the headline workload instead.
 """
 from __future__ import annotations
@@ -1134,11 +1136,12 @@ def cpu_baseline_leg(spec, budget_s):
     return out
 
 
-def run_config(name, args, d, dev, prepos):
-    """One BASELINE config -> the dict of its JSON fields (rank 0; other ranks return None)."""
+def run_config(name, args, d, dev, prepos, steps=None, warmup=None):
+    """One BASELINE config -> the dict of its JSON fields (rank 0; other ranks return None).  `steps` / `warmup`
+    None = the config's own defaults (--steps / --warmup bind the headline config only)."""
     spec = workload_spec(name)
-    steps = args.steps if args.steps is not None else DEFAULT_STEPS[name][0]
-    warmup = max(args.warmup if args.warmup is not None else DEFAULT_STEPS[name][1], 3)
+    steps = steps if steps is not None else DEFAULT_STEPS[name][0]
+    warmup = max(warmup if warmup is not None else DEFAULT_STEPS[name][1], 3)
     wl = Workload(spec, dev, prepos)
     if args.attn_path:
         wl.ctx.set_attn_path(args.attn_path)
@@ -1239,6 +1242,47 @@ def run_config(name, args, d, dev, prepos):
     return line
 
 
+DETAIL_REL = "gpurun_out/bench_detail.json"
+DETAIL_PATH = os.path.join(ROOT, "gpurun_out", "bench_detail.json")
+CONTRACT_KEYS = ("metric", "value", "unit", "n_gpus", "steps", "warmup", "ms_per_step", "higher_is_better", "scaling",
+                 "vs_baseline", "dtype", "data", "config", "roofline", "entry_pass_roofline", "cpu_baseline", "e2e",
+                 "clocks", "gpu_launches")
+
+
+def _finite(x):
+    """Non-finite floats -> None, so that the line is strict JSON."""
+    if isinstance(x, float):
+        return x if math.isfinite(x) else None
+    if isinstance(x, dict):
+        return {k: _finite(v) for k, v in x.items()}
+    if isinstance(x, (list, tuple)):
+        return [_finite(v) for v in x]
+    return x
+
+
+def contract_line(full, others):
+    """The ONE stdout line: the headline config's contract fields only, a few KB (the driver parses this line; every
+    side measurement and the other configs go to DETAIL_PATH).  `others`: {config: full dict} of the rest of the run."""
+    line = {k: full[k] for k in CONTRACT_KEYS if k in full}
+    if "cpu_baseline" in line:
+        line["cpu_baseline"] = {k: v for k, v in line["cpu_baseline"].items() if k != "one_thread"}
+    if "e2e" in line:
+        line["e2e"] = {k: v for k, v in line["e2e"].items() if k != "timing"}
+    line["kernels"] = {k: {kk: v[kk] for kk in ("ms", "frac_of_measured_hbm", "frac_of_measured_bf16") if kk in v}
+                       for k, v in full["kernels"].items()}
+    if "gate_serve" in full:
+        line["gate_serve"] = {b: {"device_us_per_call": v["device_us_per_call"], "device_us_per_serve": v["device_us_per_serve"],
+                                  "wall_us_per_call_p50": v["wall_us_per_call_p50"]}
+                              for b, v in full["gate_serve"].items() if isinstance(v, dict) and "device_us_per_call" in v}
+    if others:
+        line["other_configs"] = {n: {"us_per_session": round(o["value"], 2), "roofline_bound": o["roofline"]["bound"],
+                                     "roofline_frac": o["roofline"]["frac"],
+                                     "step_frac_of_measured_hbm": o["entry_pass_roofline"]["frac_of_measured_hbm"]}
+                                 for n, o in others.items()}
+    line["detail"] = DETAIL_REL
+    return _finite(line)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -1276,18 +1320,26 @@ def main():
         fn = {"entry_attn_fp8": run_attn_fp8, "ready_dist_w4": run_ready_dist_w4}[args.section]
         print(json.dumps({"config": spec["name"], args.section: fn(wl, prepos)}))
         return
-    names = [args.config] if args.config else ALL_CONFIGS
     head = args.config or HEADLINE
+    # the headline first, with the caller's --steps / --warmup; in the default run the other four follow with their
+    # own defaults, so that steps x ms_per_step of the printed line is the headline's timed region
+    names = [head] if args.config else [head] + [n for n in ALL_CONFIGS if n != head]
     lines = {}
     for name in names:
-        lines[name] = run_config(name, args, d, dev, prepos)
+        mine = name == head
+        lines[name] = run_config(name, args, d, dev, prepos, args.steps if mine else None, args.warmup if mine else None)
     if d.rank == 0:
-        line = lines[head]
-        if len(names) > 1:
-            line["per_config"] = {n: lines[n] for n in names if n != head}
-            line["headline"] = (f"{head}: configs[{int(head[1]) - 1}] of BASELINE.json (the largest per-session pass and the "
-                                "paper's measured model class); per_config holds the other four")
-        print(json.dumps(line))
+        others = {n: lines[n] for n in names if n != head}
+        detail = _finite({"headline": head, "configs": lines})
+        try:
+            os.makedirs(os.path.dirname(DETAIL_PATH), exist_ok=True)
+            with open(DETAIL_PATH, "w") as f:
+                json.dump(detail, f, allow_nan=False)
+            sys.stderr.write(f"bench.py: every section of every config -> {DETAIL_PATH}\n")
+        except OSError as e:   # a read-only tree: the contract line below does not depend on the side file
+            sys.stderr.write(f"bench.py: could not write {DETAIL_PATH}: {e}\n")
+        sys.stdout.write(json.dumps(contract_line(lines[head], others), allow_nan=False, separators=(",", ":")) + "\n")
+        sys.stdout.flush()
     d.barrier()
     d.close()
 

@@ -34,3 +34,35 @@ def test_bench_prints_one_contract_line():
     c = d["cpu_baseline"]
     assert c["kind"] == "oracle" and c["cores"] >= 1 and c["value"] > d["value"]
     assert d["clocks"]["sm_max_mhz"] >= d["clocks"]["sm_mhz"] > 0
+
+
+def _strict_loads(text):
+    def bad(c):
+        raise ValueError(f"non-standard JSON constant {c}")
+    return json.loads(text, parse_constant=bad)
+
+
+def test_default_invocation_prints_one_small_strict_line():
+    """What the driver runs: no --config, --steps 20 --warmup 5.  All five configs run, but stdout is ONE line of a
+    few KB holding the headline (configs[4]) contract fields; everything else goes to gpurun_out/bench_detail.json.
+    (Round 2's 24 KB line with every config nested in it was not parsed by the driver.)"""
+    r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--steps", "20", "--warmup", "5"],
+                       cwd=ROOT, capture_output=True, text=True, timeout=900)
+    assert r.returncode == 0, r.stderr[-2000:]
+    lines = [x for x in r.stdout.splitlines() if x.strip()]
+    assert len(lines) == 1, [x[:80] for x in lines[:3]]
+    assert len(lines[0]) < 4096, len(lines[0])
+    d = _strict_loads(lines[0])
+    assert d["steps"] == 20 and d["warmup"] == 5 and d["n_gpus"] == 1
+    assert d["config"]["workload"].startswith("configs[4]")
+    assert d["value"] > 0 and d["unit"] == "us/session" and d["higher_is_better"] is False
+    # one session per step: us/session is the step time, so steps x ms_per_step is the headline's timed region
+    assert abs(d["value"] - d["ms_per_step"] * 1e3) <= 1e-6 * d["value"]
+    for k in ("roofline", "cpu_baseline", "e2e", "clocks", "gpu_launches", "kernels", "gate_serve"):
+        assert k in d, k
+    assert d["roofline"]["frac"] > 0 and d["e2e"]["value"] > 0 and d["e2e"]["h2d_bytes_per_step"] > 0
+    assert d["cpu_baseline"]["kind"] == "oracle" and d["gpu_launches"] == 4 * d["steps"]
+    assert sorted(d["other_configs"]) == ["c1", "c2", "c3", "c4"]
+    detail = _strict_loads(open(os.path.join(ROOT, d["detail"])).read())
+    assert detail["headline"] == "c5" and sorted(detail["configs"]) == ["c1", "c2", "c3", "c4", "c5"]
+    assert detail["configs"]["c5"]["value"] == d["value"]
