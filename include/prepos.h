@@ -57,7 +57,8 @@
 extern "C" {
 #endif
 
-#define PREPOS_VERSION 100 /* 0.1.0 */
+#define PREPOS_VERSION 101 /* 0.1.1: bumped whenever a signature, a struct or a status code changes; the Python
+                              * binding refuses a library whose prepos_version() differs from the one it was written for */
 
 /* status codes */
 enum {
@@ -209,12 +210,16 @@ int prepos_entry_attn_fp8(prepos_ctx *ctx, int layer_begin, int layer_end, int n
  * Its CTAs therefore have a yield point at every segment boundary (a segment = the CTA's part of one
  * (layer, kv head, session row chunk), at most n_s / 128 + 1 KV tiles):
  *
- *   prepos_ctx_request_yield   sets the ctx's device yield flag with a 4-byte copy on `stream` (use the request's
- *                              high-priority stream; the copy engine does not wait for the running kernel).  Every
- *                              CTA of the running pass finishes its current segment, records how many segments it has
- *                              completed, and exits; the SMs go to whatever is queued at higher priority.  Outputs of
- *                              finished segments are final, partials of cut units stay in the ctx workspace.
- *   prepos_entry_attn_resume   clears the flag and re-issues the SAME launch on `stream`: every CTA skips the
+ *   prepos_ctx_request_yield   asks the ctx's LATEST tcgen05 attention launch to stop: a 4-byte copy on `stream` (use
+ *                              the request's high-priority stream; the copy engine does not wait for the running
+ *                              kernel) writes that launch's sequence number into the ctx's device yield word.  Every
+ *                              CTA of that launch re-reads the word at least every 8 KV tiles, finishes its current
+ *                              segment, records how many segments it has completed, and exits; the SMs go to whatever
+ *                              is queued at higher priority.  Outputs of finished segments are final, partials of cut
+ *                              units stay in the ctx workspace.  A request only ever stops the launch it names: one
+ *                              that lands after that launch has ended is inert (it cannot stop a later call or a
+ *                              resume).  PREPOS_OK without a copy when the ctx has no tcgen05 launch to stop.
+ *   prepos_entry_attn_resume   re-issues the SAME launch on `stream` under a new sequence number: every CTA skips the
  *                              segments it completed and carries on.  The result is the one an uninterrupted call
  *                              gives, bit for bit (same plan, same split, same merge order).  A no-op launch when
  *                              the pass had already finished; PREPOS_OK without a launch when nothing is open.
@@ -224,7 +229,8 @@ int prepos_entry_attn_fp8(prepos_ctx *ctx, int layer_begin, int layer_end, int n
  *                              a bounded-residency pass for callers that prefer time slices to a flag; 0 = off.
  *
  * Between a yield and its resume the ctx must not be given another prepos_entry_attn call (it would reuse the
- * workspace the stopped pass still needs; doing so abandons the stopped pass), and nothing queued behind the
+ * workspace the stopped pass still needs; doing so abandons the stopped pass -- whether it was stopped by a request or
+ * by a segment limit -- and the new call starts from clean arrival counters), and nothing queued behind the
  * stopped launch on its stream may read `out`.  Request a yield only while no further attention call of this ctx is
  * queued behind the running one.  The generic CUDA-core path has no yield point (its CTAs are short-lived).
  */

@@ -163,6 +163,8 @@ int prepos_ctx_create(prepos_ctx **out, const prepos_model_shape *shape, int max
     c->attn_kv_prefetch = 0;
     c->yield_dirty = false;
     c->pass_open = false;
+    c->pass_sliced = false;
+    c->tm_pool_kind = 0;
     c->pass_grid = c->pass_merge_grid = c->pass_head_dim = 0;
     c->pass_smem = 0;
     c->plan_staging = nullptr;
@@ -179,7 +181,7 @@ int prepos_ctx_create(prepos_ctx **out, const prepos_model_shape *shape, int max
     if (e == cudaSuccess) e = cudaMemset(c->ws + w.attn_yield, 0, 256 + sizeof(int) * kAttnMaxCtas);
     if (e == cudaSuccess) e = cudaMallocHost(reinterpret_cast<void **>(&c->yield_host), 2 * sizeof(unsigned int));
     if (e == cudaSuccess) {
-        c->yield_host[0] = 1u;
+        c->yield_host[0] = 0u;
         c->yield_host[1] = 0u;
     }
     if (e == cudaSuccess) e = cudaMallocHost(reinterpret_cast<void **>(&c->plan_staging), sizeof(AttnUnit) * c->max_units);
@@ -304,14 +306,14 @@ int plan_attn(prepos_ctx *ctx, int mode, int chunk_tok, bool entries_in_cache, i
     if (status_per_session)
         for (int i = 0; i < n_sessions; ++i)
             status_per_session[i] = (l_entry[i] > capacity_tokens[i] - n_s[i]) ? PREPOS_SKIPPED_BUDGET : PREPOS_OK;
-    ctx->pass_open = false;
-    if (ctx->yield_dirty) {
-        // a yield was requested since the last clear: drop a request that outlived its pass, and the arrival counters
-        // of a pass that was stopped and never resumed
-        PREPOS_CUDA_TRY(cudaMemsetAsync(ctx->attn_yield_flag, 0, sizeof(unsigned int), stream));
+    // The previous tcgen05 pass may have been stopped (a yield request, or a segment limit) and never resumed to its
+    // end: this call abandons it, and its half-counted arrival counters must not reach the new pass's last-arriver
+    // merge.  (The yield flag itself needs no clearing: it names the launch it stops, see prepos_ctx_request_yield.)
+    if (ctx->yield_dirty || (ctx->pass_open && ctx->pass_sliced)) {
         PREPOS_CUDA_TRY(cudaMemsetAsync(ctx->attn_counters, 0, sizeof(unsigned int) * ctx->attn_counters_n, stream));
         ctx->yield_dirty = false;
     }
+    ctx->pass_open = false;
     return PREPOS_OK;
 }
 
@@ -455,7 +457,14 @@ int prepos_ctx_set_kv_prefetch(prepos_ctx *ctx, int on)
 int prepos_ctx_request_yield(prepos_ctx *ctx, void *stream)
 {
     if (!ctx) return PREPOS_E_INVALID_ARG;
+    if (!ctx->pass_open) return PREPOS_OK;   // no tcgen05 pass was issued on this ctx: nothing to stop
     ctx->yield_dirty = true;
+    // The flag carries the sequence number of the launch it is meant for (the ctx's latest): the kernel stops only
+    // when the flag equals its own number.  A copy that lands late -- after that launch has ended, because the
+    // request's stream was backlogged -- therefore cannot stop a later pass or a resume, and nothing ever has to clear
+    // the flag (a clear could itself race with a fresh request).  The pinned source word is read when the copy
+    // executes; a newer request may have raised it by then, which only retargets the copy at the newer launch.
+    ctx->yield_host[0] = ctx->attn_launch_seq;
     PREPOS_CUDA_TRY(cudaMemcpyAsync(ctx->attn_yield_flag, ctx->yield_host, sizeof(unsigned int), cudaMemcpyHostToDevice,
                                     static_cast<cudaStream_t>(stream)));
     return PREPOS_OK;
@@ -477,10 +486,7 @@ int prepos_entry_attn_resume(prepos_ctx *ctx, void *stream)
 {
     if (!ctx) return PREPOS_E_INVALID_ARG;
     if (!ctx->pass_open) return PREPOS_OK;   // nothing to resume (no tcgen05 pass is open on this ctx)
-    if (ctx->yield_dirty) {
-        PREPOS_CUDA_TRY(cudaMemsetAsync(ctx->attn_yield_flag, 0, sizeof(unsigned int), static_cast<cudaStream_t>(stream)));
-        ctx->yield_dirty = false;
-    }
+    // the resume is a new launch with a new sequence number: the request that stopped its predecessor does not match it
     return prepos_resume_attn_umma(ctx, static_cast<cudaStream_t>(stream));
 }
 

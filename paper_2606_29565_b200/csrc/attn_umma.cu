@@ -66,7 +66,7 @@ struct UmmaParams {
                         // 32 rows of one float4 column are 512 contiguous bytes), lse2 [256], pad [256]
     unsigned int *counters;  // [n_lh][n_units] arrival counters of the cross-CTA pass (self-resetting)
     // ---- yield / resume (the idle-window pass "yields to any request")
-    const unsigned int *yield_flag;  // device word: non-zero asks every CTA to stop at its next segment boundary
+    const unsigned int *yield_flag;  // device word: == launch_seq asks every CTA of THAT launch to stop at its next segment boundary
     int *progress;                   // [grid] segments CTA c has completed in this pass (over all its launches)
     unsigned int *pass_state;        // a CTA that stops early writes launch_seq here
     unsigned int launch_seq;
@@ -477,11 +477,12 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
             SegIter it(p, t0, t1);
             Seg s;
             unsigned int yflag = (lane == 0) ? ptx::ld_volatile_global(p.yield_flag) : 0u;
+            int ypoll = 0;   // tiles since launch: the flag is re-read every 8 tiles, ACROSS segments
             while (it.next(p, s)) {
                 if (seg++ < skip) continue;
                 int stop = 0;
                 if (lane == 0) {
-                    stop = (yflag != 0u) || (p.slice > 0 && kproc >= p.slice);
+                    stop = (yflag == p.launch_seq) || (p.slice > 0 && kproc >= p.slice);
                     if (stop) ptx::st_release_cta_smem(&sched[1], kproc);
                     else ptx::st_release_cta_smem(&sched[0], kproc + 1);
                 }
@@ -506,7 +507,7 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
                 int spg_next = scale_page_of(s.tb + 1);
                 float sc_next = scale_of(scale_page_of(s.tb));
                 for (int t = s.tb; t < s.te; ++t) {
-                    if (lane == 0 && ((t - s.tb) & 7) == 7) yflag = ptx::ld_volatile_global(p.yield_flag);
+                    if (lane == 0 && (++ypoll & 7) == 0) yflag = ptx::ld_volatile_global(p.yield_flag);
                     const int pg = pg_next;
                     const float sc_now = sc_next;
                     pg_next = page_of(t + 1);
@@ -564,14 +565,18 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
         SegIter it(p, t0, t1);
         Seg s;
         int seg = 0, kproc = 0;
-        // the yield flag is read ahead of its use (at launch, then every 8 tiles): never a load on the critical path
+        // the yield flag is read ahead of its use (at launch, then every 8 tiles of the CTA's stream -- the count
+        // carries across segments, so a CTA whose segments are all shorter than 8 tiles still sees a request within
+        // 8 tiles): never a load on the critical path.  The flag names the launch it stops (its launch_seq): a request
+        // that lands late, after its pass has ended, cannot stop a later pass or a resume.
         unsigned int yflag = (!is_v && lane == 0) ? ptx::ld_volatile_global(p.yield_flag) : 0u;
+        int ypoll = 0;
         while (it.next(p, s)) {
             if (seg++ < skip) continue;
             if (!is_v) {
                 int stop = 0;
                 if (lane == 0) {
-                    stop = (yflag != 0u) || (p.slice > 0 && kproc >= p.slice);
+                    stop = (yflag == p.launch_seq) || (p.slice > 0 && kproc >= p.slice);
                     if (stop) ptx::st_release_cta_smem(&sched[1], kproc);
                     else ptx::st_release_cta_smem(&sched[0], kproc + 1);
                 }
@@ -590,7 +595,7 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
             };
             int pg_next = page_of(s.tb);
             for (int t = s.tb; t < s.te; ++t) {
-                if (!is_v && lane == 0 && ((t - s.tb) & 7) == 7) yflag = ptx::ld_volatile_global(p.yield_flag);
+                if (!is_v && lane == 0 && (++ypoll & 7) == 0) yflag = ptx::ld_volatile_global(p.yield_flag);
                 const int pg = pg_next;
                 if (t + 1 < s.te) pg_next = page_of(t + 1);
                 if (lane == 0) ptx::mbar_wait(ptx::smem_u32(&empty[slot]), ph ^ 1);
@@ -1636,9 +1641,11 @@ int launch(prepos_ctx *ctx, const AttnArgs &a, int tiles_per_lh, cudaStream_t st
             }
         }
     }
+    // (the bf16 pools take a 5-D map, the e4m3 pools a 3-D byte map: the kind is part of the cache key, since the same
+    // base address, stride value and page count can describe either when a ctx alternates between the two)
     if (kFp8) {
-        if (ctx->tm_k_ptr != a.k_pool8 || ctx->tm_v_ptr != a.v_pool8 || ctx->tm_layer_stride != a.pool_layer_stride ||
-            ctx->tm_n_pages != a.n_pages) {
+        if (ctx->tm_pool_kind != 2 || ctx->tm_k_ptr != a.k_pool8 || ctx->tm_v_ptr != a.v_pool8 ||
+            ctx->tm_layer_stride != a.pool_layer_stride || ctx->tm_n_pages != a.n_pages) {
             int st = encode_pool8_map(&ctx->tm_k, a.k_pool8, ctx->shape, a.pool_layer_stride, a.n_pages);
             if (st == PREPOS_OK) st = encode_pool8_map(&ctx->tm_v, a.v_pool8, ctx->shape, a.pool_layer_stride, a.n_pages);
             if (st != PREPOS_OK) return st;
@@ -1646,9 +1653,10 @@ int launch(prepos_ctx *ctx, const AttnArgs &a, int tiles_per_lh, cudaStream_t st
             ctx->tm_v_ptr = a.v_pool8;
             ctx->tm_layer_stride = a.pool_layer_stride;
             ctx->tm_n_pages = a.n_pages;
+            ctx->tm_pool_kind = 2;
         }
-    } else if (ctx->tm_k_ptr != a.k_pool || ctx->tm_v_ptr != a.v_pool || ctx->tm_layer_stride != a.pool_layer_stride ||
-               ctx->tm_n_pages != a.n_pages) {
+    } else if (ctx->tm_pool_kind != 1 || ctx->tm_k_ptr != a.k_pool || ctx->tm_v_ptr != a.v_pool ||
+               ctx->tm_layer_stride != a.pool_layer_stride || ctx->tm_n_pages != a.n_pages) {
         int st = encode_pool_map(&ctx->tm_k, a.k_pool, ctx->shape, a.pool_layer_stride, a.n_pages);
         if (st == PREPOS_OK) st = encode_pool_map(&ctx->tm_v, a.v_pool, ctx->shape, a.pool_layer_stride, a.n_pages);
         if (st != PREPOS_OK) return st;
@@ -1656,6 +1664,7 @@ int launch(prepos_ctx *ctx, const AttnArgs &a, int tiles_per_lh, cudaStream_t st
         ctx->tm_v_ptr = a.v_pool;
         ctx->tm_layer_stride = a.pool_layer_stride;
         ctx->tm_n_pages = a.n_pages;
+        ctx->tm_pool_kind = 1;
     }
     // entry K/V maps: they follow the call's K_new / V_new pointers (the FP8 path reads the entry from the cache)
     if (!kFp8 && (ctx->tm_kn_ptr != a.k_new || ctx->tm_vn_ptr != a.v_new || ctx->tm_new_layer_stride != a.kv_new_layer_stride ||
@@ -1737,6 +1746,7 @@ int issue(prepos_ctx *ctx, cudaStream_t stream, int resume)
         ctx->launches += 1;
     }
     ctx->pass_open = true;
+    ctx->pass_sliced = p.slice > 0;
     return PREPOS_OK;
 }
 

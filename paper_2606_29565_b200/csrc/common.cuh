@@ -102,14 +102,15 @@ struct prepos_ctx {
     unsigned int *attn_counters;  // [layers * Hkv * max_units] arrival counters (self-resetting)
     size_t attn_counters_n;
     // yield / resume of the tcgen05 attention pass (prepos_ctx_request_yield, prepos_entry_attn_resume)
-    unsigned int *attn_yield_flag;   // device word polled by the persistent CTAs
+    unsigned int *attn_yield_flag;   // device word polled by the persistent CTAs: the launch_seq of the launch to stop
     unsigned int *attn_pass_state;   // device word: launch_seq of the last launch that stopped early
     int *attn_progress;              // device [kAttnMaxCtas]: segments completed per CTA
-    unsigned int *yield_host;        // pinned: [0] = 1 (source of the flag copy), [1] = read-back of pass_state
+    unsigned int *yield_host;        // pinned: [0] = source of the flag copy (a launch_seq), [1] = read-back of pass_state
     unsigned int attn_launch_seq;
     int attn_slice;                  // > 0: at most this many segments per CTA and launch
     int attn_kv_prefetch;            // 1: cached K/V tiles may be requested before the previous kernel has ended
-    bool yield_dirty;                // a yield was requested since the flag / arrival counters were last cleared
+    bool yield_dirty;                // a yield was requested since the arrival counters were last cleared
+    bool pass_sliced;                // the last tcgen05 launch ran with a segment limit (it may have stopped early)
     bool pass_open;                  // the last attention call was a tcgen05 launch that can be resumed
     std::vector<unsigned char> pass_params;   // its kernel parameters
     int pass_grid, pass_merge_grid, pass_head_dim;
@@ -123,6 +124,7 @@ struct prepos_ctx {
     bool plan_inflight;
     // TMA descriptor cache for the KV pools
     void *tm_k_ptr, *tm_v_ptr;
+    int tm_pool_kind;                // 0 none, 1 bf16 pools (5-D map), 2 e4m3 pools (3-D byte map)
     int64_t tm_layer_stride, tm_n_pages;
     CUtensorMap tm_k, tm_v;
     // ... and for the call's entry K/V

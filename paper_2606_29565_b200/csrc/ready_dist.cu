@@ -937,9 +937,9 @@ int prepos_launch_ready_dist(prepos_ctx *ctx, int n, const int32_t *session_ids,
         p.x_rows = (p.n < kNB) ? p.n + 1 : kNB;
         const size_t x_bytes = (static_cast<size_t>(p.x_rows) * (H + kXPad) * 2 + 15) & ~size_t(15);
         const size_t fixed = 1024 + x_bytes + 2 * kMaxStages * 8 + kConsumerWarps * kNB * sizeof(RdPartial);
+        if (fixed + 2 * static_cast<size_t>(kStageBytes) > 232448) return PREPOS_E_SHAPE;   // H too large for two stages
         int stages = static_cast<int>((232448 - fixed) / kStageBytes);
         if (stages > kMaxStages) stages = kMaxStages;
-        if (stages < 2) return PREPOS_E_SHAPE;
         p.n_stages = stages;
         p.hidden = hidden + static_cast<size_t>(r0) * H;
         p.session_ids = session_ids + r0;
@@ -991,9 +991,9 @@ int prepos_launch_ready_dist_w4(prepos_ctx *ctx, int n, const int32_t *session_i
         const size_t x_bytes = (static_cast<size_t>(p.x_rows) * (H + kW4XPad) * 2 + 15) & ~size_t(15);
         const size_t fixed = 1024 + x_bytes + 2 * kMaxStages * 8 + kConsumerWarps * kNB * sizeof(RdPartial) +
                              static_cast<size_t>(H / kW4Group) * kNB * sizeof(float);
+        if (fixed + 2 * static_cast<size_t>(kW4StageBytes) > 232448) return PREPOS_E_SHAPE;   // H too large for two stages
         int stages = static_cast<int>((232448 - fixed) / kW4StageBytes);
         if (stages > kMaxStages) stages = kMaxStages;
-        if (stages < 2) return PREPOS_E_SHAPE;
         p.n_stages = stages;
         p.hidden = hidden + static_cast<size_t>(r0) * H;
         p.session_ids = session_ids + r0;

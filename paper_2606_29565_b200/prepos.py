@@ -13,8 +13,8 @@ import os
 import torch
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-# PREPOS_LIB names another build of the same library (kernel tuning experiments); the default is the in-tree build
-_SO = os.environ.get("PREPOS_LIB") or os.path.join(_HERE, "libprepos.so")
+_SO = os.path.join(_HERE, "libprepos.so")   # the in-tree build, and nothing else
+ABI_VERSION = 101                            # PREPOS_VERSION of the include/prepos.h this binding marshals for
 
 OK, SKIPPED_BUDGET = 0, 1
 E_INVALID_ARG, E_SHAPE, E_ALIGN, E_CUDA, E_WORKSPACE, E_NO_DEVICE, E_FIXED_SCRATCH = -1, -2, -3, -4, -5, -6, -7
@@ -59,6 +59,9 @@ def lib() -> C.CDLL:
         L.prepos_strerror.restype = C.c_char_p
         L.prepos_strerror.argtypes = [i32]
         L.prepos_version.restype = i32
+        if L.prepos_version() != ABI_VERSION:
+            raise RuntimeError(f"{_SO} is version {L.prepos_version()}, this binding marshals for {ABI_VERSION}: "
+                               "rebuild it (`python -m paper_2606_29565_b200.build --force`)")
         L.prepos_workspace_bytes.restype = C.c_size_t
         L.prepos_workspace_bytes.argtypes = [C.POINTER(ModelShape), i32]
         L.prepos_ctx_create.restype = i32

@@ -34,7 +34,8 @@ def test_exports_every_declared_symbol(lib):
 
 def test_record_is_48_bytes_and_codes(lib):
     from paper_2606_29565_b200 import prepos
-    assert lib.prepos_version() == 100
+    hdr_version = int(re.search(r"#define PREPOS_VERSION (\d+)", open(os.path.join(ROOT, "include", "prepos.h")).read()).group(1))
+    assert lib.prepos_version() == hdr_version == prepos.ABI_VERSION    # the binding refuses any other build
     assert prepos.RECORD_BYTES == 48
     hdr = open(os.path.join(ROOT, "include", "prepos.h")).read()
     for name, val in (("PREPOS_SERVED", 0), ("PREPOS_GAP_BELOW_TAU", 1), ("PREPOS_NOT_IN_FAST_SET", 2),

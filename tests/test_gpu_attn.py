@@ -653,3 +653,93 @@ def test_two_contexts_one_launch_per_layer_on_two_streams(prepos, oracle):
         torch.cuda.synchronize()
         for k in (0, 1):
             check_attn(outs[k], refs[k], sbs[k])
+
+
+def _short_session_batch(seed):
+    """A config-4-like batch of SHORT sessions on the 8B shape: every session has at most 6 cached tiles + 1 entry
+    tile, so no segment of any CTA is 8 tiles long (the yield flag used to be re-read only at the 8th tile of a
+    segment)."""
+    shape = synth.C2
+    g = synth.gen(seed)
+    n = 64
+    n_s = torch.randint(128, 769, (n,), generator=g).tolist()
+    l_e = torch.randint(32, 65, (n,), generator=g).tolist()
+    return shape, synth.make_sessions(shape, n_s, l_e, seed=seed, device="cuda", extra_pages=1)
+
+
+def test_yield_flag_reaches_ctas_whose_segments_are_all_short(prepos):
+    """prepos_ctx_request_yield on a pass made of short segments only (64 sessions of 128..768 cached tokens, 32
+    layers: about a hundred segments per CTA, none of 8 tiles).  The CTAs count tiles across segments when they
+    re-read the flag, so the request is seen within 8 tiles of the CTA's stream: the pass must be caught pending in
+    at least one trial, and the resumed result is the uninterrupted one bit for bit."""
+    shape, sb = _short_session_batch(synth.SEED_BASE + 404)
+    k0, v0 = sb.k_pool.clone(), sb.v_pool.clone()
+    ctx = prepos.Context(shape.layers, shape.Hq, shape.Hkv, shape.d, shape.H, shape.V, shape.page, max_sessions=64)
+    ctx.set_attn_path(2)
+    ref = torch.empty_like(sb.q)
+    ctx.entry_attn(sb.q, sb.k_new, sb.v_new, sb.k_pool, sb.v_pool, sb.page_table, sb.n_s, sb.l_entry, sb.capacity, ref)
+    ctx.sync()
+    kref, vref = sb.k_pool.clone(), sb.v_pool.clone()
+    s_lo, s_hi = torch.cuda.Stream(priority=0), torch.cuda.Stream(priority=-1)
+    caught = 0
+    for trial in range(6):
+        sb.k_pool.copy_(k0)
+        sb.v_pool.copy_(v0)
+        out = torch.full(sb.q.shape, float("nan"), dtype=torch.bfloat16, device="cuda")
+        torch.cuda.synchronize()
+        with torch.cuda.stream(s_lo):
+            ctx.entry_attn(sb.q, sb.k_new, sb.v_new, sb.k_pool, sb.v_pool, sb.page_table, sb.n_s, sb.l_entry,
+                           sb.capacity, out)
+        with torch.cuda.stream(s_hi):
+            ctx.request_yield()
+        s_hi.synchronize()
+        with torch.cuda.stream(s_lo):
+            pending = ctx.entry_attn_pending()
+            caught += int(pending)
+            ctx.entry_attn_resume()
+            assert not ctx.entry_attn_pending()
+        torch.cuda.synchronize()
+        assert torch.equal(out.view(torch.int16), ref.view(torch.int16)), trial
+        assert torch.equal(sb.k_pool.view(torch.int16), kref.view(torch.int16))
+        assert torch.equal(sb.v_pool.view(torch.int16), vref.view(torch.int16))
+    assert caught >= 1, "the yield request never reached a pass of short segments"
+
+
+def test_late_yield_request_cannot_stop_a_later_pass(prepos):
+    """A yield request names the launch it is for.  Here the request for pass A sits behind 20 ms of other work on its
+    stream and lands long after A has ended -- after pass B on the same ctx has been issued as well.  Neither B nor the
+    pass C issued after the request has landed may be stopped by it: both run to completion (not pending) and give the
+    reference result.  (With a bare 0/1 flag the late copy landed after B's call had cleared the flag, and C -- and
+    every later call -- stopped at its first yield point while returning PREPOS_OK.)"""
+    shape = synth.C2
+    sb = synth.make_sessions(shape, [4096], [24], seed=synth.SEED_BASE + 405, device="cuda", extra_pages=1)
+    k0, v0 = sb.k_pool.clone(), sb.v_pool.clone()
+    ctx = prepos.Context(shape.layers, shape.Hq, shape.Hkv, shape.d, shape.H, shape.V, shape.page, max_sessions=1)
+    ref = torch.empty_like(sb.q)
+    ctx.entry_attn(sb.q, sb.k_new, sb.v_new, sb.k_pool, sb.v_pool, sb.page_table, sb.n_s, sb.l_entry, sb.capacity, ref)
+    ctx.sync()
+    s_lo, s_hi = torch.cuda.Stream(priority=0), torch.cuda.Stream(priority=-1)
+
+    def one_pass():
+        sb.k_pool.copy_(k0)
+        sb.v_pool.copy_(v0)
+        out = torch.full(sb.q.shape, float("nan"), dtype=torch.bfloat16, device="cuda")
+        ctx.entry_attn(sb.q, sb.k_new, sb.v_new, sb.k_pool, sb.v_pool, sb.page_table, sb.n_s, sb.l_entry, sb.capacity, out)
+        return out
+
+    with torch.cuda.stream(s_lo):
+        out_a = one_pass()                                   # pass A
+    with torch.cuda.stream(s_hi):
+        torch.cuda._sleep(40_000_000)                        # ~20 ms at 1.9 GHz: the request is stuck behind this
+        ctx.request_yield()                                  # meant for A
+    s_lo.synchronize()                                       # A has ended, the request has not landed yet
+    with torch.cuda.stream(s_lo):
+        out_b = one_pass()                                   # pass B, issued while the request is still in flight
+        assert not ctx.entry_attn_pending()
+    torch.cuda.synchronize()                                 # now the late request has landed
+    with torch.cuda.stream(s_lo):
+        out_c = one_pass()                                   # pass C
+        assert not ctx.entry_attn_pending()
+    torch.cuda.synchronize()
+    for name, o in (("A", out_a), ("B", out_b), ("C", out_c)):
+        assert torch.equal(o.view(torch.int16), ref.view(torch.int16)), name
