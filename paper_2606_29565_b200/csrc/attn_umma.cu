@@ -856,6 +856,7 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
             const int mt = (n_mt == 2) ? w : 0;
             const int urow = mt * 128 + row;                   // row within the unit
             const int my_tok = s.u.tok0 + urow / G;            // entry token of this row (if urow < rows)
+            const bool row_valid = urow < rows;
             float srow = p.scale_log2;   // kFp8: softmax scale x log2(e) x 2^-k of this thread's row
             if constexpr (kFp8) {
                 // Q arrived as bf16 (8 significant bits): split it exactly into two e4m3 operands, in place.  The thread
@@ -976,8 +977,11 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
                         mx = fmaxf(fmaxf(mx, m1), fmaxf(m2, m3));
                     }
                     const float m_new = fmaxf(m_used, mx * p.scale_log2);
-                    // lazy rescale, warp-uniform because the TMEM round trip of O is warp-collective
-                    const bool need = (m_new > m_used + kRescaleThreshold);
+                    // lazy rescale, warp-uniform because the TMEM round trip of O is warp-collective.  Only rows of the
+                    // unit vote: a row past them holds whatever the Q buffer held before (another segment's, or another
+                    // launch's after a resume), and its maximum must not decide WHEN the valid rows of its warp rescale
+                    // -- the result would stay within tolerance but depend on what ran on the SM before.
+                    const bool need = row_valid && (m_new > m_used + kRescaleThreshold);
                     if (__any_sync(0xffffffffu, need)) {
                         const float alpha = (m_used == -CUDART_INF_F) ? 0.f : exp2f(m_used - m_new);
                         l_sum *= alpha;
@@ -1064,7 +1068,7 @@ attn_umma_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant
                         if (mb != -CUDART_INF_F) mx = fmaxf(mx, mb * (scb[b] * srow));
                     }
                     const float m_new = fmaxf(m_used, mx);
-                    const bool need = (m_new > m_used + kRescaleThreshold);
+                    const bool need = row_valid && (m_new > m_used + kRescaleThreshold);   // as in tile_body: valid rows vote
                     if (__any_sync(0xffffffffu, need)) {
                         const float alpha = (m_used == -CUDART_INF_F) ? 0.f : exp2f(m_used - m_new);
                         l_sum *= alpha;

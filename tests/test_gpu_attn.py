@@ -743,3 +743,34 @@ def test_late_yield_request_cannot_stop_a_later_pass(prepos):
     torch.cuda.synchronize()
     for name, o in (("A", out_a), ("B", out_b), ("C", out_c)):
         assert torch.equal(o.view(torch.int16), ref.view(torch.int16)), name
+
+
+@pytest.mark.parametrize("shape_key,n_s,l_entry", [
+    ("d128_g2_l16", [3000, 1000, 500], [200, 130, 40]),      # stream-K cuts: units merged by their last arriver
+    ("d128_g4_l8",) + _many_small(30, 1),
+])
+def test_abandoned_sliced_pass_does_not_poison_the_next_call(prepos, shape_key, n_s, l_entry):
+    """`prepos_ctx_set_attn_slice(1)` stops a pass after one segment per CTA: units cut across CTAs have counted some
+    of their arrivals.  Issuing a NEW prepos_entry_attn instead of a resume abandons that pass; the new pass must
+    start from clean arrival counters (otherwise its last-arriver merge fires early, on incomplete partials, and
+    writes wrong rows without any error).  The new call's output equals an untouched ctx's bit for bit."""
+    shape = SHAPES[shape_key]
+    sb = synth.make_sessions(shape, n_s, l_entry, seed=777 + sum(n_s))
+    out_ref, kp_ref, vp_ref, _, status, ctx0 = _gpu_run(prepos, sb, 2, poison=False)
+    ctx0.close()
+    dev = "cuda"
+    ctx = _ctx(prepos, shape, sb.n_sessions, 2)
+    q, kn, vn, pt = sb.q.to(dev), sb.k_new.to(dev), sb.v_new.to(dev), sb.page_table.to(dev)
+    for rnd in range(2):
+        ctx.set_attn_slice(1)
+        kp, vp = sb.k_pool.to(dev).clone(), sb.v_pool.to(dev).clone()
+        junk = torch.full(sb.q.shape, float("nan"), dtype=torch.bfloat16, device=dev)
+        ctx.entry_attn(q, kn, vn, kp, vp, pt, sb.n_s, sb.l_entry, sb.capacity, junk)
+        assert ctx.entry_attn_pending()
+        ctx.set_attn_slice(0)                       # ... and never resumed
+        kp, vp = sb.k_pool.to(dev).clone(), sb.v_pool.to(dev).clone()
+        out = torch.full(sb.q.shape, float("nan"), dtype=torch.bfloat16, device=dev)
+        ctx.entry_attn(q, kn, vn, kp, vp, pt, sb.n_s, sb.l_entry, sb.capacity, out)
+        assert not ctx.entry_attn_pending()
+        assert torch.equal(out.view(torch.int16), out_ref.view(torch.int16)), rnd
+        assert torch.equal(kp.view(torch.int16), kp_ref.view(torch.int16)) and torch.equal(vp.view(torch.int16), vp_ref.view(torch.int16))

@@ -156,15 +156,16 @@ def test_fp8_config2_slice_sampled(prepos, oracle):
     assert np.array_equal(k8[1].cpu().numpy(), ok8[1]) and np.array_equal(v8[1].cpu().numpy(), ov8[1])
 
 
-@pytest.mark.parametrize("name", ["c2", "c5"])
+@pytest.mark.parametrize("name", ["c2", "c3", "c5"])
 def test_fp8_full_size_configs(prepos, oracle, name):
     """The FP8 pass at BASELINE's full sizes in the launch configuration bench.py times (tcgen05 FP8 kernel, every
     layer in one launch, sessions generated on the device with bench.py's seeds and quantised by the synthetic
-    quantiser): config 2 -- every output row of every layer; config 5 -- 64 seeded (layer, head, row) samples through
+    quantiser): configs 2 and 3 (n_s = 32768, L = 16: 64 query rows per unit, 256 tiles per unit, the one shape where
+    the FP8 pass is faster than the bf16 one) -- every output row of every layer; config 5 -- 64 seeded (layer, head, row) samples through
     the ranged O7; and on both the WHOLE code pools after the call: the codes Append(E) stored for every entry token
     of every layer equal the oracle's on the sampled layers, and no other byte moved."""
-    shape = synth.C2 if name == "c2" else synth.C5
-    n_s, l_e = ([4096], [24]) if name == "c2" else ([16384], [32])
+    shape = {"c2": synth.C2, "c3": synth.C3, "c5": synth.C5}[name]
+    n_s, l_e = {"c2": ([4096], [24]), "c3": ([32768], [16]), "c5": ([16384], [32])}[name]
     seed = synth.SEED_BASE + int(name[1])
     chunk = max(64, (1 << 28) // (shape.layers * shape.Hkv * shape.page * shape.d))
     sb = synth.make_sessions(shape, n_s, l_e, seed=seed, device="cuda")
@@ -193,7 +194,8 @@ def test_fp8_full_size_configs(prepos, oracle, name):
     rng = np.random.default_rng(seed)
     G = shape.G
     worst = 0.0
-    if name == "c2":
+    every_row = name in ("c2", "c3")
+    if every_row:
         layers = range(shape.layers)
     else:
         layers = sorted(set(int(x) for x in rng.integers(0, shape.layers, 8)))
@@ -202,7 +204,7 @@ def test_fp8_full_size_configs(prepos, oracle, name):
         v8 = v0[l, idx].cpu().numpy().copy()
         ks, vs = fb.k_scale[l, idx].cpu().numpy(), fb.v_scale[l, idx].cpu().numpy()
         q, kn, vn = bits(sb.q[l]), bits(sb.k_new[l]), bits(sb.v_new[l])
-        if name == "c2":
+        if every_row:
             ref = oracle.entry_attn_fp8(q, kn, vn, k8, v8, ks, vs, table, n_s[0], sb.capacity[0])
             worst = max(worst, float(np.abs(out[l].cpu().to(torch.float64).numpy() - ref["out"]).max()))
         else:
@@ -215,3 +217,52 @@ def test_fp8_full_size_configs(prepos, oracle, name):
         assert np.array_equal(fb.k_pool8[l, idx].cpu().numpy(), k8), f"K codes differ at layer {l}"
         assert np.array_equal(fb.v_pool8[l, idx].cpu().numpy(), v8), f"V codes differ at layer {l}"
     assert worst <= ATTN_ATOL, worst
+
+
+@pytest.mark.parametrize("shape_key,n_s,l_entry,slice_n", [
+    ("d128_g4_l8", [300, 150, 410, 90, 222, 377, 64, 199, 350, 120, 280, 333], [12, 40, 7, 33, 21, 16, 45, 9, 28, 3, 37, 24], 1),
+    ("d128_g1_l16", [2500, 700, 900], [300, 257, 129], 1),   # two row chunks per session; stream-K cuts inside units
+    ("d128_g4_l8", [60 + 37 * i % 400 for i in range(40)], [1 + 13 * i % 64 for i in range(40)], 2),   # 640 units on
+                                                             # 148 CTAs, up to 256 rows (two M-tiles), two segments a launch
+])
+def test_fp8_sliced_pass_and_resume_is_bit_identical(prepos, oracle, shape_key, n_s, l_entry, slice_n):
+    """The yield points of attn_umma_kernel<128, kFp8>: a pass that stops after `slice_n` segments per CTA and is resumed
+    until nothing is pending gives the uninterrupted call's outputs and code pools bit for bit (the FP8 path shares the
+    admission words, progress counters and merge of the bf16 path, but has its own producer warp and its own polling
+    site), and an unsliced call on the same ctx afterwards is unaffected."""
+    shape = SHAPES[shape_key]
+    fb = synth.make_sessions_fp8(shape, n_s, l_entry, seed=5151 + sum(n_s))
+    sb, dev = fb.base, "cuda"
+    out_ref, k_ref, v_ref, st_ref, ctx0 = _run(prepos, fb, 2)
+    ctx0.close()
+    ctx = prepos.Context(shape.layers, shape.Hq, shape.Hkv, shape.d, shape.H, shape.V, shape.page,
+                         max_sessions=max(sb.n_sessions, 1))
+    ctx.set_attn_path(2)
+    args = (sb.q.to(dev), sb.k_new.to(dev), sb.v_new.to(dev))
+    tail = (fb.k_scale.to(dev), fb.v_scale.to(dev), sb.page_table.to(dev), sb.n_s, sb.l_entry, sb.capacity)
+    k8, v8 = fb.k_pool8.to(dev).clone(), fb.v_pool8.to(dev).clone()
+    out = torch.full(sb.q.shape, float("nan"), dtype=torch.bfloat16, device=dev)
+    ctx.set_attn_slice(slice_n)
+    st = ctx.entry_attn_fp8(*args, k8, v8, *tail, out)
+    launches = 1
+    while ctx.entry_attn_pending():
+        ctx.entry_attn_resume()
+        launches += 1
+        assert launches < 500
+    assert launches >= 2, "the pass never stopped: the slice was not honoured"
+    assert st == st_ref
+    assert torch.equal(out.view(torch.int16), out_ref.view(torch.int16))
+    assert torch.equal(k8, k_ref) and torch.equal(v8, v_ref)
+    # a sliced pass that is ABANDONED after its first launch (a new call instead of a resume) must not leak its
+    # half-counted arrival counters into the new pass
+    k8b, v8b = fb.k_pool8.to(dev).clone(), fb.v_pool8.to(dev).clone()
+    junk = torch.full(sb.q.shape, float("nan"), dtype=torch.bfloat16, device=dev)
+    ctx.entry_attn_fp8(*args, k8b, v8b, *tail, junk)
+    assert ctx.entry_attn_pending()
+    ctx.set_attn_slice(0)
+    k8c, v8c = fb.k_pool8.to(dev).clone(), fb.v_pool8.to(dev).clone()
+    out2 = torch.full(sb.q.shape, float("nan"), dtype=torch.bfloat16, device=dev)
+    ctx.entry_attn_fp8(*args, k8c, v8c, *tail, out2)
+    assert not ctx.entry_attn_pending()
+    assert torch.equal(out2.view(torch.int16), out_ref.view(torch.int16))
+    assert torch.equal(k8c, k_ref) and torch.equal(v8c, v_ref)

@@ -312,11 +312,12 @@ def test_w4_extreme_codes_and_unit_scales(prepos, oracle):
         assert np.array_equal(logits[r].cpu().numpy().astype(np.float64), ref), r
 
 
-@pytest.mark.parametrize("name,n", [("c2", 1), ("c5", 4)])
+@pytest.mark.parametrize("name,n", [("c2", 1), ("c4", 64), ("c5", 4)])
 def test_w4_full_size_vocabulary(prepos, oracle, name, n):
     """The int4 LM head at BASELINE's vocabulary shapes (V = 128256, H = 4096 / 8192) in bench.py's launch
-    configuration: every logit of every row and the records against O8 + O3."""
-    shape = synth.C2 if name == "c2" else synth.C5
+    configuration: every logit of every row and the records against O8 + O3.  Config 4 is its 64-session batch:
+    eight passes of 8 rows over the codes."""
+    shape = {"c2": synth.C2, "c4": synth.C4, "c5": synth.C5}[name]
     seed = synth.SEED_BASE + int(name[1])
     w4, sc = synth.make_w_vocab_w4(shape, seed, "cuda")
     hidden = synth.randn_bf16((n, shape.H), synth.gen(seed + 1, "cuda"))
