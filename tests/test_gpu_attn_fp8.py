@@ -266,3 +266,56 @@ def test_fp8_sliced_pass_and_resume_is_bit_identical(prepos, oracle, shape_key, 
     assert not ctx.entry_attn_pending()
     assert torch.equal(out2.view(torch.int16), out_ref.view(torch.int16))
     assert torch.equal(k8c, k_ref) and torch.equal(v8c, v_ref)
+
+
+def test_one_ctx_alternating_bf16_and_fp8_pools_at_the_same_address(prepos):
+    """A ctx caches the TMA descriptors of the KV pools it was last given.  The bf16 pools take a 5-D map, the e4m3
+    pools a 3-D byte map, and for one geometry the bf16 layer stride in elements EQUALS the FP8 layer stride in bytes:
+    when an allocator hands the FP8 pools the address the bf16 pools had, (address, stride, pages) alone cannot tell
+    the two apart.  Here both precisions deliberately live at the same base address (views of one buffer) and one ctx
+    alternates between them; every call must give what a fresh ctx gives, bit for bit."""
+    shape = SHAPES["d128_g4"]
+    fb = synth.make_sessions_fp8(shape, [700, 15, 300], [24, 96, 64], seed=77)
+    sb, dev = fb.base, "cuda"
+    n_el = sb.k_pool.numel()
+    bufs = [torch.zeros(2 * n_el, dtype=torch.uint8, device=dev) for _ in range(2)]
+    q, kn, vn, pt = sb.q.to(dev), sb.k_new.to(dev), sb.v_new.to(dev), sb.page_table.to(dev)
+    ks, vs = fb.k_scale.to(dev), fb.v_scale.to(dev)
+
+    def pools_bf16():
+        kp, vp = (b.view(torch.bfloat16).view(sb.k_pool.shape) for b in bufs)
+        kp.copy_(sb.k_pool)
+        vp.copy_(sb.v_pool)
+        return kp, vp
+
+    def pools_fp8():
+        k8, v8 = (b[:n_el].view(fb.k_pool8.shape) for b in bufs)
+        k8.copy_(fb.k_pool8)
+        v8.copy_(fb.v_pool8)
+        return k8, v8
+
+    def run_bf16(ctx):
+        kp, vp = pools_bf16()
+        out = torch.full(sb.q.shape, float("nan"), dtype=torch.bfloat16, device=dev)
+        ctx.entry_attn(q, kn, vn, kp, vp, pt, sb.n_s, sb.l_entry, sb.capacity, out)
+        ctx.sync()
+        return out
+
+    def run_fp8(ctx):
+        k8, v8 = pools_fp8()
+        assert k8.data_ptr() == bufs[0].data_ptr() and k8.stride(0) == sb.k_pool.stride(0)   # same key as the bf16 pools
+        out = torch.full(sb.q.shape, float("nan"), dtype=torch.bfloat16, device=dev)
+        ctx.entry_attn_fp8(q, kn, vn, k8, v8, ks, vs, pt, sb.n_s, sb.l_entry, sb.capacity, out)
+        ctx.sync()
+        return out
+
+    def new_ctx():
+        c = prepos.Context(shape.layers, shape.Hq, shape.Hkv, shape.d, shape.H, shape.V, shape.page, max_sessions=3)
+        c.set_attn_path(2)
+        return c
+
+    ref16, ref8 = run_bf16(new_ctx()), run_fp8(new_ctx())
+    ctx = new_ctx()
+    for rnd in range(2):
+        assert torch.equal(run_bf16(ctx).view(torch.int16), ref16.view(torch.int16)), rnd
+        assert torch.equal(run_fp8(ctx).view(torch.int16), ref8.view(torch.int16)), rnd
